@@ -1,0 +1,342 @@
+"""Plain, slow, obviously-correct CPU oracle of the RT-TDDFT time step (arXiv 2410.09189).
+
+TEST INFRASTRUCTURE.  NumPy, FP64 / complex128, no blocking, no fusion, no code shared with the CUDA
+path.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py`` (cpu_baseline / --impl reference)
+may import it.  Citations are ``PAPER.md:L<line>`` (the paper text under /root/reference) plus the
+equation / algorithm line; "DESIGN R<n>" is a reading listed in DESIGN.md where the paper is silent.
+
+What is computed (one step, Algorithm 1 lines 9-29, with the dynamic `while`
+loops replaced by fixed counts, DESIGN R1):
+
+    H1 = 2 H0 - H-1                                      (Alg. 1 line 11, L365)
+    repeat m times:
+        Hbar = (H0 + H1)/2                               (Eq. 12; Alg. 1 line 14, L373)
+        U    = W exp(-i w dt) W^T,  Hbar = W w W^T       (spectral form, L129, L147: exact)
+        P1   = U P0 U^dagger                             (Eq. 15)
+        rho  = sum_ij Re(P1)_ij phi_i phi_j              (Eq. 27, Gamma point, real orbitals)
+        V_H  = MG(V_H, 4 pi (drho - mean drho), n_vc)    (multigrid, L77; concrete cycle DESIGN R6)
+        dV   = V_H + vxc(rho) - vxc(rho0) + E.x          (V_eff terms, L73-L75; length gauge, L325, L412)
+        H1   = diag(eps) + dVol * Phi diag(dV) Phi^T     (Alg. 1 line 25, L395; Eq. 4)
+    mu = dVol sum_r x(r) rho(r)                          (Alg. 1 line 27, L400)
+    H-1, H0, P0 <- H0, H1, P1                            (Alg. 1 line 28, L403)
+
+Parity pins (tests/test_oracle_*.py): zero-field stationarity, tr P = N_e, P Hermitian and P^2 = 2P,
+closed-form non-interacting propagation, energy conservation, linear/odd response, commutator series
+(Eq. 39) == eigh propagator (L426), converged multigrid == FFT solution of the same stencil,
+continuum Gaussian-charge potential (Ewald closed form) with O(h^2) convergence, v_xc = d(rho e_xc)/d rho
+and textbook uniform-gas constants, brute-force projection/density on tiny inputs.
+Unpinned by anything outside this file: the *value* of the fixed-cycle (unconverged) V_H -- it is
+"parity to the definition" (DESIGN R6); everything it converges to is pinned.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+# --------------------------------------------------------------------------------------------------
+# Grid, field
+# --------------------------------------------------------------------------------------------------
+
+def axis_coords(n: int, h: float) -> np.ndarray:
+    """Centred sawtooth coordinate x(i) = (i - (n-1)/2) h  (length gauge, "sawtooth-like
+    potential"; no vacuum dipole correction, DESIGN R4).  Sum_i x(i) = 0."""
+    return (np.arange(n, dtype=np.float64) - 0.5 * (n - 1)) * h
+
+
+def field_potential(shape, h: float, E) -> np.ndarray:
+    """V_ext(r) = E . r on the grid, r = (x(ix), y(iy), z(iz)); flat index (ix*ny + iy)*nz + iz."""
+    nx, ny, nz = shape
+    x, y, z = axis_coords(nx, h), axis_coords(ny, h), axis_coords(nz, h)
+    v = E[0] * x[:, None, None] + E[1] * y[None, :, None] + E[2] * z[None, None, :]
+    return np.ascontiguousarray(np.broadcast_to(v, shape)).reshape(-1)
+
+
+# --------------------------------------------------------------------------------------------------
+# LDA exchange-correlation: Slater exchange + Perdew-Zunger 1981 correlation, unpolarised (DESIGN R7;
+# the paper ran PBE; north_star fixes LDA).  Hartree atomic units.
+# --------------------------------------------------------------------------------------------------
+PZ_GAMMA, PZ_BETA1, PZ_BETA2 = -0.1423, 1.0529, 0.3334
+PZ_A, PZ_B, PZ_C, PZ_D = 0.0311, -0.048, 0.0020, -0.0116
+RHO_FLOOR = 1e-30
+RHO_RS1 = 3.0 / (4.0 * np.pi)      # density at which r_s = 1; branch is taken on rho (DESIGN R7)
+
+
+def _rs(rho):
+    return (3.0 / (4.0 * np.pi * rho)) ** (1.0 / 3.0)
+
+
+def vxc_lda(rho: np.ndarray) -> np.ndarray:
+    """v_xc(rho) = v_x + v_c.  v_x = -(3 rho/pi)^(1/3).  rho <= RHO_RS1 (r_s >= 1):
+    v_c = eps_c (1 + 7/6 b1 sqrt(rs) + 4/3 b2 rs)/(1 + b1 sqrt(rs) + b2 rs); else
+    v_c = A ln rs + (B - A/3) + 2/3 C rs ln rs + (2D - C)/3 rs.   rho < RHO_FLOOR -> 0."""
+    rho = np.asarray(rho, dtype=np.float64)
+    out = np.zeros_like(rho)
+    ok = rho >= RHO_FLOOR
+    r = rho[ok]
+    rs = _rs(r)
+    vx = -np.cbrt(3.0 * r / np.pi)
+    lo = r <= RHO_RS1
+    vc = np.empty_like(r)
+    s = np.sqrt(rs[lo])
+    den = 1.0 + PZ_BETA1 * s + PZ_BETA2 * rs[lo]
+    ec = PZ_GAMMA / den
+    vc[lo] = ec * (1.0 + (7.0 / 6.0) * PZ_BETA1 * s + (4.0 / 3.0) * PZ_BETA2 * rs[lo]) / den
+    hi = ~lo
+    ln = np.log(rs[hi])
+    vc[hi] = PZ_A * ln + (PZ_B - PZ_A / 3.0) + (2.0 / 3.0) * PZ_C * rs[hi] * ln + ((2.0 * PZ_D - PZ_C) / 3.0) * rs[hi]
+    out[ok] = vx + vc
+    return out
+
+
+def exc_density_lda(rho: np.ndarray) -> np.ndarray:
+    """e_xc(rho) = rho (eps_x + eps_c) per unit volume (energy check only).  eps_x = 3/4 v_x."""
+    rho = np.asarray(rho, dtype=np.float64)
+    out = np.zeros_like(rho)
+    ok = rho >= RHO_FLOOR
+    r = rho[ok]
+    rs = _rs(r)
+    ex = -0.75 * np.cbrt(3.0 * r / np.pi)
+    lo = r <= RHO_RS1
+    ec = np.empty_like(r)
+    ec[lo] = PZ_GAMMA / (1.0 + PZ_BETA1 * np.sqrt(rs[lo]) + PZ_BETA2 * rs[lo])
+    hi = ~lo
+    ln = np.log(rs[hi])
+    ec[hi] = PZ_A * ln + PZ_B + PZ_C * rs[hi] * ln + PZ_D * rs[hi]
+    out[ok] = r * (ex + ec)
+    return out
+
+
+# --------------------------------------------------------------------------------------------------
+# Hartree: periodic 7-point Poisson, fixed count of V(nu1,nu2) cycles, weighted Jacobi (DESIGN R6)
+# --------------------------------------------------------------------------------------------------
+
+def apply_A(u: np.ndarray, h: float) -> np.ndarray:
+    """A u = -lap_h u = (6 u - sum of the 6 periodic neighbours)/h^2."""
+    nb = (np.roll(u, 1, 0) + np.roll(u, -1, 0) + np.roll(u, 1, 1) + np.roll(u, -1, 1)
+          + np.roll(u, 1, 2) + np.roll(u, -1, 2))
+    return (6.0 * u - nb) / (h * h)
+
+
+def jacobi_sweep(u: np.ndarray, f: np.ndarray, h: float, omega: float) -> np.ndarray:
+    """u <- u + omega D^-1 (f - A u), D = 6/h^2  ==  (1-omega) u + (omega/6)(h^2 f + sum_nb u)."""
+    nb = (np.roll(u, 1, 0) + np.roll(u, -1, 0) + np.roll(u, 1, 1) + np.roll(u, -1, 1)
+          + np.roll(u, 1, 2) + np.roll(u, -1, 2))
+    return (1.0 - omega) * u + (omega / 6.0) * (h * h * f + nb)
+
+
+def restrict_full_weighting(r: np.ndarray) -> np.ndarray:
+    """Tensor-product (1/4, 1/2, 1/4) full weighting; coarse point I sits on fine point 2I (periodic)."""
+    for ax in range(3):
+        r = 0.25 * np.roll(r, 1, ax) + 0.5 * r + 0.25 * np.roll(r, -1, ax)
+        r = np.take(r, np.arange(0, r.shape[ax], 2), axis=ax)
+    return r
+
+
+def prolong_trilinear(e: np.ndarray) -> np.ndarray:
+    """Tensor-product linear interpolation: fine 2I <- coarse I ; fine 2I+1 <- (coarse I + coarse I+1)/2."""
+    for ax in range(3):
+        n = e.shape[ax]
+        shp = list(e.shape)
+        shp[ax] = 2 * n
+        f = np.empty(shp, dtype=np.float64)
+        ev = [slice(None)] * 3
+        od = [slice(None)] * 3
+        ev[ax] = slice(0, 2 * n, 2)
+        od[ax] = slice(1, 2 * n, 2)
+        f[tuple(ev)] = e
+        f[tuple(od)] = 0.5 * (e + np.roll(e, -1, ax))
+        e = f
+    return e
+
+
+def lambda_1d(n: int, h: float) -> np.ndarray:
+    """Eigenvalues of the periodic 1-D operator (2 u_i - u_{i-1} - u_{i+1})/h^2: (2 - 2 cos 2 pi k/n)/h^2."""
+    return (2.0 - 2.0 * np.cos(2.0 * np.pi * np.arange(n) / n)) / (h * h)
+
+
+def spectral_solve(f: np.ndarray, h: float) -> np.ndarray:
+    """Exact solve of A u = f in the zero-mean subspace via the analytic eigenpairs (FFT)."""
+    nx, ny, nz = f.shape
+    lam = (lambda_1d(nx, h)[:, None, None] + lambda_1d(ny, h)[None, :, None] + lambda_1d(nz, h)[None, None, :])
+    fh = np.fft.fftn(f)
+    lam[0, 0, 0] = 1.0
+    uh = fh / lam
+    uh[0, 0, 0] = 0.0
+    return np.real(np.fft.ifftn(uh))
+
+
+def can_coarsen(shape) -> bool:
+    """Coarsen while every dimension is even and > 4 (DESIGN R6)."""
+    return all((n % 2 == 0) and (n > 4) for n in shape)
+
+
+def mg_level_shapes(shape):
+    shapes = [tuple(shape)]
+    while can_coarsen(shapes[-1]):
+        shapes.append(tuple(n // 2 for n in shapes[-1]))
+    return shapes
+
+
+def vcycle(u: np.ndarray, f: np.ndarray, h: float, nu1: int, nu2: int, omega: float) -> np.ndarray:
+    if not can_coarsen(u.shape):
+        return spectral_solve(f, h)                       # coarsest level: exact, zero-mean
+    for _ in range(nu1):
+        u = jacobi_sweep(u, f, h, omega)
+    r = f - apply_A(u, h)
+    fc = restrict_full_weighting(r)
+    ec = vcycle(np.zeros_like(fc), fc, 2.0 * h, nu1, nu2, omega)   # rediscretised, zero initial guess
+    u = u + prolong_trilinear(ec)
+    for _ in range(nu2):
+        u = jacobi_sweep(u, f, h, omega)
+    return u
+
+
+def hartree_mg(VH: np.ndarray, drho: np.ndarray, shape, h: float, n_vc: int,
+               nu1: int = 2, nu2: int = 2, omega: float = 6.0 / 7.0) -> np.ndarray:
+    """n_vc V-cycles on  -lap_h V_H = 4 pi (drho - mean drho), warm-started from VH (flat arrays)."""
+    f = 4.0 * np.pi * (drho - np.mean(drho))
+    u = VH.reshape(shape)
+    f = f.reshape(shape)
+    for _ in range(n_vc):
+        u = vcycle(u, f, h, nu1, nu2, omega)
+    return u.reshape(-1)
+
+
+# --------------------------------------------------------------------------------------------------
+# Grid <-> matrix contractions (Eq. 4 quadrature rule)
+# --------------------------------------------------------------------------------------------------
+
+def project(Phi: np.ndarray, v: np.ndarray, dVol: float) -> np.ndarray:
+    """<phi_i| v |phi_j> = dVol sum_r phi_i(r) v(r) phi_j(r)   (Phi is [N][Ng])."""
+    return dVol * ((Phi * v[None, :]) @ Phi.T)
+
+
+def density(Phi: np.ndarray, ReP: np.ndarray) -> np.ndarray:
+    """rho(r) = sum_ij Re(P)_ij phi_i(r) phi_j(r)  (Im P is antisymmetric and drops out for real phi)."""
+    return np.sum((ReP @ Phi) * Phi, axis=0)
+
+
+def dipole(rho: np.ndarray, shape, h: float) -> np.ndarray:
+    """mu_q = dVol sum_r x_q(r) rho(r)  (= tr(P M_q), Alg. 1 line 27 with mu_0 folded in, DESIGN R3)."""
+    nx, ny, nz = shape
+    r3 = rho.reshape(shape)
+    dVol = h ** 3
+    return dVol * np.array([
+        np.sum(axis_coords(nx, h)[:, None, None] * r3),
+        np.sum(axis_coords(ny, h)[None, :, None] * r3),
+        np.sum(axis_coords(nz, h)[None, None, :] * r3)])
+
+
+# --------------------------------------------------------------------------------------------------
+# Propagators
+# --------------------------------------------------------------------------------------------------
+
+def propagator_eigh(Hbar: np.ndarray, dt: float) -> np.ndarray:
+    """U = exp(-i Hbar dt) = W exp(-i w dt) W^T by exact diagonalisation."""
+    w, W = np.linalg.eigh(Hbar)
+    return (W * np.exp(-1j * w * dt)[None, :]) @ W.T
+
+
+def propagate_eigh(Hbar: np.ndarray, P0: np.ndarray, dt: float) -> np.ndarray:
+    """P1 = U P0 U^dagger (Eq. 15)."""
+    U = propagator_eigh(Hbar, dt)
+    return U @ P0 @ U.conj().T
+
+
+def propagate_commutator(Hbar: np.ndarray, P0: np.ndarray, dt: float, dP_thrs: float = 1e-14,
+                         kmax: int = 200):
+    """The paper's own propagator, Eq. 39 (L310-L319) / Alg. 1 lines 15-23 (L375-L390) with S = 1:
+    dP^(k) = (1/k)(-i dt)[Hbar, dP^(k-1)],  P1 = P0 + sum_k dP^(k), until max|dP^(k)| <= dP_thrs.
+    Garbled lines 17/19 of the listing read as k <- 0, dP <- P0 / k <- k+1 (DESIGN R2).
+    Used only as an independent cross-check of propagate_eigh (L426).  Returns (P1, k)."""
+    P1 = P0.astype(np.complex128).copy()
+    dP = P0.astype(np.complex128).copy()
+    k = 0
+    err = 2.0 * dP_thrs
+    while err > dP_thrs and k < kmax:
+        k += 1
+        dP = (-1j * dt / k) * (Hbar @ dP - dP @ Hbar)
+        P1 = P1 + dP
+        err = np.max(np.abs(dP))
+    return P1, k
+
+
+# --------------------------------------------------------------------------------------------------
+# The time stepper
+# --------------------------------------------------------------------------------------------------
+
+class RTOracle:
+    """State machine with the same time semantics as the C-ABI (include/rt_tddft.h).
+
+    After construction t = 0, P = diag(occ), rho = rho0, V_H = 0, H0 = H-1 = diag(eps) + Proj(E0.x)
+    (Alg. 1 lines 7-8, L355-L358; delta-kick sampled at the end points, DESIGN R5).  ``step()`` uses
+    the field set by the last ``set_field`` (default 0) as E(t_{n+1}).
+    """
+
+    def __init__(self, shape, h, Phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2,
+                 nu_pre=2, nu_post=2, omega=6.0 / 7.0, hartree=True, xc=True):
+        self.shape = tuple(int(n) for n in shape)
+        self.h = float(h)
+        self.dVol = self.h ** 3
+        self.Phi = np.asarray(Phi, dtype=np.float64)
+        self.N, self.Ng = self.Phi.shape
+        assert self.Ng == int(np.prod(self.shape))
+        self.eps = np.asarray(eps, dtype=np.float64).copy()
+        self.occ = np.asarray(occ, dtype=np.float64).copy()
+        self.dt = float(dt)
+        self.m, self.n_vc = int(n_hupdates), int(n_vcycles)
+        self.nu1, self.nu2, self.omega = int(nu_pre), int(nu_post), float(omega)
+        self.hartree, self.xc = bool(hartree), bool(xc)
+        self.t = 0.0
+        self.P0 = np.diag(self.occ).astype(np.complex128)
+        self.rho0 = density(self.Phi, np.diag(self.occ))
+        self.rho = self.rho0.copy()
+        self.vxc0 = vxc_lda(self.rho0) if self.xc else np.zeros(self.Ng)
+        self.VH = np.zeros(self.Ng)
+        self.E_next = np.zeros(3)
+        self.H0 = np.diag(self.eps) + project(self.Phi, field_potential(self.shape, self.h, np.asarray(E0, float)), self.dVol)
+        self.Hm1 = self.H0.copy()
+
+    def set_field(self, E):
+        self.E_next = np.asarray(E, dtype=np.float64).copy()
+
+    def delta_v(self, rho):
+        """dV(r) = V_H[drho] + v_xc(rho) - v_xc(rho0) + E(t_{n+1}).x ; updates the warm-started V_H."""
+        dv = field_potential(self.shape, self.h, self.E_next)
+        if self.hartree:
+            self.VH = hartree_mg(self.VH, rho - self.rho0, self.shape, self.h, self.n_vc,
+                                 self.nu1, self.nu2, self.omega)
+            dv = dv + self.VH
+        if self.xc:
+            dv = dv + vxc_lda(rho) - self.vxc0
+        return dv
+
+    def step(self, nsteps: int = 1):
+        for _ in range(nsteps):
+            H1 = 2.0 * self.H0 - self.Hm1                                  # Alg. 1 line 11
+            for _it in range(self.m):                                      # lines 13-26, fixed m
+                Hbar = 0.5 * (self.H0 + H1)                                # line 14 / Eq. 12
+                P1 = propagate_eigh(Hbar, self.P0, self.dt)                # Eq. 15
+                rho = density(self.Phi, P1.real)                           # Eq. 27
+                H1 = np.diag(self.eps) + project(self.Phi, self.delta_v(rho), self.dVol)   # line 25
+            self.rho = rho
+            self.Hm1, self.H0, self.P0 = self.H0, H1, P1                   # line 28
+            self.t += self.dt
+
+    def dipole(self):
+        return dipole(self.rho, self.shape, self.h)                        # line 27
+
+    def density(self):
+        return self.rho
+
+    def energy(self):
+        """E = sum_i eps_i Re P_ii + 1/2 dVol sum drho V_H + dVol sum [e_xc(rho) - e_xc(rho0) - vxc0 drho]
+        (+ dVol sum E.x drho while a field is on).  Its functional derivative w.r.t. rho is delta_v, so it
+        is conserved by the exact dynamics when E = 0 (test aid; uses the current, unconverged V_H)."""
+        drho = self.rho - self.rho0
+        e = float(np.sum(self.eps * np.real(np.diag(self.P0))))
+        if self.hartree:
+            e += 0.5 * self.dVol * float(np.sum(drho * self.VH))
+        if self.xc:
+            e += self.dVol * float(np.sum(exc_density_lda(self.rho) - exc_density_lda(self.rho0) - self.vxc0 * drho))
+        e += self.dVol * float(np.sum(field_potential(self.shape, self.h, self.E_next) * drho))
+        return e
