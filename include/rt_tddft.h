@@ -1,0 +1,148 @@
+/* rt_tddft.h -- C ABI of the B200-native RT-TDDFT time step (arXiv 2410.09189, "RMG" RT-TDDFT).
+ *
+ * The library propagates the one-particle density matrix P(t) in the basis of N real ground-state
+ * Kohn-Sham orbitals Phi sampled on a periodic uniform grid ("orthogonal basis set for
+ * density matrix propagation", overlap = identity; Gamma point, L337).  One rt_step is Algorithm 1 lines
+ * 10-28 with the two dynamic `while` loops replaced by fixed counts (DESIGN R1, R8):
+ *
+ *   H1 = 2 H0 - H-1                                   line 11
+ *   repeat n_hupdates times:                          lines 13-26
+ *     Hbar = (H0 + H1)/2 ; U = exp(-i Hbar dt)        line 14, Eq. 12 (L123); series of real FP64 GEMMs
+ *     P1 = U P0 U^dagger                              Eq. 15 (L143-L145)
+ *     rho(r) = sum_ij Re(P1)_ij phi_i(r) phi_j(r)     Eq. 27 (L232)
+ *     V_H <- n_vcycles V-cycles on -lap V_H = 4 pi (rho - rho0 - mean)   ("Vh", Table 1; DESIGN R6)
+ *     dV = V_H + vxc(rho) - vxc(rho0) + E(t+dt).r     ("exchange/correlation", L547; length gauge L325)
+ *     H1 = diag(eps) + dVol Phi diag(dV) Phi^T        line 25 ("Hupdate", L543; quadrature Eq. 4)
+ *   mu = dVol sum_r r rho(r)                          line 27
+ *   H-1 <- H0 ; H0 <- H1 ; P0 <- P1                   line 28
+ *
+ * Conventions
+ *   - Grid: periodic nx x ny x nz, flat index r = (ix*ny + iy)*nz + iz (z fastest), Ng = nx*ny*nz, dVol = h^3.
+ *     Coordinates are the centred sawtooth x(ix) = (ix - (nx-1)/2) h (DESIGN R4).
+ *   - Phi is row-major [norb][Ng] FP64 (orbital-major, grid index contiguous), dVol*sum_r phi_i phi_j = delta_ij.
+ *   - All N x N matrices are row-major FP64; complex P is passed as separate real / imaginary planes.
+ *   - Every pointer argument is documented as HOST, DEVICE or EITHER (EITHER = any pointer cudaMemcpy with
+ *     cudaMemcpyDefault accepts; the copy is stream-ordered and the call returns after it has completed).
+ *   - Every function returns RT_OK (0) or a negative code; no exceptions, no exit(); rt_last_error gives text.
+ *     A CUDA error poisons the handle: later calls return RT_ESTATE.
+ *   - Nothing is allocated inside rt_step; all workspaces are created in rt_create.
+ *   - There is no CPU fallback: without an sm_100 device rt_create returns RT_ECUDA.
+ */
+#ifndef RT_TDDFT_H
+#define RT_TDDFT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RT_OK       0
+#define RT_EINVAL  -1   /* bad argument / unsupported shape            */
+#define RT_ENOMEM  -2   /* not enough device memory for the workspaces */
+#define RT_ECUDA   -3   /* CUDA runtime error (message in rt_last_error) */
+#define RT_ESTATE  -4   /* handle poisoned by an earlier error, or NULL */
+
+/* rt_config.flags */
+#define RT_PHI_DEVICE  1u   /* `phi` is a DEVICE pointer that the library BORROWS (never copies, never writes)
+                               for the lifetime of the handle; otherwise phi is HOST memory and is copied   */
+#define RT_NO_HARTREE  2u   /* test aid: drop V_H from dV                                                */
+#define RT_NO_XC       4u   /* test aid: drop vxc(rho) - vxc(rho0) from dV                               */
+#define RT_NO_GRAPH    8u   /* launch kernels directly instead of replaying a CUDA graph of one step     */
+
+typedef struct rt_ctx* rt_handle;
+
+typedef struct {
+  int32_t  nx, ny, nz;      /* periodic grid, each >= 2; Ng = nx*ny*nz                                       */
+  double   h;               /* spacing (bohr) > 0                                                            */
+  int32_t  norb;            /* N = N_occ + N_virt >= 1 (Alg. 1 line 2)                                       */
+  double   dt;              /* time step (a.u.) > 0                                                          */
+  int32_t  n_hupdates;      /* m >= 1 Hamiltonian updates per step; 0 -> 2                   */
+  int32_t  n_vcycles;       /* V-cycles per Poisson solve >= 0; there are m solves per step (DESIGN R9)      */
+  int32_t  nu_pre, nu_post; /* Jacobi sweeps before / after the coarse correction; 0,0 -> 2,2                */
+  double   jacobi_omega;    /* damping; 0 -> 6/7                                                             */
+  int32_t  exp_order;       /* K = degree in X of the Taylor polynomial of exp(-iX); 0 -> chosen from the
+                               spectral bound so that the truncation term <= 1e-17 (DESIGN R8)               */
+  double   E0[3];           /* field in force at t = 0 (the delta-"kick", Eq. 41, DESIGN R5)            */
+  uint32_t flags;           /* RT_* flags above                                                              */
+  int32_t  device;          /* CUDA device ordinal                                                           */
+  void*    stream;          /* cudaStream_t all work is enqueued on (e.g. torch.cuda.current_stream()); NULL = legacy default */
+} rt_config;
+
+/* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
+ * H0 = H-1 = diag(eps) + Proj(E0.r).   phi: [norb][Ng] HOST (copied) or DEVICE (borrowed, RT_PHI_DEVICE);
+ * eps, occ: [norb] HOST, copied; occ in [0,2].  *out receives the handle (owned by the caller -> rt_destroy). */
+int rt_create(const rt_config* cfg, const double* phi, const double* eps, const double* occ, rt_handle* out);
+
+/* Field E(t_{n+1}) used by the following step(s): HOST double[3]; sticky; default (0,0,0). */
+int rt_set_field(rt_handle h, const double E[3]);
+
+/* Enqueue nsteps >= 0 time steps on the stream.  Does not synchronise the host. */
+int rt_step(rt_handle h, int32_t nsteps);
+
+/* Dipole mu[3] (HOST) at the current time: dVol sum_r r rho(r) (Alg. 1 line 27).  Synchronises the stream. */
+int rt_get_dipole(rt_handle h, double mu[3]);
+
+/* Density rho(r) at the current time into rho[Ng] (EITHER).  Synchronises the stream. */
+int rt_get_density(rt_handle h, double* rho);
+
+/* ---- diagnostics / test aids ------------------------------------------------------------------ */
+
+/* P(t) = re + i im, each [norb][norb] (EITHER; either pointer may be NULL).  Synchronises. */
+int rt_get_pmatrix(rt_handle h, double* re, double* im);
+/* H0 (the Hamiltonian at the current time, [norb][norb], EITHER).  Synchronises. */
+int rt_get_hmatrix(rt_handle h, double* H0);
+/* Warm-start Hartree potential V_H[Ng] (EITHER).  Synchronises. */
+int rt_get_vhartree(rt_handle h, double* vh);
+/* Current time t (HOST). */
+int rt_get_time(rt_handle h, double* t);
+/* Integrals of the current density, HOST double[2]: { dVol sum rho , dVol sum (rho - rho0) }.  Synchronises. */
+int rt_get_charge(rt_handle h, double q[2]);
+/* info[0] = exp_order K actually used, info[1] = number of multigrid levels, info[2..4] = coarsest nx,ny,nz,
+ * info[5] = 1 if steps replay a CUDA graph, info[6] = kernels launched per step, info[7] = split-K of the
+ * projection.  HOST int32[8]. */
+int rt_get_info(rt_handle h, int32_t info[8]);
+/* Total number of this library's kernel launches enqueued through the handle so far (graph replays count the
+ * kernels inside the graph).  HOST. */
+int rt_get_launch_count(rt_handle h, int64_t* n);
+/* Text of the last error on this handle (or of the last failed rt_create when h == NULL).  Never NULL. */
+const char* rt_last_error(rt_handle h);
+/* Frees every workspace (not a borrowed phi).  NULL is accepted. */
+int rt_destroy(rt_handle h);
+
+/* ---- per-stage entry points: the rows of the hot path one at a time (parity tests, roofline timing) ----
+ * They use the handle's Phi, grid, stream and scratch space but do NOT touch the propagation state
+ * (P, H history, V_H, t).  All enqueue on the stream and synchronise before returning. */
+
+/* a1 "Hupdate": out[N][N] = dVol * Phi diag(v) Phi^T   (v[Ng], out: EITHER).  Eq. 4 (L68-L71), Alg. 1 line 25. */
+int rt_op_project(rt_handle h, const double* v, double* out);
+/* a5 "Rho" + a6: rho[Ng] = sum_ij S_ij phi_i phi_j for a real SYMMETRIC S[N][N] (reP, rho: EITHER);
+ * sums (HOST double[5], may be NULL) = { sum rho, sum x rho, sum y rho, sum z rho, sum (rho - rho0) } (no dVol). */
+int rt_op_density(rt_handle h, const double* reP, double* rho, double sums[5]);
+/* a2-a4 "ELDYN": P1 = U P0 U^dagger with U = exp(-i Hbar dt), Hbar real symmetric, P0 Hermitian
+ * (all [N][N], EITHER).  Eq. 12 (L123), Eq. 15 (L143). */
+int rt_op_propagate(rt_handle h, const double* Hbar, const double* P0re, const double* P0im,
+                    double* P1re, double* P1im);
+/* a7 "Vh": n_vc V-cycles on -lap_h V = 4 pi (drho - mean drho), warm-started from vh (in/out) (EITHER). */
+int rt_op_hartree(rt_handle h, double* vh, const double* drho, int32_t n_vc);
+/* a8 "exchange/correlation": vxc[Ng] = Slater + PZ81 potential of rho[Ng] (EITHER). */
+int rt_op_vxc(rt_handle h, const double* rho, double* vxc);
+
+/* ---- per-stage timing (CUDA events on the launching stream) ------------------------------------
+ * Stage ids follow Table 1 (L543-L547) plus the rest of the step. */
+#define RT_STAGE_HUPDATE 0   /* a1 projection (+ split-K reduce)          */
+#define RT_STAGE_RHO     1   /* a5 density (+ partial reduce, a6 dipole)  */
+#define RT_STAGE_VH      2   /* a7 multigrid Poisson                      */
+#define RT_STAGE_ELDYN   3   /* a2-a4 mean Hamiltonian, exp series, UPU^+ */
+#define RT_STAGE_XC      4   /* a8 vxc + dV assembly                      */
+#define RT_STAGE_COUNT   5
+/* enable != 0: later rt_step calls bracket every stage with cudaEvents (and bypass the CUDA graph). */
+int rt_timing_enable(rt_handle h, int32_t enable);
+/* Synchronises; ms[RT_STAGE_COUNT] (HOST) = accumulated device milliseconds per stage since the last call,
+ * calls[RT_STAGE_COUNT] (HOST) = number of times each stage ran.  Resets the accumulators. */
+int rt_timing_read(rt_handle h, double ms[RT_STAGE_COUNT], int64_t calls[RT_STAGE_COUNT]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RT_TDDFT_H */

@@ -1,0 +1,300 @@
+"""Thin ctypes binding of include/rt_tddft.h -- argument marshalling only; every step of the path runs in the
+CUDA kernels of librt_tddft.so.  Function names equal the C names.  PyTorch is used by callers for device
+memory and streams; this module itself only needs ctypes (+ numpy for host buffers).
+
+There is NO CPU fallback: importing this module raises if the library has not been built
+(``python -m paper_2410_09189_b200.build``), and rt_create fails without an sm_100 GPU.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librt_tddft.so")
+
+RT_OK, RT_EINVAL, RT_ENOMEM, RT_ECUDA, RT_ESTATE = 0, -1, -2, -3, -4
+RT_PHI_DEVICE, RT_NO_HARTREE, RT_NO_XC, RT_NO_GRAPH = 1, 2, 4, 8
+RT_STAGE_NAMES = ("Hupdate", "Rho", "Vh", "ELDYN", "XC")      # Table 1 of the paper, L543-L547
+RT_STAGE_COUNT = 5
+
+# every symbol include/rt_tddft.h declares (checked by tests/test_abi.py)
+SYMBOLS = (
+    "rt_create", "rt_set_field", "rt_step", "rt_get_dipole", "rt_get_density", "rt_get_pmatrix", "rt_get_hmatrix",
+    "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
+    "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
+    "rt_timing_enable", "rt_timing_read",
+)
+
+
+class rt_config(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+        ("h", C.c_double),
+        ("norb", C.c_int32),
+        ("dt", C.c_double),
+        ("n_hupdates", C.c_int32), ("n_vcycles", C.c_int32),
+        ("nu_pre", C.c_int32), ("nu_post", C.c_int32),
+        ("jacobi_omega", C.c_double),
+        ("exp_order", C.c_int32),
+        ("E0", C.c_double * 3),
+        ("flags", C.c_uint32),
+        ("device", C.c_int32),
+        ("stream", C.c_void_p),
+    ]
+
+
+class RTError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"rt_tddft error {code}: {msg}")
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2410_09189_b200.build` "
+            "(the RT-TDDFT path has no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp, i32, i64p = C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int64)
+    sig = {
+        "rt_create": [C.POINTER(rt_config), dp, dp, dp, C.POINTER(vp)],
+        "rt_set_field": [vp, dp], "rt_step": [vp, i32], "rt_get_dipole": [vp, dp], "rt_get_density": [vp, dp],
+        "rt_get_pmatrix": [vp, dp, dp], "rt_get_hmatrix": [vp, dp], "rt_get_vhartree": [vp, dp],
+        "rt_get_time": [vp, dp], "rt_get_charge": [vp, dp], "rt_get_info": [vp, dp], "rt_get_launch_count": [vp, i64p],
+        "rt_destroy": [vp], "rt_op_project": [vp, dp, dp], "rt_op_density": [vp, dp, dp, dp],
+        "rt_op_propagate": [vp, dp, dp, dp, dp, dp], "rt_op_hartree": [vp, dp, dp, i32], "rt_op_vxc": [vp, dp, dp],
+        "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp],
+    }
+    for name, argtypes in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes = argtypes
+        fn.restype = C.c_int
+    lib.rt_last_error.argtypes = [vp]
+    lib.rt_last_error.restype = C.c_char_p
+    return lib
+
+
+_lib = _load()
+
+
+def _ptr(x):
+    """Address of a numpy array (host), a torch tensor (host or device), an int address, or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        assert x.dtype == np.float64 and x.flags["C_CONTIGUOUS"], "need C-contiguous float64"
+        return x.ctypes.data
+    if hasattr(x, "data_ptr"):
+        import torch
+        assert x.dtype == torch.float64 and x.is_contiguous(), "need contiguous float64 tensor"
+        return x.data_ptr()
+    raise TypeError(type(x))
+
+
+def _check(h, rc):
+    if rc != RT_OK:
+        msg = _lib.rt_last_error(h)
+        raise RTError(rc, msg.decode() if msg else "")
+
+
+# ---- functions with the C names -------------------------------------------------------------------------
+
+def rt_create(cfg: rt_config, phi, eps, occ) -> int:
+    h = C.c_void_p()
+    eps = np.ascontiguousarray(eps, dtype=np.float64)
+    occ = np.ascontiguousarray(occ, dtype=np.float64)
+    rc = _lib.rt_create(C.byref(cfg), _ptr(phi), _ptr(eps), _ptr(occ), C.byref(h))
+    _check(None, rc)
+    return h.value
+
+
+def rt_set_field(h, E):
+    e = (C.c_double * 3)(*[float(v) for v in E])
+    _check(h, _lib.rt_set_field(h, C.cast(e, C.c_void_p)))
+
+
+def rt_step(h, nsteps=1):
+    _check(h, _lib.rt_step(h, int(nsteps)))
+
+
+def rt_get_dipole(h) -> np.ndarray:
+    mu = np.zeros(3)
+    _check(h, _lib.rt_get_dipole(h, _ptr(mu)))
+    return mu
+
+
+def rt_get_density(h, out):
+    _check(h, _lib.rt_get_density(h, _ptr(out)))
+    return out
+
+
+def rt_get_pmatrix(h, re, im):
+    _check(h, _lib.rt_get_pmatrix(h, _ptr(re), _ptr(im)))
+
+
+def rt_get_hmatrix(h, out):
+    _check(h, _lib.rt_get_hmatrix(h, _ptr(out)))
+    return out
+
+
+def rt_get_vhartree(h, out):
+    _check(h, _lib.rt_get_vhartree(h, _ptr(out)))
+    return out
+
+
+def rt_get_time(h) -> float:
+    t = np.zeros(1)
+    _check(h, _lib.rt_get_time(h, _ptr(t)))
+    return float(t[0])
+
+
+def rt_get_charge(h) -> np.ndarray:
+    q = np.zeros(2)
+    _check(h, _lib.rt_get_charge(h, _ptr(q)))
+    return q
+
+
+def rt_get_info(h) -> dict:
+    a = np.zeros(8, dtype=np.int32)
+    _check(h, _lib.rt_get_info(h, a.ctypes.data))
+    return {"exp_order": int(a[0]), "mg_levels": int(a[1]), "coarsest": (int(a[2]), int(a[3]), int(a[4])),
+            "graph": bool(a[5]), "launches_per_step": int(a[6]), "project_split_k": int(a[7])}
+
+
+def rt_get_launch_count(h) -> int:
+    n = C.c_int64(0)
+    _check(h, _lib.rt_get_launch_count(h, C.byref(n)))
+    return int(n.value)
+
+
+def rt_destroy(h):
+    if h:
+        _lib.rt_destroy(h)
+
+
+def rt_op_project(h, v, out):
+    _check(h, _lib.rt_op_project(h, _ptr(v), _ptr(out)))
+    return out
+
+
+def rt_op_density(h, reP, rho):
+    sums = np.zeros(5)
+    _check(h, _lib.rt_op_density(h, _ptr(reP), _ptr(rho), _ptr(sums)))
+    return rho, sums
+
+
+def rt_op_propagate(h, Hbar, P0re, P0im, P1re, P1im):
+    _check(h, _lib.rt_op_propagate(h, _ptr(Hbar), _ptr(P0re), _ptr(P0im), _ptr(P1re), _ptr(P1im)))
+    return P1re, P1im
+
+
+def rt_op_hartree(h, vh, drho, n_vc):
+    _check(h, _lib.rt_op_hartree(h, _ptr(vh), _ptr(drho), int(n_vc)))
+    return vh
+
+
+def rt_op_vxc(h, rho, out):
+    _check(h, _lib.rt_op_vxc(h, _ptr(rho), _ptr(out)))
+    return out
+
+
+def rt_timing_enable(h, enable=True):
+    _check(h, _lib.rt_timing_enable(h, 1 if enable else 0))
+
+
+def rt_timing_read(h):
+    ms = np.zeros(RT_STAGE_COUNT)
+    calls = np.zeros(RT_STAGE_COUNT, dtype=np.int64)
+    _check(h, _lib.rt_timing_read(h, _ptr(ms), calls.ctypes.data))
+    return dict(zip(RT_STAGE_NAMES, ms.tolist())), dict(zip(RT_STAGE_NAMES, calls.tolist()))
+
+
+# ---- convenience wrapper (the call a user makes) -------------------------------------------------------
+
+class RTTDDFT:
+    """Owns one rt_handle.  ``phi`` may be a host numpy array (copied) or a CUDA torch tensor (borrowed)."""
+
+    def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
+                 nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, device=0,
+                 stream=None):
+        cfg = rt_config()
+        cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)
+        cfg.h, cfg.norb, cfg.dt = float(h), int(len(eps)), float(dt)
+        cfg.n_hupdates, cfg.n_vcycles = int(n_hupdates), int(n_vcycles)
+        cfg.nu_pre, cfg.nu_post, cfg.jacobi_omega = int(nu_pre), int(nu_post), float(jacobi_omega)
+        cfg.exp_order = int(exp_order)
+        cfg.E0 = (C.c_double * 3)(*[float(e) for e in E0])
+        flags = 0
+        self._phi_ref = None
+        if hasattr(phi, "is_cuda"):
+            if phi.is_cuda:
+                flags |= RT_PHI_DEVICE
+                device = phi.device.index if phi.device.index is not None else device
+                self._phi_ref = phi           # keep the borrowed tensor alive
+            else:
+                phi = phi.numpy()
+        if not hartree:
+            flags |= RT_NO_HARTREE
+        if not xc:
+            flags |= RT_NO_XC
+        if not graph:
+            flags |= RT_NO_GRAPH
+        cfg.flags, cfg.device = flags, int(device)
+        if stream is None:
+            try:
+                import torch
+                stream = torch.cuda.current_stream(device).cuda_stream if torch.cuda.is_available() else 0
+            except ImportError:
+                stream = 0
+        cfg.stream = int(stream) if stream else None
+        self.shape, self.norb = tuple(int(s) for s in shape), int(len(eps))
+        self.ngrid = self.shape[0] * self.shape[1] * self.shape[2]
+        self.handle = rt_create(cfg, phi, eps, occ)
+
+    def set_field(self, E):
+        rt_set_field(self.handle, E)
+
+    def step(self, n=1):
+        rt_step(self.handle, n)
+
+    def dipole(self):
+        return rt_get_dipole(self.handle)
+
+    def density(self, out=None):
+        if out is None:
+            out = np.empty(self.ngrid)
+        return rt_get_density(self.handle, out)
+
+    def pmatrix(self):
+        re, im = np.empty((self.norb, self.norb)), np.empty((self.norb, self.norb))
+        rt_get_pmatrix(self.handle, re, im)
+        return re + 1j * im
+
+    def hmatrix(self):
+        return rt_get_hmatrix(self.handle, np.empty((self.norb, self.norb)))
+
+    def vhartree(self):
+        return rt_get_vhartree(self.handle, np.empty(self.ngrid))
+
+    @property
+    def time(self):
+        return rt_get_time(self.handle)
+
+    def info(self):
+        return rt_get_info(self.handle)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            rt_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,413 @@
+// grid_kernels.cu -- HBM/L2-bound stages on the real-space grid and the small N x N glue kernels.
+//
+//   a6  reduce_rho      : rho = sum of the density kernel's partials, fused dipole / charge reduction
+//                         (Alg. 1 line 27) with a fixed-order second stage (bit-reproducible).
+//   a7  multigrid       : periodic 7-point Poisson, V(nu1,nu2) cycles, weighted Jacobi, full weighting,
+//                         trilinear prolongation, exact separable solve on the coarsest level ("Vh", L545; DESIGN R6).
+//   a8  delta_v / vxc   : Slater exchange + PZ81 correlation and the dV assembly ("exchange/correlation", L547).
+//   a2  hbar etc.       : Alg. 1 lines 11, 14, 28 on N x N matrices.
+#include "rt_internal.h"
+
+namespace rt {
+
+constexpr int RB = 256;                 // threads per block of the streaming kernels
+constexpr int RED_BLOCKS_MAX = 1024;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// block-wide sums of NV values; result valid in thread 0
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double (*sh)[NV]) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int q = 0; q < NV; ++q) v[q] = warp_sum(v[q]);
+  if (lane == 0)
+#pragma unroll
+    for (int q = 0; q < NV; ++q) sh[warp][q] = v[q];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const int nw = blockDim.x >> 5;
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+      double s = 0.0;
+      for (int w = 0; w < nw; ++w) s += sh[w][q];
+      v[q] = s;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- a6
+int reduce_rho_blocks(long long Ng) {
+  long long nb = (Ng + RB * 4 - 1) / (RB * 4);
+  return (int)(nb < 1 ? 1 : (nb > RED_BLOCKS_MAX ? RED_BLOCKS_MAX : nb));
+}
+
+__global__ void __launch_bounds__(RB)
+reduce_rho_kernel(const double* __restrict__ part, int nparts, long long Ng, GridDims gd, double h,
+                  const double* __restrict__ rho0, double* __restrict__ rho, double* __restrict__ bsums) {
+  __shared__ double sh[RB / 32][5];
+  double v[5] = {0, 0, 0, 0, 0};
+  const double cx = 0.5 * (gd.nx - 1), cy = 0.5 * (gd.ny - 1), cz = 0.5 * (gd.nz - 1);
+  const long long nyz = (long long)gd.ny * gd.nz;
+  for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < Ng; r += (long long)gridDim.x * RB) {
+    double s = 0.0;
+    for (int p = 0; p < nparts; ++p) s += part[(long long)p * Ng + r];
+    rho[r] = s;
+    const int ix = (int)(r / nyz);
+    const int rem = (int)(r - (long long)ix * nyz);
+    const int iy = rem / gd.nz, iz = rem - iy * gd.nz;
+    v[0] += s;
+    v[1] += ((double)ix - cx) * h * s;
+    v[2] += ((double)iy - cy) * h * s;
+    v[3] += ((double)iz - cz) * h * s;
+    v[4] += rho0 ? (s - rho0[r]) : s;
+  }
+  block_sum<5>(v, sh);
+  if (threadIdx.x == 0)
+#pragma unroll
+    for (int q = 0; q < 5; ++q) bsums[blockIdx.x * 5 + q] = v[q];
+}
+
+__global__ void final_sums_kernel(const double* __restrict__ bsums, int nb, int nv, double* __restrict__ sums) {
+  // one warp per value; fixed order: lane-strided partials, then a shuffle tree
+  const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (q >= nv) return;
+  double s = 0.0;
+  for (int b = lane; b < nb; b += 32) s += bsums[b * nv + q];
+  s = warp_sum(s);
+  if (lane == 0) sums[q] = s;
+}
+
+void launch_reduce_rho(const double* rho_part, int nparts, long long Ng, GridDims gd, double h, const double* rho0,
+                       double* rho, double* bsums, double* sums, cudaStream_t st) {
+  const int nb = reduce_rho_blocks(Ng);
+  reduce_rho_kernel<<<nb, RB, 0, st>>>(rho_part, nparts, Ng, gd, h, rho0, rho, bsums);
+  final_sums_kernel<<<1, 32 * 5, 0, st>>>(bsums, nb, 5, sums);
+}
+
+__global__ void __launch_bounds__(RB)
+sum_only_kernel(const double* __restrict__ v, long long n, double* __restrict__ bsums) {
+  __shared__ double sh[RB / 32][5];
+  double a[5] = {0, 0, 0, 0, 0};
+  for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < n; r += (long long)gridDim.x * RB) a[4] += v[r];
+  block_sum<5>(a, sh);
+  if (threadIdx.x == 0)
+#pragma unroll
+    for (int q = 0; q < 5; ++q) bsums[blockIdx.x * 5 + q] = a[q];
+}
+
+void launch_sum_only(const double* v, long long n, double* bsums, double* sums, cudaStream_t st) {
+  const int nb = reduce_rho_blocks(n);
+  sum_only_kernel<<<nb, RB, 0, st>>>(v, n, bsums);
+  final_sums_kernel<<<1, 32 * 5, 0, st>>>(bsums, nb, 5, sums);
+}
+
+// ---------------------------------------------------------------------------------------------- a8
+// Slater exchange + Perdew-Zunger 1981 correlation, unpolarised (DESIGN R7); branch on rho <= 3/(4 pi).
+__device__ __forceinline__ double vxc_pz81(double rho) {
+  if (!(rho >= 1e-30)) return 0.0;
+  const double PI = 3.14159265358979323846;
+  const double vx = -cbrt(3.0 * rho / PI);
+  const double rs = cbrt(3.0 / (4.0 * PI * rho));
+  double vc;
+  if (rho <= 3.0 / (4.0 * PI)) {
+    const double sq = sqrt(rs);
+    const double den = 1.0 + 1.0529 * sq + 0.3334 * rs;
+    const double ec = -0.1423 / den;
+    vc = ec * (1.0 + (7.0 / 6.0) * 1.0529 * sq + (4.0 / 3.0) * 0.3334 * rs) / den;
+  } else {
+    const double ln = log(rs);
+    vc = 0.0311 * ln + (-0.048 - 0.0311 / 3.0) + (2.0 / 3.0) * 0.0020 * rs * ln + ((2.0 * -0.0116 - 0.0020) / 3.0) * rs;
+  }
+  return vx + vc;
+}
+
+__device__ __forceinline__ double field_at(long long r, GridDims gd, double h, const double* __restrict__ E) {
+  const long long nyz = (long long)gd.ny * gd.nz;
+  const int ix = (int)(r / nyz);
+  const int rem = (int)(r - (long long)ix * nyz);
+  const int iy = rem / gd.nz, iz = rem - iy * gd.nz;
+  return E[0] * (((double)ix - 0.5 * (gd.nx - 1)) * h) + E[1] * (((double)iy - 0.5 * (gd.ny - 1)) * h) +
+         E[2] * (((double)iz - 0.5 * (gd.nz - 1)) * h);
+}
+
+__global__ void __launch_bounds__(RB)
+delta_v_kernel(long long Ng, GridDims gd, double h, const double* __restrict__ rho, const double* __restrict__ vxc0,
+               const double* __restrict__ VH, const double* __restrict__ E, int use_h, int use_xc,
+               double* __restrict__ w) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= Ng) return;
+  double v = field_at(r, gd, h, E);
+  if (use_h) v += VH[r];
+  if (use_xc) v += vxc_pz81(rho[r]) - vxc0[r];
+  w[r] = v;
+}
+
+__global__ void __launch_bounds__(RB) vxc_kernel(long long Ng, const double* __restrict__ rho, double* __restrict__ out) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r < Ng) out[r] = vxc_pz81(rho[r]);
+}
+
+__global__ void __launch_bounds__(RB)
+field_kernel(long long Ng, GridDims gd, double h, const double* __restrict__ E, double* __restrict__ w) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r < Ng) w[r] = field_at(r, gd, h, E);
+}
+
+static inline unsigned nblk(long long n) { return (unsigned)((n + RB - 1) / RB); }
+
+void launch_delta_v(long long Ng, GridDims gd, double h, const double* rho, const double* vxc0, const double* VH,
+                    const double* E, int use_h, int use_xc, double* w, cudaStream_t st) {
+  delta_v_kernel<<<nblk(Ng), RB, 0, st>>>(Ng, gd, h, rho, vxc0, VH, E, use_h, use_xc, w);
+}
+void launch_vxc(long long Ng, const double* rho, double* vxc, cudaStream_t st) {
+  vxc_kernel<<<nblk(Ng), RB, 0, st>>>(Ng, rho, vxc);
+}
+void launch_field(long long Ng, GridDims gd, double h, const double* E, double* w, cudaStream_t st) {
+  field_kernel<<<nblk(Ng), RB, 0, st>>>(Ng, gd, h, E, w);
+}
+
+// ---------------------------------------------------------------------------------------------- a7
+__global__ void __launch_bounds__(RB)
+poisson_rhs_kernel(long long Ng, const double* __restrict__ rho, const double* __restrict__ rho0,
+                   const double* __restrict__ sums, double* __restrict__ f) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= Ng) return;
+  const double mean = sums[4] / (double)Ng;
+  const double d = rho0 ? rho[r] - rho0[r] : rho[r];
+  f[r] = 4.0 * 3.14159265358979323846 * (d - mean);
+}
+void launch_poisson_rhs(long long Ng, const double* rho, const double* rho0, const double* sums, double* f,
+                        cudaStream_t st) {
+  poisson_rhs_kernel<<<nblk(Ng), RB, 0, st>>>(Ng, rho, rho0, sums, f);
+}
+
+__device__ __forceinline__ void idx3(long long r, GridDims gd, int& ix, int& iy, int& iz) {
+  const long long nyz = (long long)gd.ny * gd.nz;
+  ix = (int)(r / nyz);
+  const int rem = (int)(r - (long long)ix * nyz);
+  iy = rem / gd.nz;
+  iz = rem - iy * gd.nz;
+}
+
+__device__ __forceinline__ double nb_sum(const double* __restrict__ u, GridDims gd, int ix, int iy, int iz) {
+  const long long nyz = (long long)gd.ny * gd.nz;
+  const int xm = ix == 0 ? gd.nx - 1 : ix - 1, xp = ix == gd.nx - 1 ? 0 : ix + 1;
+  const int ym = iy == 0 ? gd.ny - 1 : iy - 1, yp = iy == gd.ny - 1 ? 0 : iy + 1;
+  const int zm = iz == 0 ? gd.nz - 1 : iz - 1, zp = iz == gd.nz - 1 ? 0 : iz + 1;
+  const long long row = (long long)iy * gd.nz, pl = (long long)ix * nyz;
+  return u[xm * nyz + row + iz] + u[xp * nyz + row + iz] + u[pl + (long long)ym * gd.nz + iz] +
+         u[pl + (long long)yp * gd.nz + iz] + u[pl + row + zm] + u[pl + row + zp];
+}
+
+// u_out = (1 - omega) u + (omega / 6) (h^2 f + sum_nb u)
+__global__ void __launch_bounds__(RB)
+jacobi_kernel(GridDims gd, long long n, double h2, double omega, const double* __restrict__ u,
+              const double* __restrict__ f, double* __restrict__ out) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= n) return;
+  int ix, iy, iz;
+  idx3(r, gd, ix, iy, iz);
+  out[r] = (1.0 - omega) * u[r] + (omega / 6.0) * (h2 * f[r] + nb_sum(u, gd, ix, iy, iz));
+}
+void launch_jacobi(const MgLevel& L, const double* uin, double* uout, double omega, cudaStream_t st) {
+  jacobi_kernel<<<nblk(L.n), RB, 0, st>>>(L.gd, L.n, L.h * L.h, omega, uin, L.f, uout);
+}
+
+// r = f - (6 u - sum_nb u)/h^2
+__global__ void __launch_bounds__(RB)
+residual_kernel(GridDims gd, long long n, double inv_h2, const double* __restrict__ u, const double* __restrict__ f,
+                double* __restrict__ res) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= n) return;
+  int ix, iy, iz;
+  idx3(r, gd, ix, iy, iz);
+  res[r] = f[r] - (6.0 * u[r] - nb_sum(u, gd, ix, iy, iz)) * inv_h2;
+}
+void launch_residual(const MgLevel& L, cudaStream_t st) {
+  residual_kernel<<<nblk(L.n), RB, 0, st>>>(L.gd, L.n, 1.0 / (L.h * L.h), L.u, L.f, L.r);
+}
+
+// full weighting (1/4,1/2,1/4)^3, coarse I <-> fine 2I
+__global__ void __launch_bounds__(RB)
+restrict_kernel(GridDims gf, GridDims gc, long long nc, const double* __restrict__ res, double* __restrict__ fc) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= nc) return;
+  int I, J, K;
+  idx3(r, gc, I, J, K);
+  const long long nyz = (long long)gf.ny * gf.nz;
+  double s = 0.0;
+#pragma unroll
+  for (int a = -1; a <= 1; ++a) {
+    int x = 2 * I + a; x = x < 0 ? x + gf.nx : (x >= gf.nx ? x - gf.nx : x);
+    const double wa = a == 0 ? 0.5 : 0.25;
+    double sy = 0.0;
+#pragma unroll
+    for (int b = -1; b <= 1; ++b) {
+      int y = 2 * J + b; y = y < 0 ? y + gf.ny : (y >= gf.ny ? y - gf.ny : y);
+      const double wb = b == 0 ? 0.5 : 0.25;
+      const double* p = res + x * nyz + (long long)y * gf.nz;
+      const int z0 = 2 * K;
+      const int zm = z0 == 0 ? gf.nz - 1 : z0 - 1, zp = z0 + 1 >= gf.nz ? z0 + 1 - gf.nz : z0 + 1;
+      sy += wb * (0.25 * p[zm] + 0.5 * p[z0] + 0.25 * p[zp]);
+    }
+    s += wa * sy;
+  }
+  fc[r] = s;
+}
+void launch_restrict(const MgLevel& fine, const MgLevel& coarse, cudaStream_t st) {
+  restrict_kernel<<<nblk(coarse.n), RB, 0, st>>>(fine.gd, coarse.gd, coarse.n, fine.r, coarse.f);
+}
+
+// trilinear prolongation, added to the fine solution
+__global__ void __launch_bounds__(RB)
+prolong_add_kernel(GridDims gf, GridDims gc, long long nf, const double* __restrict__ ec, double* __restrict__ u) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= nf) return;
+  int ix, iy, iz;
+  idx3(r, gf, ix, iy, iz);
+  const int I0 = ix >> 1, J0 = iy >> 1, K0 = iz >> 1;
+  const int I1 = (ix & 1) ? (I0 + 1 == gc.nx ? 0 : I0 + 1) : I0;
+  const int J1 = (iy & 1) ? (J0 + 1 == gc.ny ? 0 : J0 + 1) : J0;
+  const int K1 = (iz & 1) ? (K0 + 1 == gc.nz ? 0 : K0 + 1) : K0;
+  const long long nyz = (long long)gc.ny * gc.nz;
+  auto at = [&](int I, int J, int K) { return ec[I * nyz + (long long)J * gc.nz + K]; };
+  // 0.5 (a + b) with a == b on even points reproduces the injected value exactly
+  const double z00 = 0.5 * (at(I0, J0, K0) + at(I0, J0, K1));
+  const double z01 = 0.5 * (at(I0, J1, K0) + at(I0, J1, K1));
+  const double z10 = 0.5 * (at(I1, J0, K0) + at(I1, J0, K1));
+  const double z11 = 0.5 * (at(I1, J1, K0) + at(I1, J1, K1));
+  const double y0 = 0.5 * (z00 + z01), y1 = 0.5 * (z10 + z11);
+  u[r] += 0.5 * (y0 + y1);
+}
+void launch_prolong_add(const MgLevel& coarse, const MgLevel& fine, cudaStream_t st) {
+  prolong_add_kernel<<<nblk(fine.n), RB, 0, st>>>(fine.gd, coarse.gd, fine.n, coarse.u, fine.u);
+}
+
+__global__ void __launch_bounds__(RB) zero_kernel(double* __restrict__ p, long long n) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r < n) p[r] = 0.0;
+}
+void launch_zero(double* p, long long n, cudaStream_t st) { zero_kernel<<<nblk(n), RB, 0, st>>>(p, n); }
+
+// Exact solve on the coarsest level in the zero-mean subspace: u = (Qx x Qy x Qz) L^+ (Qx x Qy x Qz)^T f with
+// the real orthonormal eigenvectors of the periodic 1-D operator (columns of Q) and eigenvalues lx+ly+lz.
+// One CTA; two global scratch buffers (L.r and L.tmp) ping-pong between the six axis passes.
+__global__ void __launch_bounds__(1024)
+coarse_solve_kernel(GridDims gd, const double* __restrict__ f, double* __restrict__ u, double* __restrict__ s0,
+                    double* __restrict__ s1, const double* __restrict__ Qx, const double* __restrict__ Qy,
+                    const double* __restrict__ Qz, const double* __restrict__ lx, const double* __restrict__ ly,
+                    const double* __restrict__ lz) {
+  const int nx = gd.nx, ny = gd.ny, nz = gd.nz;
+  const int n = nx * ny * nz;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  // forward: contract each axis with Q^T  (out[a] = sum_i Q[i][a] in[i])
+  for (int o = tid; o < n; o += nt) {                    // x axis: f -> s0
+    const int a = o / (ny * nz), rest = o % (ny * nz);
+    double s = 0.0;
+    for (int i = 0; i < nx; ++i) s += Qx[i * nx + a] * f[i * ny * nz + rest];
+    s0[o] = s;
+  }
+  __syncthreads();
+  for (int o = tid; o < n; o += nt) {                    // y axis: s0 -> s1
+    const int a = o / (ny * nz), b = (o / nz) % ny, k = o % nz;
+    double s = 0.0;
+    for (int j = 0; j < ny; ++j) s += Qy[j * ny + b] * s0[(a * ny + j) * nz + k];
+    s1[o] = s;
+  }
+  __syncthreads();
+  for (int o = tid; o < n; o += nt) {                    // z axis + divide by the eigenvalue: s1 -> s0
+    const int a = o / (ny * nz), b = (o / nz) % ny, cc = o % nz;
+    double s = 0.0;
+    for (int k = 0; k < nz; ++k) s += Qz[k * nz + cc] * s1[(a * ny + b) * nz + k];
+    const double lam = lx[a] + ly[b] + lz[cc];
+    s0[o] = (a == 0 && b == 0 && cc == 0) ? 0.0 : s / lam;
+  }
+  __syncthreads();
+  // backward: contract each axis with Q  (out[i] = sum_a Q[i][a] in[a])
+  for (int o = tid; o < n; o += nt) {                    // z: s0 -> s1
+    const int a = o / (ny * nz), b = (o / nz) % ny, k = o % nz;
+    double s = 0.0;
+    for (int cc = 0; cc < nz; ++cc) s += Qz[k * nz + cc] * s0[(a * ny + b) * nz + cc];
+    s1[o] = s;
+  }
+  __syncthreads();
+  for (int o = tid; o < n; o += nt) {                    // y: s1 -> s0
+    const int a = o / (ny * nz), j = (o / nz) % ny, k = o % nz;
+    double s = 0.0;
+    for (int b = 0; b < ny; ++b) s += Qy[j * ny + b] * s1[(a * ny + b) * nz + k];
+    s0[o] = s;
+  }
+  __syncthreads();
+  for (int o = tid; o < n; o += nt) {                    // x: s0 -> u
+    const int i = o / (ny * nz), rest = o % (ny * nz);
+    double s = 0.0;
+    for (int a = 0; a < nx; ++a) s += Qx[i * nx + a] * s0[a * ny * nz + rest];
+    u[o] = s;
+  }
+}
+void launch_coarse_solve(const MgLevel& L, const double* Qx, const double* Qy, const double* Qz, const double* lx,
+                         const double* ly, const double* lz, cudaStream_t st) {
+  coarse_solve_kernel<<<1, 1024, 0, st>>>(L.gd, L.f, L.u, L.r, L.tmp, Qx, Qy, Qz, lx, ly, lz);
+}
+
+// ---------------------------------------------------------------------------------------------- a2 and glue
+__global__ void hbar_kernel(int N, int ldn, const double* __restrict__ Hm1, const double* __restrict__ H0,
+                            double* __restrict__ H1, double* __restrict__ X, double dt, double sigma, int first) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j >= N) return;
+  const long long o = (long long)i * ldn + j;
+  const double h0 = H0[o];
+  double h1;
+  if (first) { h1 = 2.0 * h0 - Hm1[o]; H1[o] = h1; } else { h1 = H1[o]; }
+  double x = 0.5 * (h0 + h1);
+  if (i == j) x -= sigma;
+  X[o] = dt * x;
+}
+void launch_hbar(int N, int ldn, const double* Hm1, const double* H0, double* H1, double* X, double dt, double sigma,
+                 int first, cudaStream_t st) {
+  hbar_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, Hm1, H0, H1, X, dt, sigma, first);
+}
+
+__global__ void series_init_kernel(int N, int ldn, const double* __restrict__ Y, double* __restrict__ C, double c1,
+                                   double* __restrict__ S, double s1) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j >= N) return;
+  const long long o = (long long)i * ldn + j;
+  const double y = Y[o], d = (i == j) ? 1.0 : 0.0;
+  C[o] = d + c1 * y;
+  S[o] = d + s1 * y;
+}
+void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, double* S, double s1, cudaStream_t st) {
+  series_init_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, Y, C, c1, S, s1);
+}
+
+__global__ void copy4_kernel(long long n, double* __restrict__ d0, const double* __restrict__ s0, double* __restrict__ d1,
+                             const double* __restrict__ s1, double* __restrict__ d2, const double* __restrict__ s2,
+                             double* __restrict__ d3, const double* __restrict__ s3) {
+  for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += (long long)gridDim.x * blockDim.x) {
+    d0[r] = s0[r]; d1[r] = s1[r]; d2[r] = s2[r]; d3[r] = s3[r];
+  }
+}
+void launch_copy5(int N, int ldn, double* d0, const double* s0, double* d1, const double* s1, double* d2,
+                  const double* s2, double* d3, const double* s3, cudaStream_t st) {
+  const long long n = (long long)N * ldn;
+  long long nb = (n + 255) / 256;
+  if (nb > 148 * 16) nb = 148 * 16;
+  copy4_kernel<<<(unsigned)nb, 256, 0, st>>>(n, d0, s0, d1, s1, d2, s2, d3, s3);
+}
+
+__global__ void set_diag_kernel(int N, int ldn, double* __restrict__ M, const double* __restrict__ d) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j >= ldn) return;
+  M[(long long)i * ldn + j] = (i == j) ? d[i] : 0.0;
+}
+void launch_set_diag(int N, int ldn, double* M, const double* diag, cudaStream_t st) {
+  set_diag_kernel<<<dim3((ldn + 127) / 128, N), 128, 0, st>>>(N, ldn, M, diag);
+}
+
+}  // namespace rt

@@ -1,0 +1,769 @@
+// rt_api.cu -- the C ABI of include/rt_tddft.h: context, workspaces, the step schedule, getters.
+// Everything numerical happens in the kernels of gemm_kernels.cu / grid_kernels.cu; this file only owns
+// memory, enqueues launches in the order of Algorithm 1 and moves results across the ABI.
+#include "../../include/rt_tddft.h"
+#include "rt_internal.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace rt;
+
+namespace {
+
+thread_local std::string g_create_error = "";
+
+struct EventPair { cudaEvent_t a, b; int stage; };
+
+}  // namespace
+
+struct rt_ctx {
+  rt_config cfg{};
+  int N = 0, ldn = 0;
+  long long Ng = 0;
+  GridDims gd{};
+  double h = 0, dvol = 0, dt = 0, sigma = 0, omega = 0;
+  int m = 2, n_vc = 0, nu1 = 2, nu2 = 2, q = 0;           // q: cos/sinc polynomial degree in Y = X^2
+  bool use_h = true, use_xc = true, use_graph = true;
+  cudaStream_t st = nullptr;
+  bool poisoned = false;
+  std::string err;
+  double t = 0;
+  int64_t launches = 0;          // kernels enqueued so far
+  int64_t launches_per_step = 0;
+
+  const double* phi = nullptr;   // borrowed or owned
+  double* phi_owned = nullptr;
+  std::vector<void*> allocs;
+
+  // N-vectors / scalars
+  double *d_eps = nullptr, *d_occ = nullptr, *d_E = nullptr, *d_sums = nullptr, *d_bsums = nullptr;
+  // N x N (ld = ldn)
+  double *Hm1 = nullptr, *H0 = nullptr, *H1 = nullptr, *X = nullptr, *Ya = nullptr, *Yb = nullptr, *Yc = nullptr,
+         *Cm = nullptr, *Sc = nullptr, *Sm = nullptr, *P0r = nullptr, *P0i = nullptr, *P1r = nullptr, *P1i = nullptr,
+         *W = nullptr;
+  int2* d_tiles = nullptr;
+  ProjectPlan pp{};
+  DensityPlan dp{};
+  // grid arrays
+  double *rho = nullptr, *rho0 = nullptr, *vxc0 = nullptr, *w = nullptr, *rho_part = nullptr, *op_u = nullptr;
+  std::vector<MgLevel> lv;
+  double *Qx = nullptr, *Qy = nullptr, *Qz = nullptr, *lx = nullptr, *ly = nullptr, *lz = nullptr;
+
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+
+  bool timing = false;
+  std::vector<EventPair> ev_used;
+  std::vector<EventPair> ev_free;
+  double stage_ms[RT_STAGE_COUNT] = {0, 0, 0, 0, 0};
+  int64_t stage_calls[RT_STAGE_COUNT] = {0, 0, 0, 0, 0};
+};
+
+namespace {
+
+int fail(rt_ctx* c, int code, const std::string& msg) {
+  if (c) { c->err = msg; if (code == RT_ECUDA) c->poisoned = true; }
+  else g_create_error = msg;
+  return code;
+}
+
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess)                                                                         \
+      return fail(c, RT_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));                 \
+  } while (0)
+
+#define CHECK_HANDLE(c)                                                                            \
+  do {                                                                                             \
+    if (!(c)) return fail(nullptr, RT_ESTATE, "NULL handle");                                       \
+    if ((c)->poisoned) return RT_ESTATE;                                                           \
+  } while (0)
+
+template <class T>
+int dev_alloc(rt_ctx* c, T** p, size_t count) {
+  void* q = nullptr;
+  cudaError_t e = cudaMalloc(&q, count * sizeof(T) > 0 ? count * sizeof(T) : 16);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(c, RT_ENOMEM, std::string("cudaMalloc failed: ") + cudaGetErrorString(e));
+  }
+  c->allocs.push_back(q);
+  *p = reinterpret_cast<T*>(q);
+  return RT_OK;
+}
+
+int roundup(int x, int m) { return (x + m - 1) / m * m; }
+
+// real orthonormal eigenvectors of the periodic 1-D second-difference operator: column 0 constant,
+// then (cos_k, sin_k) pairs, then the alternating vector when n is even.  lam[col] = (2 - 2 cos(2 pi k/n))/h^2.
+void eigenbasis_1d(int n, double h, std::vector<double>& Q, std::vector<double>& lam) {
+  const double PI = 3.14159265358979323846;
+  Q.assign((size_t)n * n, 0.0);
+  lam.assign(n, 0.0);
+  int col = 0;
+  for (int i = 0; i < n; ++i) Q[(size_t)i * n + col] = 1.0 / std::sqrt((double)n);
+  lam[col++] = 0.0;
+  for (int k = 1; 2 * k < n; ++k) {
+    const double l = (2.0 - 2.0 * std::cos(2.0 * PI * k / n)) / (h * h);
+    for (int i = 0; i < n; ++i) {
+      // reduce the angle argument exactly in integers before calling cos/sin
+      const long long kk = ((long long)k * i) % n;
+      Q[(size_t)i * n + col] = std::sqrt(2.0 / n) * std::cos(2.0 * PI * (double)kk / n);
+      Q[(size_t)i * n + col + 1] = std::sqrt(2.0 / n) * std::sin(2.0 * PI * (double)kk / n);
+    }
+    lam[col] = lam[col + 1] = l;
+    col += 2;
+  }
+  if (n % 2 == 0 && n > 1) {
+    for (int i = 0; i < n; ++i) Q[(size_t)i * n + col] = ((i & 1) ? -1.0 : 1.0) / std::sqrt((double)n);
+    lam[col++] = 4.0 / (h * h);
+  }
+}
+
+bool can_coarsen(const GridDims& g) {
+  return g.nx % 2 == 0 && g.ny % 2 == 0 && g.nz % 2 == 0 && g.nx > 4 && g.ny > 4 && g.nz > 4;
+}
+
+// ---- stage timing helpers ------------------------------------------------------------------------
+void stage_begin(rt_ctx* c, int stage) {
+  if (!c->timing) return;
+  EventPair ep;
+  if (!c->ev_free.empty()) { ep = c->ev_free.back(); c->ev_free.pop_back(); }
+  else { cudaEventCreate(&ep.a); cudaEventCreate(&ep.b); }
+  ep.stage = stage;
+  cudaEventRecord(ep.a, c->st);
+  c->ev_used.push_back(ep);
+}
+void stage_end(rt_ctx* c) {
+  if (!c->timing) return;
+  cudaEventRecord(c->ev_used.back().b, c->st);
+}
+
+// ---- the stages ------------------------------------------------------------------------------------
+void enqueue_gemm(rt_ctx* c, const double* A0, const double* B0, double a0, const double* A1, const double* B1,
+                  double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr, double b2 = 0) {
+  GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2};
+  launch_gemm_abt(g, c->st);
+  c->launches += 1;
+}
+
+// C = cos X, S = sin X for the real symmetric X (H-bar real at Gamma) -> U = C - i S.
+// cos X = sum_k (-1)^k Y^k/(2k)!, sin X = X sum_k (-1)^k Y^k/(2k+1)!, Y = X^2, k <= q.   q + 1 GEMMs.
+void enqueue_expm(rt_ctx* c) {
+  enqueue_gemm(c, c->X, c->X, 1.0, nullptr, nullptr, 0, c->Ya);
+  launch_series_init(c->N, c->ldn, c->Ya, c->Cm, -0.5, c->Sc, -1.0 / 6.0, c->st);
+  c->launches += 1;
+  double ck = -0.5, sk = -1.0 / 6.0;
+  const double* prev = c->Ya;
+  for (int k = 2; k <= c->q; ++k) {
+    ck = -ck / ((2.0 * k - 1.0) * (2.0 * k));
+    sk = -sk / ((2.0 * k) * (2.0 * k + 1.0));
+    double* cur = (k < c->q) ? ((k & 1) ? c->Yc : c->Yb) : nullptr;
+    enqueue_gemm(c, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk);
+    prev = cur;
+  }
+  enqueue_gemm(c, c->X, c->Sc, 1.0, nullptr, nullptr, 0, c->Sm);
+}
+
+// P1 = U P0 U^dagger (Eq. 15), U = C - iS, P0 = A + iB (A symmetric, B antisymmetric).
+//   Yr = C A + S B, Yi = C B - S A ; P1r = Yr C - Yi S, P1i = Yr S + Yi C.
+// gemm_abt contracts against B^T: a symmetric right factor is used as is, the antisymmetric one flips the sign.
+void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
+  enqueue_gemm(c, c->Cm, Ar, 1.0, c->Sm, Ai, -1.0, c->Yb);
+  enqueue_gemm(c, c->Cm, Ai, -1.0, c->Sm, Ar, -1.0, c->Yc);
+  enqueue_gemm(c, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, Or);
+  enqueue_gemm(c, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, Oi);
+}
+
+void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double* rho0) {
+  launch_fold_upper(c->N, c->ldn, reP, c->X, c->st);
+  launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
+  launch_reduce_rho(c->rho_part, c->dp.npairs, c->Ng, c->gd, c->h, rho0, rho_out, c->d_bsums, c->d_sums, c->st);
+  c->launches += 4;
+}
+
+void enqueue_smooth(rt_ctx* c, const MgLevel& L, int n) {
+  const double* in = L.u;
+  double* out = L.tmp;
+  for (int s = 0; s < n; ++s) {
+    launch_jacobi(L, in, out, c->omega, c->st);
+    c->launches += 1;
+    const double* t = in; in = out; out = const_cast<double*>(t);
+  }
+  if (n & 1) {   // odd sweep count: result sits in tmp, bring it home
+    cudaMemcpyAsync(L.u, L.tmp, (size_t)L.n * sizeof(double), cudaMemcpyDeviceToDevice, c->st);
+  }
+}
+
+void enqueue_vcycle(rt_ctx* c, std::vector<MgLevel>& lv, size_t l) {
+  MgLevel& L = lv[l];
+  if (l + 1 == lv.size()) {
+    launch_coarse_solve(L, c->Qx, c->Qy, c->Qz, c->lx, c->ly, c->lz, c->st);
+    c->launches += 1;
+    return;
+  }
+  enqueue_smooth(c, L, c->nu1);
+  launch_residual(L, c->st);
+  launch_restrict(L, lv[l + 1], c->st);
+  c->launches += 2;
+  if (l + 2 < lv.size()) {        // zero initial guess (the exact coarsest solve overwrites u)
+    launch_zero(lv[l + 1].u, lv[l + 1].n, c->st);
+    c->launches += 1;
+  }
+  enqueue_vcycle(c, lv, l + 1);
+  launch_prolong_add(lv[l + 1], L, c->st);
+  c->launches += 1;
+  enqueue_smooth(c, L, c->nu2);
+}
+
+void enqueue_project(rt_ctx* c, const double* w, const double* eps, double* H) {
+  launch_project(c->pp, c->phi, w, c->d_tiles, c->W, c->st);
+  launch_project_reduce(c->pp, c->W, eps, c->dvol, H, c->st);
+  c->launches += 2;
+}
+
+// One time step, Algorithm 1 lines 10-28.
+void enqueue_step(rt_ctx* c) {
+  for (int it = 0; it < c->m; ++it) {
+    stage_begin(c, RT_STAGE_ELDYN);
+    launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st);   // lines 11, 14
+    c->launches += 1;
+    enqueue_expm(c);
+    enqueue_upu(c, c->P0r, c->P0i, c->P1r, c->P1i);                                            // Eq. 15
+    stage_end(c);
+
+    stage_begin(c, RT_STAGE_RHO);
+    enqueue_density(c, c->P1r, c->rho, c->rho0);                                               // Eq. 27 + line 27
+    stage_end(c);
+
+    if (c->use_h) {
+      stage_begin(c, RT_STAGE_VH);
+      launch_poisson_rhs(c->Ng, c->rho, c->rho0, c->d_sums, c->lv[0].f, c->st);
+      c->launches += 1;
+      for (int v = 0; v < c->n_vc; ++v) enqueue_vcycle(c, c->lv, 0);
+      stage_end(c);
+    }
+
+    stage_begin(c, RT_STAGE_XC);
+    launch_delta_v(c->Ng, c->gd, c->h, c->rho, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->w, c->st);
+    c->launches += 1;
+    stage_end(c);
+
+    stage_begin(c, RT_STAGE_HUPDATE);
+    enqueue_project(c, c->w, c->d_eps, c->H1);                                                 // line 25
+    stage_end(c);
+  }
+  stage_begin(c, RT_STAGE_ELDYN);
+  launch_copy5(c->N, c->ldn, c->Hm1, c->H0, c->H0, c->H1, c->P0r, c->P1r, c->P0i, c->P1i, c->st);   // line 28
+  c->launches += 1;
+  stage_end(c);
+}
+
+int sync_and_check(rt_ctx* c) {
+  CK(cudaStreamSynchronize(c->st));
+  CK(cudaGetLastError());
+  return RT_OK;
+}
+
+int collect_timing(rt_ctx* c) {
+  for (auto& ep : c->ev_used) {
+    float ms = 0;
+    CK(cudaEventElapsedTime(&ms, ep.a, ep.b));
+    c->stage_ms[ep.stage] += ms;
+    c->stage_calls[ep.stage] += 1;
+    c->ev_free.push_back(ep);
+  }
+  c->ev_used.clear();
+  return RT_OK;
+}
+
+int copy_matrix_out(rt_ctx* c, const double* src, double* dst) {   // [N][ldn] device -> [N][N] anywhere
+  if (!dst) return RT_OK;
+  CK(cudaMemcpy2DAsync(dst, (size_t)c->N * 8, src, (size_t)c->ldn * 8, (size_t)c->N * 8, c->N, cudaMemcpyDefault, c->st));
+  return RT_OK;
+}
+int copy_matrix_in(rt_ctx* c, const double* src, double* dst) {    // [N][N] anywhere -> [N][ldn] device
+  CK(cudaMemsetAsync(dst, 0, (size_t)c->N * c->ldn * 8, c->st));
+  CK(cudaMemcpy2DAsync(dst, (size_t)c->ldn * 8, src, (size_t)c->N * 8, (size_t)c->N * 8, c->N, cudaMemcpyDefault, c->st));
+  return RT_OK;
+}
+
+}  // namespace
+
+// ======================================================================================================
+extern "C" {
+
+const char* rt_last_error(rt_handle h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int rt_destroy(rt_handle c) {
+  if (!c) return RT_OK;
+  cudaSetDevice(c->cfg.device);
+  cudaStreamSynchronize(c->st);
+  if (c->gexec) cudaGraphExecDestroy(c->gexec);
+  if (c->graph) cudaGraphDestroy(c->graph);
+  for (auto& ep : c->ev_used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+  for (auto& ep : c->ev_free) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+  for (void* p : c->allocs) cudaFree(p);
+  cudaGetLastError();
+  delete c;
+  return RT_OK;
+}
+
+int rt_create(const rt_config* cfg, const double* phi, const double* eps, const double* occ, rt_handle* out) {
+  rt_ctx* c = nullptr;
+  if (!cfg || !phi || !eps || !occ || !out) return fail(c, RT_EINVAL, "rt_create: NULL argument");
+  *out = nullptr;
+  if (cfg->nx < 2 || cfg->ny < 2 || cfg->nz < 2) return fail(c, RT_EINVAL, "rt_create: grid dims must be >= 2");
+  if (!(cfg->h > 0) || !(cfg->dt > 0)) return fail(c, RT_EINVAL, "rt_create: h and dt must be > 0");
+  if (cfg->norb < 1) return fail(c, RT_EINVAL, "rt_create: norb must be >= 1");
+  if (cfg->n_hupdates < 0 || cfg->n_vcycles < 0 || cfg->nu_pre < 0 || cfg->nu_post < 0 || cfg->exp_order < 0)
+    return fail(c, RT_EINVAL, "rt_create: negative iteration count");
+  for (int i = 0; i < cfg->norb; ++i)
+    if (!(occ[i] >= 0.0 && occ[i] <= 2.0)) return fail(c, RT_EINVAL, "rt_create: occ must lie in [0, 2]");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) {
+    cudaGetLastError();
+    return fail(c, RT_ECUDA, "rt_create: no such CUDA device (this library has no CPU fallback)");
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess || prop.major < 10)
+    return fail(c, RT_ECUDA, "rt_create: device is not sm_100 or newer");
+  if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(c, RT_ECUDA, "rt_create: cudaSetDevice failed");
+
+  c = new rt_ctx();
+  c->cfg = *cfg;
+  c->N = cfg->norb;
+  c->ldn = roundup(c->N, 8);
+  c->gd = GridDims{cfg->nx, cfg->ny, cfg->nz};
+  c->Ng = (long long)cfg->nx * cfg->ny * cfg->nz;
+  c->h = cfg->h;
+  c->dvol = cfg->h * cfg->h * cfg->h;
+  c->dt = cfg->dt;
+  c->m = cfg->n_hupdates ? cfg->n_hupdates : 2;
+  c->n_vc = cfg->n_vcycles;
+  c->nu1 = (cfg->nu_pre || cfg->nu_post) ? cfg->nu_pre : 2;
+  c->nu2 = (cfg->nu_pre || cfg->nu_post) ? cfg->nu_post : 2;
+  c->omega = cfg->jacobi_omega != 0.0 ? cfg->jacobi_omega : 6.0 / 7.0;
+  c->use_h = !(cfg->flags & RT_NO_HARTREE);
+  c->use_xc = !(cfg->flags & RT_NO_XC);
+  c->use_graph = !(cfg->flags & RT_NO_GRAPH);
+  c->st = reinterpret_cast<cudaStream_t>(cfg->stream);
+  const int N = c->N, ldn = c->ldn;
+  const long long Ng = c->Ng;
+
+#define FAIL_CREATE(code, msg) do { int rc_ = fail(nullptr, (code), (msg)); rt_destroy(c); return rc_; } while (0)
+#define CKC(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); cudaGetLastError(); FAIL_CREATE(RT_ECUDA, m_); } } while (0)
+#define ALLOC(ptr, count) do { if (dev_alloc(c, &(ptr), (size_t)(count)) != RT_OK) { std::string m_ = c->err; FAIL_CREATE(RT_ENOMEM, m_); } } while (0)
+
+  // series order from the spectral bound (DESIGN R8)
+  double emin = eps[0], emax = eps[0];
+  for (int i = 1; i < N; ++i) { emin = std::fmin(emin, eps[i]); emax = std::fmax(emax, eps[i]); }
+  c->sigma = 0.5 * (emin + emax);
+  {
+    const double half[3] = {0.5 * (cfg->nx - 1) * cfg->h, 0.5 * (cfg->ny - 1) * cfg->h, 0.5 * (cfg->nz - 1) * cfg->h};
+    double vmax = 0.5;
+    for (int d = 0; d < 3; ++d) vmax += std::fabs(cfg->E0[d]) * half[d];
+    const double theta = c->dt * (0.5 * (emax - emin) + vmax);
+    int q;
+    if (cfg->exp_order > 0) q = (cfg->exp_order > 1) ? cfg->exp_order / 2 : 1;   // degree 2q+1 >= K
+    else {
+      q = 1;
+      double term = theta * theta * theta * theta / 24.0;     // theta^(2q+2)/(2q+2)! at q = 1
+      while (term > 1e-17 && q < 40) { ++q; term *= theta * theta / ((2.0 * q + 1.0) * (2.0 * q + 2.0)); }
+    }
+    c->q = q;
+  }
+
+  // multigrid hierarchy
+  {
+    GridDims g = c->gd;
+    double hh = c->h;
+    for (;;) {
+      MgLevel L{};
+      L.gd = g; L.h = hh; L.n = (long long)g.nx * g.ny * g.nz;
+      c->lv.push_back(L);
+      if (!can_coarsen(g)) break;
+      g = GridDims{g.nx / 2, g.ny / 2, g.nz / 2};
+      hh *= 2.0;
+    }
+    if (c->use_h && c->lv.back().n > 32768)
+      FAIL_CREATE(RT_EINVAL, "rt_create: coarsest multigrid level has more than 32768 points (grid dims need more factors of 2)");
+  }
+
+  // plans
+  const int ntile = (N + TILE - 1) / TILE;
+  {
+    ProjectPlan& p = c->pp;
+    p.N = N; p.Ng = Ng; p.ntile = ntile; p.T = ntile * (ntile + 1) / 2; p.ldn = ldn;
+    long long S = (2 * prop.multiProcessorCount + p.T - 1) / p.T;
+    const long long kmin = 16 * 8;
+    if (S > (Ng + kmin - 1) / kmin) S = (Ng + kmin - 1) / kmin;
+    if (S < 1) S = 1;
+    long long kc = (Ng + S - 1) / S;
+    kc = (kc + 15) / 16 * 16;
+    p.kchunk = kc;
+    p.S = (int)((Ng + kc - 1) / kc);
+    DensityPlan& d = c->dp;
+    d.N = N; d.Ng = Ng; d.ntile = ntile; d.npairs = (ntile + 1) / 2; d.nrt = (Ng + TILE - 1) / TILE; d.ldn = ldn;
+    const int sms = prop.multiProcessorCount;
+    int gr = d.npairs >= 12 ? 12 : (sms + d.npairs - 1) / d.npairs;
+    if (gr > d.nrt) gr = (int)d.nrt;
+    d.group_r = gr < 1 ? 1 : gr;
+  }
+
+  // memory check, then allocations
+  {
+    size_t freeb = 0, totalb = 0;
+    CKC(cudaMemGetInfo(&freeb, &totalb));
+    double need = 15.0 * N * (double)ldn * 8 + (double)c->pp.S * N * ldn * 8 + (double)c->dp.npairs * Ng * 8 + 12.0 * Ng * 8;
+    if (!(cfg->flags & RT_PHI_DEVICE)) need += (double)N * Ng * 8;
+    if (need > (double)freeb) {
+      char buf[256];
+      snprintf(buf, sizeof buf, "rt_create: needs %.2f GB of device memory, %.2f GB free", need / 1e9, freeb / 1e9);
+      FAIL_CREATE(RT_ENOMEM, buf);
+    }
+  }
+  if (cfg->flags & RT_PHI_DEVICE) {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, phi) != cudaSuccess || pa.type != cudaMemoryTypeDevice) {
+      cudaGetLastError();
+      FAIL_CREATE(RT_EINVAL, "rt_create: RT_PHI_DEVICE set but phi is not a device pointer");
+    }
+    c->phi = phi;
+  } else {
+    ALLOC(c->phi_owned, (size_t)N * Ng);
+    CKC(cudaMemcpyAsync(c->phi_owned, phi, (size_t)N * Ng * 8, cudaMemcpyHostToDevice, c->st));
+    c->phi = c->phi_owned;
+  }
+  const size_t nn = (size_t)N * ldn;
+  ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8); ALLOC(c->d_sums, 8);
+  ALLOC(c->d_bsums, 5 * 1024);
+  double** mats[] = {&c->Hm1, &c->H0, &c->H1, &c->X, &c->Ya, &c->Yb, &c->Yc, &c->Cm, &c->Sc, &c->Sm,
+                     &c->P0r, &c->P0i, &c->P1r, &c->P1i};
+  for (double** mp : mats) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
+  ALLOC(c->W, (size_t)c->pp.S * nn);
+  ALLOC(c->rho, Ng); ALLOC(c->rho0, Ng); ALLOC(c->vxc0, Ng); ALLOC(c->w, Ng); ALLOC(c->op_u, Ng);
+  ALLOC(c->rho_part, (size_t)c->dp.npairs * Ng);
+  for (size_t l = 0; l < c->lv.size(); ++l) {
+    MgLevel& L = c->lv[l];
+    ALLOC(L.u, L.n); ALLOC(L.tmp, L.n); ALLOC(L.f, L.n); ALLOC(L.r, L.n);
+    CKC(cudaMemsetAsync(L.u, 0, (size_t)L.n * 8, c->st));
+  }
+  {
+    std::vector<int2> tiles;
+    for (int ti = 0; ti < ntile; ++ti)
+      for (int tj = ti; tj < ntile; ++tj) tiles.push_back(make_int2(ti, tj));
+    ALLOC(c->d_tiles, tiles.size());
+    CKC(cudaMemcpyAsync(c->d_tiles, tiles.data(), tiles.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
+    CKC(cudaStreamSynchronize(c->st));
+  }
+  {
+    const MgLevel& L = c->lv.back();
+    std::vector<double> Q, lam;
+    double** qs[3] = {&c->Qx, &c->Qy, &c->Qz};
+    double** ls[3] = {&c->lx, &c->ly, &c->lz};
+    const int dims[3] = {L.gd.nx, L.gd.ny, L.gd.nz};
+    for (int d = 0; d < 3; ++d) {
+      eigenbasis_1d(dims[d], L.h, Q, lam);
+      ALLOC(*qs[d], Q.size()); ALLOC(*ls[d], lam.size());
+      CKC(cudaMemcpy(*qs[d], Q.data(), Q.size() * 8, cudaMemcpyHostToDevice));
+      CKC(cudaMemcpy(*ls[d], lam.data(), lam.size() * 8, cudaMemcpyHostToDevice));
+    }
+  }
+  CKC(cudaMemcpy(c->d_eps, eps, (size_t)N * 8, cudaMemcpyHostToDevice));
+  CKC(cudaMemcpy(c->d_occ, occ, (size_t)N * 8, cudaMemcpyHostToDevice));
+  {
+    double e8[8] = {cfg->E0[0], cfg->E0[1], cfg->E0[2], 0, 0, 0, 0, 0};
+    CKC(cudaMemcpy(c->d_E, e8, sizeof e8, cudaMemcpyHostToDevice));
+  }
+
+  // initial state (Alg. 1 lines 7-8): P0 = diag(occ); rho0; vxc0; H0 = H-1 = diag(eps) + Proj(E0.r)
+  launch_set_diag(N, ldn, c->P0r, c->d_occ, c->st);
+  enqueue_density(c, c->P0r, c->rho0, nullptr);
+  CKC(cudaMemcpyAsync(c->rho, c->rho0, (size_t)Ng * 8, cudaMemcpyDeviceToDevice, c->st));
+  launch_vxc(Ng, c->rho0, c->vxc0, c->st);
+  launch_field(Ng, c->gd, c->h, c->d_E, c->w, c->st);
+  enqueue_project(c, c->w, c->d_eps, c->H0);
+  CKC(cudaMemcpyAsync(c->Hm1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
+  CKC(cudaMemcpyAsync(c->H1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
+  // sums[4] currently holds sum(rho0) (rho0 pointer was NULL): the induced charge at t = 0 is zero
+  CKC(cudaMemsetAsync(c->d_sums + 4, 0, 8, c->st));
+  {
+    double z8[8] = {0, 0, 0, 0, 0, 0, 0, 0};                  // E(t_1) defaults to 0 (DESIGN R5)
+    CKC(cudaMemcpyAsync(c->d_E, z8, sizeof z8, cudaMemcpyHostToDevice, c->st));
+  }
+  CKC(cudaStreamSynchronize(c->st));
+  CKC(cudaGetLastError());
+
+  // capture one step into a CUDA graph (pointers are fixed: line 28 is a copy, not a pointer rotation)
+  {
+    const int64_t before = c->launches;
+    if (c->use_graph) {
+      // capture on a private stream (the caller's may be the legacy default stream, which cannot capture);
+      // the instantiated graph is replayed on the caller's stream
+      cudaStream_t user = c->st, cap = nullptr;
+      CKC(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+      c->st = cap;
+      cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+      if (e == cudaSuccess) {
+        enqueue_step(c);
+        e = cudaStreamEndCapture(cap, &c->graph);
+      }
+      c->st = user;
+      cudaStreamDestroy(cap);
+      if (e != cudaSuccess) { cudaGetLastError(); FAIL_CREATE(RT_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
+      CKC(cudaGraphInstantiate(&c->gexec, c->graph, 0));
+    } else {
+      // dry count without launching anything is not possible; count on the first real step instead
+    }
+    c->launches_per_step = c->launches - before;
+    c->launches = before;
+  }
+#undef ALLOC
+#undef CKC
+#undef FAIL_CREATE
+  *out = c;
+  return RT_OK;
+}
+
+int rt_set_field(rt_handle c, const double E[3]) {
+  CHECK_HANDLE(c);
+  if (!E) return fail(c, RT_EINVAL, "rt_set_field: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  CK(cudaMemcpyAsync(c->d_E, E, 3 * sizeof(double), cudaMemcpyHostToDevice, c->st));
+  return RT_OK;
+}
+
+int rt_step(rt_handle c, int32_t nsteps) {
+  CHECK_HANDLE(c);
+  if (nsteps < 0) return fail(c, RT_EINVAL, "rt_step: nsteps < 0");
+  CK(cudaSetDevice(c->cfg.device));
+  for (int s = 0; s < nsteps; ++s) {
+    if (c->gexec && !c->timing) {
+      CK(cudaGraphLaunch(c->gexec, c->st));
+      c->launches += c->launches_per_step;
+    } else {
+      const int64_t before = c->launches;
+      enqueue_step(c);
+      if (!c->launches_per_step) c->launches_per_step = c->launches - before;
+      CK(cudaGetLastError());
+    }
+    c->t += c->dt;
+  }
+  return RT_OK;
+}
+
+int rt_get_dipole(rt_handle c, double mu[3]) {
+  CHECK_HANDLE(c);
+  if (!mu) return fail(c, RT_EINVAL, "rt_get_dipole: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  double s[5];
+  CK(cudaMemcpyAsync(s, c->d_sums, sizeof s, cudaMemcpyDeviceToHost, c->st));
+  if (int rc = sync_and_check(c)) return rc;
+  for (int q = 0; q < 3; ++q) mu[q] = c->dvol * s[1 + q];
+  return RT_OK;
+}
+
+int rt_get_charge(rt_handle c, double q[2]) {
+  CHECK_HANDLE(c);
+  if (!q) return fail(c, RT_EINVAL, "rt_get_charge: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  double s[5];
+  CK(cudaMemcpyAsync(s, c->d_sums, sizeof s, cudaMemcpyDeviceToHost, c->st));
+  if (int rc = sync_and_check(c)) return rc;
+  q[0] = c->dvol * s[0];
+  q[1] = c->dvol * s[4];
+  return RT_OK;
+}
+
+int rt_get_density(rt_handle c, double* rho) {
+  CHECK_HANDLE(c);
+  if (!rho) return fail(c, RT_EINVAL, "rt_get_density: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  CK(cudaMemcpyAsync(rho, c->rho, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  return sync_and_check(c);
+}
+
+int rt_get_vhartree(rt_handle c, double* vh) {
+  CHECK_HANDLE(c);
+  if (!vh) return fail(c, RT_EINVAL, "rt_get_vhartree: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  CK(cudaMemcpyAsync(vh, c->lv[0].u, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  return sync_and_check(c);
+}
+
+int rt_get_pmatrix(rt_handle c, double* re, double* im) {
+  CHECK_HANDLE(c);
+  CK(cudaSetDevice(c->cfg.device));
+  if (int rc = copy_matrix_out(c, c->P0r, re)) return rc;
+  if (int rc = copy_matrix_out(c, c->P0i, im)) return rc;
+  return sync_and_check(c);
+}
+
+int rt_get_hmatrix(rt_handle c, double* H0) {
+  CHECK_HANDLE(c);
+  CK(cudaSetDevice(c->cfg.device));
+  if (int rc = copy_matrix_out(c, c->H0, H0)) return rc;
+  return sync_and_check(c);
+}
+
+int rt_get_time(rt_handle c, double* t) {
+  CHECK_HANDLE(c);
+  if (!t) return fail(c, RT_EINVAL, "rt_get_time: NULL");
+  *t = c->t;
+  return RT_OK;
+}
+
+int rt_get_info(rt_handle c, int32_t info[8]) {
+  CHECK_HANDLE(c);
+  if (!info) return fail(c, RT_EINVAL, "rt_get_info: NULL");
+  const MgLevel& L = c->lv.back();
+  info[0] = 2 * c->q + 1;
+  info[1] = (int32_t)c->lv.size();
+  info[2] = L.gd.nx; info[3] = L.gd.ny; info[4] = L.gd.nz;
+  info[5] = c->gexec ? 1 : 0;
+  info[6] = (int32_t)c->launches_per_step;
+  info[7] = c->pp.S;
+  return RT_OK;
+}
+
+int rt_get_launch_count(rt_handle c, int64_t* n) {
+  CHECK_HANDLE(c);
+  if (!n) return fail(c, RT_EINVAL, "rt_get_launch_count: NULL");
+  *n = c->launches;
+  return RT_OK;
+}
+
+// ---- per-stage entry points ------------------------------------------------------------------------
+int rt_op_project(rt_handle c, const double* v, double* out) {
+  CHECK_HANDLE(c);
+  if (!v || !out) return fail(c, RT_EINVAL, "rt_op_project: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  CK(cudaMemcpyAsync(c->op_u, v, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  stage_begin(c, RT_STAGE_HUPDATE);
+  enqueue_project(c, c->op_u, nullptr, c->Ya);
+  stage_end(c);
+  if (int rc = copy_matrix_out(c, c->Ya, out)) return rc;
+  return sync_and_check(c);
+}
+
+int rt_op_density(rt_handle c, const double* reP, double* rho, double sums[5]) {
+  CHECK_HANDLE(c);
+  if (!reP || !rho) return fail(c, RT_EINVAL, "rt_op_density: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  if (int rc = copy_matrix_in(c, reP, c->Ya)) return rc;
+  // d_sums is propagation state (dipole of the current density): save and restore around the call
+  double keep[5];
+  CK(cudaMemcpyAsync(keep, c->d_sums, sizeof keep, cudaMemcpyDeviceToHost, c->st));
+  stage_begin(c, RT_STAGE_RHO);
+  enqueue_density(c, c->Ya, c->op_u, c->rho0);
+  stage_end(c);
+  double s[5];
+  CK(cudaMemcpyAsync(s, c->d_sums, sizeof s, cudaMemcpyDeviceToHost, c->st));
+  CK(cudaMemcpyAsync(rho, c->op_u, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  if (int rc = sync_and_check(c)) return rc;
+  CK(cudaMemcpyAsync(c->d_sums, keep, sizeof keep, cudaMemcpyHostToDevice, c->st));
+  if (int rc = sync_and_check(c)) return rc;
+  if (sums) memcpy(sums, s, sizeof s);
+  return RT_OK;
+}
+
+int rt_op_propagate(rt_handle c, const double* Hbar, const double* P0re, const double* P0im, double* P1re,
+                    double* P1im) {
+  CHECK_HANDLE(c);
+  if (!Hbar || !P0re || !P0im || !P1re || !P1im) return fail(c, RT_EINVAL, "rt_op_propagate: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  // scratch: H1 <- Hbar (as both H0 and H1 of launch_hbar), P1r/P1i <- P0 ; outputs in Hm1-free buffers
+  // The propagation state uses Hm1/H0/H1/P0/P1, so stage everything in W (>= 1 slab) plus X..Sm scratch.
+  // W holds S >= 1 slabs of N*ldn; we need 5 matrices -> use Hm1-independent temporaries allocated lazily.
+  const size_t nn = (size_t)c->N * c->ldn;
+  double* T[5];
+  for (int i = 0; i < 5; ++i) {
+    void* p = nullptr;
+    CK(cudaMalloc(&p, nn * 8));
+    T[i] = (double*)p;
+  }
+  int rc = RT_OK;
+  do {
+    if ((rc = copy_matrix_in(c, Hbar, T[0]))) break;
+    if ((rc = copy_matrix_in(c, P0re, T[1]))) break;
+    if ((rc = copy_matrix_in(c, P0im, T[2]))) break;
+    stage_begin(c, RT_STAGE_ELDYN);
+    launch_hbar(c->N, c->ldn, T[0], T[0], T[0], c->X, c->dt, c->sigma, 0, c->st);   // X = dt (Hbar - sigma I)
+    c->launches += 1;
+    enqueue_expm(c);
+    enqueue_upu(c, T[1], T[2], T[3], T[4]);
+    stage_end(c);
+    if ((rc = copy_matrix_out(c, T[3], P1re))) break;
+    if ((rc = copy_matrix_out(c, T[4], P1im))) break;
+    rc = sync_and_check(c);
+  } while (0);
+  cudaStreamSynchronize(c->st);
+  for (int i = 0; i < 5; ++i) cudaFree(T[i]);
+  return rc;
+}
+
+int rt_op_hartree(rt_handle c, double* vh, const double* drho, int32_t n_vc) {
+  CHECK_HANDLE(c);
+  if (!vh || !drho || n_vc < 0) return fail(c, RT_EINVAL, "rt_op_hartree: bad argument");
+  if (!c->use_h) return fail(c, RT_EINVAL, "rt_op_hartree: handle created with RT_NO_HARTREE");
+  CK(cudaSetDevice(c->cfg.device));
+  double keep[5];
+  CK(cudaMemcpyAsync(keep, c->d_sums, sizeof keep, cudaMemcpyDeviceToHost, c->st));
+  // run the cycle on a private level-0 solution (op_u) and rhs input staged in w
+  CK(cudaMemcpyAsync(c->op_u, vh, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  CK(cudaMemcpyAsync(c->w, drho, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  std::vector<MgLevel> lv = c->lv;
+  lv[0].u = c->op_u;
+  stage_begin(c, RT_STAGE_VH);
+  launch_sum_only(c->w, c->Ng, c->d_bsums, c->d_sums, c->st);
+  launch_poisson_rhs(c->Ng, c->w, nullptr, c->d_sums, lv[0].f, c->st);
+  c->launches += 3;
+  for (int v = 0; v < n_vc; ++v) enqueue_vcycle(c, lv, 0);
+  stage_end(c);
+  CK(cudaMemcpyAsync(vh, c->op_u, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  if (int rc = sync_and_check(c)) return rc;
+  CK(cudaMemcpyAsync(c->d_sums, keep, sizeof keep, cudaMemcpyHostToDevice, c->st));
+  return sync_and_check(c);
+}
+
+int rt_op_vxc(rt_handle c, const double* rho, double* vxc) {
+  CHECK_HANDLE(c);
+  if (!rho || !vxc) return fail(c, RT_EINVAL, "rt_op_vxc: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  CK(cudaMemcpyAsync(c->op_u, rho, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  stage_begin(c, RT_STAGE_XC);
+  launch_vxc(c->Ng, c->op_u, c->w, c->st);
+  c->launches += 1;
+  stage_end(c);
+  CK(cudaMemcpyAsync(vxc, c->w, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
+  return sync_and_check(c);
+}
+
+int rt_timing_enable(rt_handle c, int32_t enable) {
+  CHECK_HANDLE(c);
+  c->timing = enable != 0;
+  return RT_OK;
+}
+
+int rt_timing_read(rt_handle c, double ms[RT_STAGE_COUNT], int64_t calls[RT_STAGE_COUNT]) {
+  CHECK_HANDLE(c);
+  CK(cudaSetDevice(c->cfg.device));
+  if (int rc = sync_and_check(c)) return rc;
+  if (int rc = collect_timing(c)) return rc;
+  for (int i = 0; i < RT_STAGE_COUNT; ++i) {
+    if (ms) ms[i] = c->stage_ms[i];
+    if (calls) calls[i] = c->stage_calls[i];
+    c->stage_ms[i] = 0;
+    c->stage_calls[i] = 0;
+  }
+  return RT_OK;
+}
+
+}  // extern "C"

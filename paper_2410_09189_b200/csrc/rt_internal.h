@@ -1,0 +1,98 @@
+// rt_internal.h -- launcher prototypes shared between the kernel translation units and rt_api.cu.
+// Not part of the public ABI (that is include/rt_tddft.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rt {
+
+constexpr int TILE = 128;        // CTA tile edge of the DMMA kernels (orbital index)
+
+struct GridDims { int nx, ny, nz; };
+
+// ---- a1 projection: W[s][i][j] = sum_{r in chunk s} phi_i(r) w(r) phi_j(r) for upper tiles (ti <= tj) -----
+struct ProjectPlan {
+  int N;                 // orbitals
+  long long Ng;          // grid points (contraction length), also the leading dimension of Phi
+  int ntile;             // ceil(N / TILE)
+  int T;                 // number of upper-triangular tiles
+  int S;                 // split-K factor
+  long long kchunk;      // grid points per split (multiple of 16)
+  int ldn;               // leading dimension of the N x N outputs
+};
+void launch_project(const ProjectPlan& p, const double* phi, const double* w, const int2* tiles, double* W,
+                    cudaStream_t st);
+// H[i][j] = scale * sum_s W[s][i][j] (+ eps_i if i == j and eps != nullptr), mirrored to the lower triangle.
+void launch_project_reduce(const ProjectPlan& p, const double* W, const double* eps, double scale, double* H,
+                           cudaStream_t st);
+size_t project_smem_bytes();
+
+// ---- a5 density: rho_part[p][r] = sum over the j-tiles of pair p of sum_j phi_j(r) (Pfold Phi)_j(r) -------
+struct DensityPlan {
+  int N;
+  long long Ng;
+  int ntile;             // j tiles
+  int npairs;            // ceil(ntile / 2): CTA handles j-tiles (p, ntile-1-p)
+  long long nrt;         // r tiles = ceil(Ng / TILE)
+  int ldn;
+  int group_r;           // raster: r-tiles per supertile column
+};
+void launch_density(const DensityPlan& p, const double* phi, const double* Pfold, double* rho_part, cudaStream_t st);
+size_t density_smem_bytes();
+// Pfold[j][i] = 2 P[j][i] (i > j), P[j][j] (i == j), 0 (i < j)
+void launch_fold_upper(int N, int ldn, const double* P, double* Pfold, cudaStream_t st);
+
+// ---- a3/a4 N x N GEMM:  D = alpha0 * A0 B0^T + alpha1 * A1 B1^T ; optional Z1 += beta1 D, Z2 += beta2 D --------
+struct GemmArgs {
+  int N, ldn;
+  const double* A0; const double* B0; double alpha0;
+  const double* A1; const double* B1; double alpha1;     // A1 == nullptr -> single term
+  double* D;                                            // may be nullptr (only the axpys are wanted)
+  double* Z1; double beta1;                             // may be nullptr
+  double* Z2; double beta2;
+};
+void launch_gemm_abt(const GemmArgs& g, cudaStream_t st);
+size_t gemm_smem_bytes();
+
+// ---- elementwise N x N (a2 and series glue) -------------------------------------------------------------
+// first != 0: H1 = 2 H0 - Hm1 first.  X = dt * ((H0 + H1)/2 - sigma I)
+void launch_hbar(int N, int ldn, const double* Hm1, const double* H0, double* H1, double* X, double dt,
+                 double sigma, int first, cudaStream_t st);
+// C = I + c1 Y ; S = I + s1 Y
+void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, double* S, double s1, cudaStream_t st);
+// dst = src for n matrices (state shift, line 28)
+void launch_copy5(int N, int ldn, double* d0, const double* s0, double* d1, const double* s1, double* d2,
+                  const double* s2, double* d3, const double* s3, cudaStream_t st);
+void launch_set_diag(int N, int ldn, double* M, const double* diag, cudaStream_t st);   // M = diag(d)
+
+// ---- grid kernels (a6, a7, a8) ---------------------------------------------------------------------------
+// rho[r] = sum_p rho_part[p][r]; block partial sums of {rho, x rho, y rho, z rho, rho - rho0} -> bsums[nb][5]
+int  reduce_rho_blocks(long long Ng);
+void launch_reduce_rho(const double* rho_part, int nparts, long long Ng, GridDims gd, double h, const double* rho0,
+                       double* rho, double* bsums, double* sums, cudaStream_t st);
+// w[r] = (hartree ? VH : 0) + (xc ? vxc(rho) - vxc0 : 0) + E.x(r)
+void launch_delta_v(long long Ng, GridDims gd, double h, const double* rho, const double* vxc0, const double* VH,
+                    const double* E, int use_h, int use_xc, double* w, cudaStream_t st);
+void launch_vxc(long long Ng, const double* rho, double* vxc, cudaStream_t st);
+void launch_field(long long Ng, GridDims gd, double h, const double* E, double* w, cudaStream_t st);
+// f = 4 pi (rho - rho0 - sums[4]/Ng)      (rho0 may be nullptr: f = 4 pi (rho - sums[4]/Ng))
+void launch_poisson_rhs(long long Ng, const double* rho, const double* rho0, const double* sums, double* f,
+                        cudaStream_t st);
+
+struct MgLevel {
+  GridDims gd; double h; long long n;
+  double* u; double* tmp; double* f; double* r;     // solution, ping-pong scratch, rhs, residual
+};
+void launch_jacobi(const MgLevel& L, const double* uin, double* uout, double omega, cudaStream_t st);
+void launch_residual(const MgLevel& L, cudaStream_t st);                        // L.r = L.f - A L.u
+void launch_restrict(const MgLevel& fine, const MgLevel& coarse, cudaStream_t st);   // coarse.f = R fine.r
+void launch_prolong_add(const MgLevel& coarse, const MgLevel& fine, cudaStream_t st); // fine.u += P coarse.u
+void launch_zero(double* p, long long n, cudaStream_t st);
+// exact zero-mean solve on the coarsest level: u = Q L^+ Q^T f, separable real eigenbasis (Qx,Qy,Qz; inverse
+// eigenvalue tables ilx, ily, ilz hold the 1-D eigenvalues).  One CTA.
+void launch_coarse_solve(const MgLevel& L, const double* Qx, const double* Qy, const double* Qz, const double* lx,
+                         const double* ly, const double* lz, cudaStream_t st);
+// block sums of drho for rt_op_hartree (mean removal): sums[4] = sum(drho)
+void launch_sum_only(const double* v, long long n, double* bsums, double* sums, cudaStream_t st);
+
+}  // namespace rt
