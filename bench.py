@@ -1,0 +1,420 @@
+#!/usr/bin/env python
+"""bench.py -- RT-TDDFT steps/s on B200 (arXiv 2410.09189 time step), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config nano|24k|mid|small|tiny|...] [--impl reference]
+
+A "step" is one pass of the whole hot path (Algorithm 1 lines 10-28: m x [ELDYN, Rho, Vh, XC, Hupdate]) on one
+synthetic system.  Default workload: `nano` (128^3 grid, 2,400 orbitals, Phi = 40 GB
+resident), the largest config whose default run finishes within minutes; `--config 24k` runs the 13,000-orbital
+case.  N > 1 (torchrun): the path does not shard yet ("replicas only"): every rank propagates its own
+system, no data-path collective, value = all ranks' steps / max-over-ranks time, scaling = weak.
+
+`--impl reference` times the CPU oracle (oracle/rt_oracle.py, as it stands) on the host cores on a bounded sample
+of the same workload; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "RT-TDDFT steps/sec"
+UNIT = "steps/s"
+SMI_FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={SMI_FIELDS}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, power, reasons = [], None, [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f:
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 8:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax = float(parts[1])
+                power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": smax, "reasons": ["no samples"]}
+        pmax = max(power)
+        load = [c for c, p in zip(sm, power) if p >= 0.5 * pmax] or sm
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "power_w_max": pmax, "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle sample
+def oracle_sample(w, slab_pts, phi_slab=None, seed=0):
+    """One bounded sample of the oracle's work for workload `w`: returns a function that runs ONE Hamiltonian update
+    of oracle/rt_oracle.py on a grid slab of `slab_pts` points (all N orbitals) plus the full-size N x N propagator and
+    the full-grid Poisson / xc, and the factor by which the slab part must be scaled to the whole grid."""
+    from oracle import rt_oracle as O
+    N, Ng = w.norb, w.ngrid
+    rng = np.random.default_rng(seed)
+    if phi_slab is None:
+        phi_slab = rng.standard_normal((N, slab_pts)) / math.sqrt(Ng * w.dvol)
+    eps = np.sort(rng.uniform(w.eps_range[0], w.eps_range[1], N))
+    occ = np.zeros(N)
+    occ[: w.nocc] = 2.0
+    A = rng.standard_normal((N, N)) * 1e-4
+    Hbar = np.diag(eps) + 0.5 * (A + A.T)
+    P0 = np.diag(occ).astype(np.complex128)
+    rho_full = np.abs(rng.standard_normal(Ng)) * (occ.sum() / (Ng * w.dvol))
+    rho0_full = rho_full * (1 + 1e-6 * rng.standard_normal(Ng))
+    vxc0 = O.vxc_lda(rho0_full)
+    VH = np.zeros(Ng)
+
+    def parts():
+        t0 = time.perf_counter()
+        P1 = O.propagate_eigh(Hbar, P0, w.dt)                       # ELDYN
+        t1 = time.perf_counter()
+        rho_s = O.density(phi_slab, P1.real)                         # Rho on the slab
+        t2 = time.perf_counter()
+        vh = O.hartree_mg(VH, rho_full - rho0_full, w.shape, w.h, w.n_vcycles)     # Vh, full grid
+        t3 = time.perf_counter()
+        dv = vh + O.vxc_lda(rho_full) - vxc0 + O.field_potential(w.shape, w.h, (1e-4, 0, 0))   # XC, full grid
+        t4 = time.perf_counter()
+        H1 = O.project(phi_slab, dv[:slab_pts] + 0 * rho_s, w.dvol)   # Hupdate on the slab
+        t5 = time.perf_counter()
+        return {"ELDYN": t1 - t0, "Rho": t2 - t1, "Vh": t3 - t2, "XC": t4 - t3, "Hupdate": t5 - t4}, H1
+
+    return parts, Ng / slab_pts
+
+
+def oracle_step_seconds(w, parts, scale):
+    t, _ = parts()
+    per_update = t["ELDYN"] + t["Vh"] + t["XC"] + scale * (t["Rho"] + t["Hupdate"])
+    return w.n_hupdates * per_update, t
+
+
+def full_oracle(w):
+    from oracle import rt_oracle as O
+    from paper_2410_09189_b200.workloads import make_inputs_numpy
+    Phi, eps, occ = make_inputs_numpy(w)
+    E0 = w.kick if not w.laser else w.E_of_t(0.0)
+    return O.RTOracle(w.shape, w.h, Phi, eps, occ, dt=w.dt, E0=E0, n_hupdates=w.n_hupdates, n_vcycles=w.n_vcycles)
+
+
+def slab_points(w):
+    # ~10-30 s of CPU work: 4 N^2 slab flops per update at ~100 GFLOP/s -> a few seconds
+    pts = int(2.5e11 / (4.0 * w.norb * w.norb))
+    pts = max(1024, min(w.ngrid, pts))
+    return (pts // 1024) * 1024 if pts >= 1024 else pts
+
+
+def threads_used():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 0) for p in threadpool_info() if p.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return os.cpu_count()
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    big = w.norb * w.ngrid * 8 > 2e9
+    times = []
+    if big:
+        pts = slab_points(w)
+        parts, scale = oracle_sample(w, pts, seed=w.seed)
+        sample = (f"per step: {w.n_hupdates} Hamiltonian updates, each = full {w.norb}^2 eigh propagator + full-grid "
+                  f"Poisson/xc + density & projection on a {pts}-point grid slab (all {w.norb} orbitals), slab time "
+                  f"scaled by Ng/slab = {scale:.1f}")
+        for i in range(args.warmup + args.steps):
+            sec, _ = oracle_step_seconds(w, parts, scale)
+            if i >= args.warmup:
+                times.append(sec)
+    else:
+        o = full_oracle(w)
+        sample = "full oracle steps on the whole workload"
+        for i in range(args.warmup + args.steps):
+            if w.laser:
+                o.set_field(w.E_of_t((i + 1) * w.dt))
+            t0 = time.perf_counter()
+            o.step(1)
+            times.append(time.perf_counter() - t0) if i >= args.warmup else None
+    sec = sum(times) / len(times)
+    val = 1.0 / sec
+    cores = threads_used()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(w, args),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(w, args):
+    return {"workload": w.name, "grid": list(w.shape), "h_bohr": w.h, "norb": w.norb, "nocc": w.nocc, "dt_au": w.dt,
+            "n_hupdates": w.n_hupdates, "n_vcycles": w.n_vcycles, "phi_gb": round(w.norb * w.ngrid * 8 / 1e9, 2),
+            "l2": "inputs larger than L2 (Phi streamed twice per Hamiltonian update)" if w.norb * w.ngrid * 8 > 2.5e8
+            else "L2 flushed between timed steps is not possible inside a CUDA graph: working set fits L2 (stated)",
+            "parallelism": "replicas only" if args.gpus > 1 else "single GPU"}
+
+
+# ------------------------------------------------------------------------------------------------ CUDA arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="nano")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+
+    from paper_2410_09189_b200.workloads import WORKLOADS, make_inputs_device, make_inputs_numpy
+    w = WORKLOADS[args.config]
+    if args.impl == "reference":
+        return run_reference(args, w)
+
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the RT-TDDFT path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2410_09189_b200.build import build
+    if rank == 0:
+        build()
+    if world > 1:
+        dist.barrier()
+    from paper_2410_09189_b200 import binding as B
+
+    # inputs: every rank propagates its own seeded system (replicas; seed offset by rank)
+    import dataclasses
+    wr = dataclasses.replace(w, seed=w.seed + 100 * rank)
+    big = w.norb * w.ngrid * 8 > 2e9
+    t_gen = time.perf_counter()
+    if big:
+        phi, eps, occ, ortho_err = make_inputs_device(wr, device=f"cuda:{local}")
+    else:
+        Phi, eps, occ = make_inputs_numpy(wr)
+        phi = torch.from_numpy(Phi).to(f"cuda:{local}")
+        ortho_err = float(np.max(np.abs(w.dvol * Phi @ Phi.T - np.eye(w.norb))))
+    torch.cuda.synchronize()
+    t_gen = time.perf_counter() - t_gen
+
+    stream = torch.cuda.Stream(device=local)
+    E0 = w.kick if not w.laser else w.E_of_t(0.0)
+    with torch.cuda.stream(stream):
+        sim = B.RTTDDFT(w.shape, w.h, phi, eps, occ, w.dt, E0=E0, n_hupdates=w.n_hupdates, n_vcycles=w.n_vcycles,
+                        device=local, stream=stream.cuda_stream)
+        info = sim.info()
+        peak_dmma, peak_dfma = B.rt_probe_fp64_peak(local)
+
+        # stage events inside the timed region when a step is long enough that they cost nothing
+        stage_in_timed = w.norb * w.norb * w.ngrid > 1e12
+        step_no = [0]
+
+        def one_step():
+            if w.laser:
+                sim.set_field(w.E_of_t((step_no[0] + 1) * w.dt))
+            sim.step(1)
+            step_no[0] += 1
+
+        for _ in range(args.warmup):
+            one_step()
+        stream.synchronize()
+        if stage_in_timed:
+            B.rt_timing_enable(sim.handle, True)
+            B.rt_timing_read(sim.handle)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local) if rank == 0 else None
+        l0 = B.rt_get_launch_count(sim.handle)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(args.steps):
+            one_step()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        ms_total = ev0.elapsed_time(ev1)
+        launches = B.rt_get_launch_count(sim.handle) - l0
+        clocks = sampler.stop() if sampler else None
+        if stage_in_timed:
+            stage_ms, stage_calls = B.rt_timing_read(sim.handle)
+            B.rt_timing_enable(sim.handle, False)
+        else:
+            B.rt_timing_enable(sim.handle, True)
+            B.rt_timing_read(sim.handle)
+            for _ in range(args.steps):
+                one_step()
+            stage_ms, stage_calls = B.rt_timing_read(sim.handle)
+            B.rt_timing_enable(sim.handle, False)
+
+        # end to end through the public API with HOST buffers: field in (pinned host -> device), step, dipole and
+        # density out (device -> pinned host), every step
+        rho_host = torch.empty(w.ngrid, dtype=torch.float64).pin_memory()
+        e_host = torch.zeros(3, dtype=torch.float64).pin_memory()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            E = w.E_of_t((step_no[0] + 1) * w.dt)
+            e_host[0], e_host[1], e_host[2] = E
+            B._check(sim.handle, B._lib.rt_set_field(sim.handle, e_host.data_ptr()))
+            sim.step(1)
+            step_no[0] += 1
+            mu = sim.dipole()
+            B.rt_get_density(sim.handle, rho_host)
+        torch.cuda.synchronize()
+        e2e_sec = time.perf_counter() - t0
+        charge = B.rt_get_charge(sim.handle)
+
+    tmax = torch.tensor([ms_total, e2e_sec * 1e3], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total, e2e_ms = float(tmax[0]), float(tmax[1])
+    if rank != 0:
+        sim.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    ms_per_step = ms_total / args.steps
+    value = world * args.steps / (ms_total * 1e-3)
+    e2e_value = world * args.steps / (e2e_ms * 1e-3)
+
+    # roofline of the dominant kernel (the stage with the largest share)
+    N, Ng = w.norb, w.ngrid
+    alg = {"Hupdate": ("tensor", N * (N + 1.0) * Ng, "a1 projection project_kernel: N(N+1)Ng flop per launch (symmetric output)"),
+           "Rho": ("tensor", 1.0 * N * N * Ng, "a5 density density_kernel: N^2 Ng flop per launch (triangular fold)"),
+           "ELDYN": ("tensor", (2.0 * (info["exp_order"] // 2 + 1) + 16.0) * N ** 3,
+                     "a3+a4 gemm_abt_kernel: (q+1) series GEMMs + 8 for U P U^dagger, 2N^3 each"),
+           "Vh": ("hbm", 167.0 * Ng * 8 / 7 * w.n_vcycles, "a7 V-cycles: 167 B/pt/cycle unfused x 8/7"),
+           "XC": ("hbm", 32.0 * Ng, "a8 delta_v_kernel: 32 B/pt")}
+    shares = {k: (stage_ms[k] / max(1, stage_calls[k])) for k in stage_ms}
+    tot_stage = sum(stage_ms.values())
+    dom = max(stage_ms, key=lambda k: stage_ms[k])
+    per_kernel = {}
+    peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    hbm_peak, hbm_src = 6650.0, "fallback"
+    if os.path.exists(peaks_file):
+        with open(peaks_file) as f:
+            hbm_peak, hbm_src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    for k, (bound, work, note) in alg.items():
+        if not stage_calls[k]:
+            continue
+        ms = shares[k]
+        if bound == "tensor":
+            ach, peak, unit = work / (ms * 1e-3) / 1e12, peak_dmma, "TFLOP/s"
+        else:
+            ach, peak, unit = work / (ms * 1e-3) / 1e9, hbm_peak, "GB/s"
+        per_kernel[k] = {"bound": bound, "ms_per_call": ms, "share": stage_ms[k] / tot_stage if tot_stage else None,
+                         "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "work": note}
+    traffic = None
+    tfile = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(tfile):
+        with open(tfile) as f:
+            traffic = json.load(f).get(w.name, {}).get(dom)
+    roof = dict(per_kernel[dom])
+    roof.update({"kernel": dom, "traffic": traffic,
+                 "peak_source": ("FP64 DMMA issue rate measured live by rt_probe_fp64_peak in this run "
+                                 f"(DFMA: {peak_dfma:.2f} TFLOP/s)") if roof["bound"] == "tensor" else hbm_src,
+                 "timed": "CUDA events around every stage inside the timed region" if stage_in_timed else
+                 "CUDA events around every stage in a second pass of K steps (graph bypassed) right after the timed region"})
+
+    # CPU baseline: the oracle as it stands on the host cores, bounded sample
+    cpu = None
+    if not args.no_cpu_baseline:
+        cores = threads_used()
+        if big:
+            pts = slab_points(w)
+            slab = phi[:, :pts].contiguous().cpu().numpy()
+            parts, scale = oracle_sample(w, pts, phi_slab=slab, seed=w.seed)
+            sec, t = oracle_step_seconds(w, parts, scale)
+            cpu = {"value": 1.0 / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": (f"one Hamiltonian update of oracle/rt_oracle.py: full {N}^2 eigh propagator + full-grid "
+                              f"Poisson/xc + density & projection on the first {pts} grid points of the same Phi, slab "
+                              f"time x {scale:.1f}, x m = {w.n_hupdates}; measured parts (s): "
+                              + ", ".join(f"{k}={v:.2f}" for k, v in t.items()))}
+        else:
+            o = full_oracle(w)
+            n = 0
+            t0 = time.perf_counter()
+            while n < 3 or (time.perf_counter() - t0 < 10.0 and n < w.nsteps):
+                if w.laser:
+                    o.set_field(w.E_of_t((n + 1) * w.dt))
+                o.step(1)
+                n += 1
+            sec = (time.perf_counter() - t0) / n
+            cpu = {"value": 1.0 / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": f"{n} full oracle steps on the whole workload"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(w, args), "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 24, "d2h_bytes_per_step": 24 + 8 * w.ngrid,
+                    "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": int(launches), "roofline": roof, "per_kernel": per_kernel, "cpu_baseline": cpu,
+            "fp64_peaks_tflops": {"dmma": peak_dmma, "dfma": peak_dfma}, "lib": info,
+            "checks": {"ortho_err": ortho_err, "charge": float(charge[0]), "n_electrons": 2.0 * w.nocc,
+                       "induced_charge": float(charge[1]), "dipole": [float(x) for x in mu]},
+            "setup_s": {"inputs": t_gen}}
+    print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

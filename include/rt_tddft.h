@@ -142,6 +142,12 @@ int rt_timing_enable(rt_handle h, int32_t enable);
  * calls[RT_STAGE_COUNT] (HOST) = number of times each stage ran.  Resets the accumulators. */
 int rt_timing_read(rt_handle h, double ms[RT_STAGE_COUNT], int64_t calls[RT_STAGE_COUNT]);
 
+/* ---- calibration instrument (not on the hot path) ----------------------------------------------------
+ * Measures the FP64 issue-rate ceilings of `device` with register-resident operands: DMMA.8x8x4 (mma.sync
+ * m8n8k4 f64) and DFMA, in TFLOP/s (HOST doubles).  Takes ~0.5 s.  The roofline fractions bench.py reports for
+ * the a1/a3/a4/a5 kernels are quoted against the DMMA figure measured in the same run. */
+int rt_probe_fp64_peak(int32_t device, double* dmma_tflops, double* dfma_tflops);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,7 @@ SYMBOLS = (
     "rt_create", "rt_set_field", "rt_step", "rt_get_dipole", "rt_get_density", "rt_get_pmatrix", "rt_get_hmatrix",
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
-    "rt_timing_enable", "rt_timing_read",
+    "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak",
 )
 
 
@@ -72,6 +72,8 @@ def _load():
         fn = getattr(lib, name)
         fn.argtypes = argtypes
         fn.restype = C.c_int
+    lib.rt_probe_fp64_peak.argtypes = [i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.rt_probe_fp64_peak.restype = C.c_int
     lib.rt_last_error.argtypes = [vp]
     lib.rt_last_error.restype = C.c_char_p
     return lib
@@ -212,6 +214,15 @@ def rt_timing_read(h):
     calls = np.zeros(RT_STAGE_COUNT, dtype=np.int64)
     _check(h, _lib.rt_timing_read(h, _ptr(ms), calls.ctypes.data))
     return dict(zip(RT_STAGE_NAMES, ms.tolist())), dict(zip(RT_STAGE_NAMES, calls.tolist()))
+
+
+def rt_probe_fp64_peak(device=0):
+    """(DMMA TFLOP/s, DFMA TFLOP/s) issue-rate ceilings of the device (calibration instrument)."""
+    a, b = C.c_double(0), C.c_double(0)
+    rc = _lib.rt_probe_fp64_peak(int(device), C.byref(a), C.byref(b))
+    if rc != RT_OK:
+        raise RTError(rc, "rt_probe_fp64_peak failed")
+    return a.value, b.value
 
 
 # ---- convenience wrapper (the call a user makes) -------------------------------------------------------

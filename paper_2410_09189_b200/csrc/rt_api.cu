@@ -258,10 +258,8 @@ void enqueue_step(rt_ctx* c) {
     enqueue_project(c, c->w, c->d_eps, c->H1);                                                 // line 25
     stage_end(c);
   }
-  stage_begin(c, RT_STAGE_ELDYN);
   launch_copy5(c->N, c->ldn, c->Hm1, c->H0, c->H0, c->H1, c->P0r, c->P1r, c->P0i, c->P1i, c->st);   // line 28
   c->launches += 1;
-  stage_end(c);
 }
 
 int sync_and_check(rt_ctx* c) {
@@ -401,17 +399,30 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   {
     ProjectPlan& p = c->pp;
     p.N = N; p.Ng = Ng; p.ntile = ntile; p.T = ntile * (ntile + 1) / 2; p.ldn = ldn;
-    long long S = (2 * prop.multiProcessorCount + p.T - 1) / p.T;
+    // split-K factor: enough CTAs for >= 2 waves when the tile count is small, and T*S chosen to fill whole
+    // waves of one CTA per SM (wave quantisation was 14% of the first nano profile at S = 2: 380 CTAs = 2.57 waves)
+    const int sms = prop.multiProcessorCount;
     const long long kmin = 16 * 8;
-    if (S > (Ng + kmin - 1) / kmin) S = (Ng + kmin - 1) / kmin;
-    if (S < 1) S = 1;
+    long long smax = (Ng + kmin - 1) / kmin;
+    if (smax > 4 * sms) smax = 4 * sms;
+    const double slab_bytes = (double)N * ldn * 8;
+    while (smax > 1 && smax * slab_bytes > 2.0e9) --smax;          // workspace cap
+    long long S = 1;
+    double best = -1.0;
+    for (long long s = 1; s <= smax; ++s) {
+      const long long ctas = (long long)p.T * s;
+      if (ctas < 2LL * sms && s < smax) continue;                   // want at least two waves of work
+      const long long waves = (ctas + sms - 1) / sms;
+      const double eff = (double)ctas / (double)(waves * sms);
+      if (eff > best + 1e-9) { best = eff; S = s; }
+      if (eff > 0.985) break;
+    }
     long long kc = (Ng + S - 1) / S;
     kc = (kc + 15) / 16 * 16;
     p.kchunk = kc;
     p.S = (int)((Ng + kc - 1) / kc);
     DensityPlan& d = c->dp;
     d.N = N; d.Ng = Ng; d.ntile = ntile; d.npairs = (ntile + 1) / 2; d.nrt = (Ng + TILE - 1) / TILE; d.ldn = ldn;
-    const int sms = prop.multiProcessorCount;
     int gr = d.npairs >= 12 ? 12 : (sms + d.npairs - 1) / d.npairs;
     if (gr > d.nrt) gr = (int)d.nrt;
     d.group_r = gr < 1 ? 1 : gr;
