@@ -49,6 +49,8 @@ extern "C" {
 #define RT_NO_HARTREE  2u   /* test aid: drop V_H from dV                                                */
 #define RT_NO_XC       4u   /* test aid: drop vxc(rho) - vxc(rho0) from dV                               */
 #define RT_NO_GRAPH    8u   /* launch kernels directly instead of replaying a CUDA graph of one step     */
+#define RT_NO_TMA     16u   /* use the cp.async versions of the DMMA kernels even where TMA applies (the
+                               library falls back to them by itself when Ng is odd or phi is not 16-byte aligned) */
 
 typedef struct rt_ctx* rt_handle;
 
@@ -99,8 +101,8 @@ int rt_get_time(rt_handle h, double* t);
 /* Integrals of the current density, HOST double[2]: { dVol sum rho , dVol sum (rho - rho0) }.  Synchronises. */
 int rt_get_charge(rt_handle h, double q[2]);
 /* info[0] = exp_order K actually used, info[1] = number of multigrid levels, info[2..4] = coarsest nx,ny,nz,
- * info[5] = 1 if steps replay a CUDA graph, info[6] = kernels launched per step, info[7] = split-K of the
- * projection.  HOST int32[8]. */
+ * info[5] = 1 if steps replay a CUDA graph (+2 if the TMA-fed DMMA kernels are in use), info[6] = kernels launched
+ * per step, info[7] = split-K of the projection.  HOST int32[8]. */
 int rt_get_info(rt_handle h, int32_t info[8]);
 /* Total number of this library's kernel launches enqueued through the handle so far (graph replays count the
  * kernels inside the graph).  HOST. */

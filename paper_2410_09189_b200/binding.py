@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librt_tddft.so")
 
 RT_OK, RT_EINVAL, RT_ENOMEM, RT_ECUDA, RT_ESTATE = 0, -1, -2, -3, -4
-RT_PHI_DEVICE, RT_NO_HARTREE, RT_NO_XC, RT_NO_GRAPH = 1, 2, 4, 8
+RT_PHI_DEVICE, RT_NO_HARTREE, RT_NO_XC, RT_NO_GRAPH, RT_NO_TMA = 1, 2, 4, 8, 16
 RT_STAGE_NAMES = ("Hupdate", "Rho", "Vh", "ELDYN", "XC")      # Table 1 of the paper, L543-L547
 RT_STAGE_COUNT = 5
 
@@ -165,7 +165,8 @@ def rt_get_info(h) -> dict:
     a = np.zeros(8, dtype=np.int32)
     _check(h, _lib.rt_get_info(h, a.ctypes.data))
     return {"exp_order": int(a[0]), "mg_levels": int(a[1]), "coarsest": (int(a[2]), int(a[3]), int(a[4])),
-            "graph": bool(a[5]), "launches_per_step": int(a[6]), "project_split_k": int(a[7])}
+            "graph": bool(a[5] & 1), "tma": bool(a[5] & 2), "launches_per_step": int(a[6]),
+            "project_split_k": int(a[7])}
 
 
 def rt_get_launch_count(h) -> int:
@@ -231,8 +232,8 @@ class RTTDDFT:
     """Owns one rt_handle.  ``phi`` may be a host numpy array (copied) or a CUDA torch tensor (borrowed)."""
 
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
-                 nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, device=0,
-                 stream=None):
+                 nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
+                 device=0, stream=None):
         cfg = rt_config()
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)
         cfg.h, cfg.norb, cfg.dt = float(h), int(len(eps)), float(dt)
@@ -255,6 +256,8 @@ class RTTDDFT:
             flags |= RT_NO_XC
         if not graph:
             flags |= RT_NO_GRAPH
+        if not tma:
+            flags |= RT_NO_TMA
         cfg.flags, cfg.device = flags, int(device)
         if stream is None:
             try:

@@ -1,0 +1,417 @@
+// gemm_tma.cu -- TMA-fed, warp-specialised versions of the three FP64 DMMA stages (the default path on sm_100a;
+// gemm_kernels.cu keeps the cp.async versions for shapes TMA cannot describe: odd Ng or unaligned Phi).
+//
+//   a1 project_tma_kernel : dH_ij = sum_r phi_i(r) dV(r) phi_j(r)   (Table 1 "Hupdate" L543; Alg. 1 line 25)
+//   a5 density_tma_kernel : rho(r) = sum_j phi_j(r) (Pfold Phi)_j(r) ("Rho" L544; Eq. 27), persistent CTAs
+//   a3/a4 gemm_abt_tma    : D = a0 A0 B0^T + a1 A1 B1^T              ("ELDYN" L546)
+//
+// CTA = 8 consumer warps (2 x 4, warp tile 64 x 32 = 8 x 4 DMMA.8x8x4 tiles) + 1 producer warp (one elected lane
+// issues TMA).  6-stage ring, 32 KB per stage (A 128x16 + B 128x16 doubles), full/empty mbarriers.
+#include "rt_internal.h"
+#include "tma_core.cuh"
+
+namespace rt {
+
+namespace {
+
+constexpr int FA = 8, FB = 4, WM = 2, WN = 4;
+constexpr int NCONS = WM * WN;                 // consumer warps
+constexpr int NTHREADS = 32 * (NCONS + 4);     // + one producer warpgroup (only its first lane works)
+// setmaxnreg budget: the CTA is launched with 384 x 168 = 64512 registers; 256*240 + 128*24 = 64512 exactly
+constexpr int REGS_CONSUMER = 240, REGS_PRODUCER = 24;
+constexpr int ST = 6;                          // pipeline stages
+constexpr int TILE_D = TILE * BK;              // doubles in one 128 x 16 operand tile (16 KB)
+constexpr int STAGE_D = 2 * TILE_D;            // A + B
+constexpr uint32_t TILE_BYTES = TILE_D * 8;
+
+struct alignas(8) Bars { unsigned long long full[ST]; unsigned long long empty[ST]; };
+
+// dynamic shared layout: [ST][A|B] (1024-aligned) | weights [ST][16] | barriers | reduce scratch
+constexpr size_t SMEM_TILES = (size_t)ST * STAGE_D * 8;
+constexpr size_t SMEM_W = (size_t)ST * BK * 8;
+constexpr size_t SMEM_RED = (size_t)WM * TILE * 8;
+constexpr size_t SMEM_TOTAL = 1024 + SMEM_TILES + SMEM_W + sizeof(Bars) + SMEM_RED;
+
+__device__ __forceinline__ double* align1024(void* p) {
+  return reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(p) + 1023) & ~uintptr_t(1023));
+}
+
+__device__ __forceinline__ void regs_consumer() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_CONSUMER)); }
+__device__ __forceinline__ void regs_producer() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_PRODUCER)); }
+
+__device__ __forceinline__ void init_bars(Bars* bars) {
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < ST; ++s) {
+      mbar_init(smem_u32(&bars->full[s]), 1);
+      mbar_init(smem_u32(&bars->empty[s]), NCONS);
+    }
+    fence_barrier_init();
+  }
+  __syncthreads();
+}
+
+}  // namespace
+
+// ======================================================================================================
+// a1 projection
+// ======================================================================================================
+__global__ void __launch_bounds__(NTHREADS, 1)
+project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __restrict__ w,
+                   const int2* __restrict__ tiles, double* __restrict__ W, int N, long long Ng, int T,
+                   long long kchunk, int ldn) {
+  extern __shared__ uint8_t smem_raw[];
+  double* tilesm = align1024(smem_raw);
+  double* wsm = tilesm + (size_t)ST * STAGE_D;
+  Bars* bars = reinterpret_cast<Bars*>(wsm + ST * BK);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  init_bars(bars);
+
+  const int s = blockIdx.x / T, t = blockIdx.x % T;
+  const int2 tt = tiles[t];
+  const int i0 = tt.x * TILE, j0 = tt.y * TILE;
+  const long long kbeg = (long long)s * kchunk;
+  const long long kend = (kbeg + kchunk < Ng) ? kbeg + kchunk : Ng;
+  const int nk = (int)((kend - kbeg + BK - 1) / BK);
+
+  if (warp >= NCONS) {
+    // ===== producer =====
+    regs_producer();
+    if (warp == NCONS && lane == 0) {
+      tma_prefetch_desc(&tmPhi);
+      for (int kt = 0; kt < nk; ++kt) {
+        const int slot = kt % ST;
+        if (kt >= ST) mbar_wait(smem_u32(&bars->empty[slot]), ((kt / ST) - 1) & 1);
+        const uint32_t full = smem_u32(&bars->full[slot]);
+        mbar_expect_tx(full, 2 * TILE_BYTES + BK * 8);
+        const long long k0 = kbeg + (long long)kt * BK;
+        double* sA = tilesm + (size_t)slot * STAGE_D;
+        tma_load_2d(sA, &tmPhi, (int)k0, i0, full);
+        tma_load_2d(sA + TILE_D, &tmPhi, (int)k0, j0, full);
+        bulk_load_1d(wsm + slot * BK, w + k0, BK * 8, full);     // w is padded to a multiple of 16 doubles
+      }
+    }
+    return;
+  }
+
+  // ===== consumers =====
+  regs_consumer();
+  const int g = lane >> 2, c = lane & 3, pg = perm8(g);
+  const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
+  double acc[FA][FB][2];
+#pragma unroll
+  for (int a = 0; a < FA; ++a)
+#pragma unroll
+    for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+
+  for (int kt = 0; kt < nk; ++kt) {
+    const int slot = kt % ST;
+    mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
+    const double* sA = tilesm + (size_t)slot * STAGE_D;
+    mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+  }
+
+  // epilogue: raw partial sums into slab s.  MMA row g <-> tile row perm8(g); tile col n' <-> perm8(n')
+  double* Ws = W + (long long)s * N * ldn;
+#pragma unroll
+  for (int a = 0; a < FA; ++a) {
+    const int row = i0 + wrow + 8 * a + pg;
+    if (row < N) {
+#pragma unroll
+      for (int b = 0; b < FB; ++b) {
+        const int col = j0 + wcol + 8 * b + c;        // perm8(2c) = c, perm8(2c+1) = c + 4
+        if (col < N) Ws[(long long)row * ldn + col] = acc[a][b][0];
+        if (col + 4 < N) Ws[(long long)row * ldn + col + 4] = acc[a][b][1];
+      }
+    }
+  }
+}
+
+size_t tma_smem_bytes() { return SMEM_TOTAL; }
+
+void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const double* w, const int2* tiles, double* W,
+                        cudaStream_t st) {
+  project_tma_kernel<<<p.T * p.S, NTHREADS, SMEM_TOTAL, st>>>(tmPhi, w, tiles, W, p.N, p.Ng, p.T, p.kchunk, p.ldn);
+}
+
+// ======================================================================================================
+// a5 density (persistent)
+// ======================================================================================================
+struct DensWork { int pair; long long rt; bool valid; };
+
+__device__ __forceinline__ DensWork dens_decode(long long L, int npairs, long long nrt, int group_r) {
+  const long long per_group = (long long)group_r * npairs;
+  const long long grp = L / per_group, in = L % per_group;
+  const long long r_first = grp * group_r;
+  const long long gr_here = (nrt - r_first < group_r) ? (nrt - r_first) : group_r;
+  DensWork d;
+  d.pair = (int)(in / gr_here);
+  d.rt = r_first + in % gr_here;
+  d.valid = d.pair < npairs && d.rt < nrt;
+  return d;
+}
+
+__global__ void __launch_bounds__(NTHREADS, 1)
+density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmPhiN,
+                   const double* __restrict__ phi, double* __restrict__ rho_part, int N, long long Ng, int ntile,
+                   int npairs, long long nrt, int group_r, long long nwork) {
+  extern __shared__ uint8_t smem_raw[];
+  double* tilesm = align1024(smem_raw);
+  double* wsm = tilesm + (size_t)ST * STAGE_D;
+  Bars* bars = reinterpret_cast<Bars*>(wsm + ST * BK);
+  double* colred = reinterpret_cast<double*>(bars + 1);       // [WM][TILE]
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  init_bars(bars);
+
+  if (warp >= NCONS) {
+    // ===== producer: runs ahead across j-tiles and work items =====
+    regs_producer();
+    if (warp == NCONS && lane == 0) {
+      tma_prefetch_desc(&tmP);
+      tma_prefetch_desc(&tmPhiN);
+      long long it = 0;
+      for (long long L = blockIdx.x; L < nwork; L += gridDim.x) {
+        const DensWork wk = dens_decode(L, npairs, nrt, group_r);
+        if (!wk.valid) continue;
+        const long long r0 = wk.rt * TILE;
+        for (int which = 0; which < 2; ++which) {
+          const int jt = which == 0 ? wk.pair : ntile - 1 - wk.pair;
+          if (which == 1 && jt <= wk.pair) break;
+          const int j0 = jt * TILE;
+          const int nk = (N - j0 + BK - 1) / BK;
+          for (int kt = 0; kt < nk; ++kt, ++it) {
+            const int slot = (int)(it % ST);
+            if (it >= ST) mbar_wait(smem_u32(&bars->empty[slot]), (uint32_t)((it / ST) - 1) & 1);
+            const uint32_t full = smem_u32(&bars->full[slot]);
+            mbar_expect_tx(full, 2 * TILE_BYTES);
+            const int k0 = j0 + kt * BK;
+            double* sA = tilesm + (size_t)slot * STAGE_D;
+            tma_load_2d(sA, &tmP, k0, j0, full);                              // Pfold[j0.., k0..]
+#pragma unroll
+            for (int bx = 0; bx < 8; ++bx)                                    // Phi[k0.., r0 + 16 bx ..]
+              tma_load_2d(sA + TILE_D + bx * 256, &tmPhiN, (int)(r0 + 16 * bx), k0, full);
+          }
+        }
+      }
+    }
+    return;
+  }
+
+  // ===== consumers =====
+  regs_consumer();
+  const int g = lane >> 2, c = lane & 3, pg = perm8(g);
+  const int wm = warp / WN, wn = warp % WN;
+  const int wrow = wm * (8 * FA), wcol = wn * (8 * FB);
+  const int ctid = threadIdx.x;                                 // 0..255
+  const bool vecF = ((Ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(phi) & 15) == 0);
+  long long it = 0;
+  for (long long L = blockIdx.x; L < nwork; L += gridDim.x) {
+    const DensWork wk = dens_decode(L, npairs, nrt, group_r);
+    if (!wk.valid) continue;
+    const long long r0 = wk.rt * TILE;
+    double colsum[FB / 2][4];
+#pragma unroll
+    for (int t = 0; t < FB / 2; ++t)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) colsum[t][q] = 0.0;
+
+    for (int which = 0; which < 2; ++which) {
+      const int jt = which == 0 ? wk.pair : ntile - 1 - wk.pair;
+      if (which == 1 && jt <= wk.pair) break;
+      const int j0 = jt * TILE;
+      const int nk = (N - j0 + BK - 1) / BK;
+      double acc[FA][FB][2];
+#pragma unroll
+      for (int a = 0; a < FA; ++a)
+#pragma unroll
+        for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+
+      for (int kt = 0; kt < nk; ++kt, ++it) {
+        const int slot = (int)(it % ST);
+        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        const double* sA = tilesm + (size_t)slot * STAGE_D;
+        mma_stage_nc_tma<FA, FB>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+      }
+
+      // fused row-dot: colsum(r) += sum_j phi_j(r) T_j(r); lane owns columns wcol + 16 t + 4 c + {0..3}
+#pragma unroll
+      for (int a = 0; a < FA; ++a) {
+        const int j = j0 + wrow + 8 * a + pg;
+        if (j < N) {
+          const double* prow = phi + (long long)j * Ng + r0 + wcol + 4 * c;
+#pragma unroll
+          for (int t = 0; t < FB / 2; ++t) {
+            const long long col = r0 + wcol + 16 * t + 4 * c;
+            double f[4];
+            if (vecF && col + 3 < Ng) {
+              const double2 f01 = *reinterpret_cast<const double2*>(prow + 16 * t);
+              const double2 f23 = *reinterpret_cast<const double2*>(prow + 16 * t + 2);
+              f[0] = f01.x; f[1] = f01.y; f[2] = f23.x; f[3] = f23.y;
+            } else {
+#pragma unroll
+              for (int q = 0; q < 4; ++q) f[q] = (col + q < Ng) ? prow[16 * t + q] : 0.0;
+            }
+            colsum[t][0] += f[0] * acc[a][2 * t][0];
+            colsum[t][1] += f[1] * acc[a][2 * t + 1][0];
+            colsum[t][2] += f[2] * acc[a][2 * t][1];
+            colsum[t][3] += f[3] * acc[a][2 * t + 1][1];
+          }
+        }
+      }
+    }
+
+    // reduce over the 8 row groups of the warp, then over the WM warps sharing columns
+#pragma unroll
+    for (int t = 0; t < FB / 2; ++t)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        double v = colsum[t][q];
+        v += __shfl_xor_sync(0xffffffffu, v, 4);
+        v += __shfl_xor_sync(0xffffffffu, v, 8);
+        v += __shfl_xor_sync(0xffffffffu, v, 16);
+        colsum[t][q] = v;
+      }
+    if (g == 0) {
+#pragma unroll
+      for (int t = 0; t < FB / 2; ++t)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) colred[wm * TILE + wcol + 16 * t + 4 * c + q] = colsum[t][q];
+    }
+    consumer_sync(32 * NCONS);
+    if (ctid < TILE) {
+      const long long r = r0 + ctid;
+      if (r < Ng) {
+        double v = 0.0;
+#pragma unroll
+        for (int m = 0; m < WM; ++m) v += colred[m * TILE + ctid];
+        rho_part[(long long)wk.pair * Ng + r] = v;
+      }
+    }
+    consumer_sync(32 * NCONS);
+  }
+}
+
+void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, const double* phi,
+                        double* rho_part, int sms, cudaStream_t st) {
+  const long long ngroups = (p.nrt + p.group_r - 1) / p.group_r;
+  const long long nwork = ngroups * p.group_r * p.npairs;
+  const long long grid = nwork < sms ? nwork : sms;
+  density_tma_kernel<<<(unsigned)grid, NTHREADS, SMEM_TOTAL, st>>>(tmP, tmPhiN, phi, rho_part, p.N, p.Ng, p.ntile,
+                                                                   p.npairs, p.nrt, p.group_r, nwork);
+}
+
+// ======================================================================================================
+// a3/a4 N x N GEMM
+// ======================================================================================================
+struct GemmTmaArgs {
+  int N, ldn, nterms;
+  double alpha0, alpha1;
+  double* D; double* Z1; double beta1; double* Z2; double beta2;
+};
+
+__global__ void __launch_bounds__(NTHREADS, 1)
+gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmB0,
+                    const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmB1,
+                    GemmTmaArgs ga) {
+  extern __shared__ uint8_t smem_raw[];
+  double* tilesm = align1024(smem_raw);
+  double* wsm = tilesm + (size_t)ST * STAGE_D;
+  Bars* bars = reinterpret_cast<Bars*>(wsm + ST * BK);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  init_bars(bars);
+  const int N = ga.N, ldn = ga.ldn;
+  const int i0 = blockIdx.y * TILE, j0 = blockIdx.x * TILE;
+  const int nk1 = (N + BK - 1) / BK;
+  const int nk = ga.nterms * nk1;
+
+  if (warp >= NCONS) {
+    regs_producer();
+    if (warp == NCONS && lane == 0) {
+      tma_prefetch_desc(&tmA0);
+      tma_prefetch_desc(&tmB0);
+      for (int kt = 0; kt < nk; ++kt) {
+        const int slot = kt % ST;
+        if (kt >= ST) mbar_wait(smem_u32(&bars->empty[slot]), ((kt / ST) - 1) & 1);
+        const uint32_t full = smem_u32(&bars->full[slot]);
+        mbar_expect_tx(full, 2 * TILE_BYTES);
+        const bool second = kt >= nk1;
+        const int k0 = (second ? kt - nk1 : kt) * BK;
+        double* sA = tilesm + (size_t)slot * STAGE_D;
+        tma_load_2d(sA, second ? &tmA1 : &tmA0, k0, i0, full);
+        tma_load_2d(sA + TILE_D, second ? &tmB1 : &tmB0, k0, j0, full);
+      }
+    }
+    return;
+  }
+
+  regs_consumer();
+  const int g = lane >> 2, c = lane & 3, pg = perm8(g);
+  const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
+  double acc[FA][FB][2];
+#pragma unroll
+  for (int a = 0; a < FA; ++a)
+#pragma unroll
+    for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+  const double ratio = ga.nterms == 2 ? ga.alpha1 / ga.alpha0 : 1.0;
+
+  for (int kt = 0; kt < nk; ++kt) {
+    const int slot = kt % ST;
+    mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
+    if (kt == nk1 && ratio != 1.0) {            // fold alpha1/alpha0 (+-1 in this library: exact) into the accumulators
+      const double inv = 1.0 / ratio;
+#pragma unroll
+      for (int a = 0; a < FA; ++a)
+#pragma unroll
+        for (int b = 0; b < FB; ++b) { acc[a][b][0] *= inv; acc[a][b][1] *= inv; }
+    }
+    const double* sA = tilesm + (size_t)slot * STAGE_D;
+    mma_stage_kc_tma<FA, FB, false>(acc, sA, sA + TILE_D, nullptr, wrow, wcol, pg, c);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+  }
+  const double fin = (ga.nterms == 2 && ratio != 1.0) ? ga.alpha0 * ratio : ga.alpha0;
+
+#pragma unroll
+  for (int a = 0; a < FA; ++a) {
+    const int row = i0 + wrow + 8 * a + pg;
+    if (row < N) {
+#pragma unroll
+      for (int b = 0; b < FB; ++b) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int col = j0 + wcol + 8 * b + c + 4 * e;
+          if (col < N) {
+            const long long o = (long long)row * ldn + col;
+            const double d = fin * acc[a][b][e];
+            if (ga.D) ga.D[o] = d;
+            if (ga.Z1) ga.Z1[o] += ga.beta1 * d;
+            if (ga.Z2) ga.Z2[o] += ga.beta2 * d;
+          }
+        }
+      }
+    }
+  }
+}
+
+void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
+                         const CUtensorMap& tmB1, cudaStream_t st) {
+  GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2};
+  const int nt = (g.N + TILE - 1) / TILE;
+  gemm_abt_tma_kernel<<<dim3(nt, nt), NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
+}
+
+int init_tma_kernels() {
+  cudaError_t e;
+  e = cudaFuncSetAttribute(project_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
+  if (e != cudaSuccess) return (int)e;
+  e = cudaFuncSetAttribute(density_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
+  if (e != cudaSuccess) return (int)e;
+  e = cudaFuncSetAttribute(gemm_abt_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
+  return (int)e;
+}
+
+}  // namespace rt

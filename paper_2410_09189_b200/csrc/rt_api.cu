@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -56,6 +57,13 @@ struct rt_ctx {
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t gexec = nullptr;
 
+  // TMA descriptors: Phi as a K-contiguous operand (box 16 x 128) and as an N-contiguous one (box 16 x 16);
+  // one K-contiguous descriptor per library-owned N x N buffer
+  bool use_tma = false;
+  int sms = 148;
+  CUtensorMap tmPhiK{}, tmPhiN{};
+  std::map<const double*, CUtensorMap> tmN;
+
   bool timing = false;
   std::vector<EventPair> ev_used;
   std::vector<EventPair> ev_free;
@@ -98,6 +106,7 @@ int dev_alloc(rt_ctx* c, T** p, size_t count) {
 }
 
 int roundup(int x, int m) { return (x + m - 1) / m * m; }
+constexpr int BK_HOST = 16;      // doubles per pipeline stage (dmma_core.cuh BK)
 
 // real orthonormal eigenvectors of the periodic 1-D second-difference operator: column 0 constant,
 // then (cos_k, sin_k) pairs, then the alternating vector when n is even.  lam[col] = (2 - 2 cos(2 pi k/n))/h^2.
@@ -129,6 +138,46 @@ bool can_coarsen(const GridDims& g) {
   return g.nx % 2 == 0 && g.ny % 2 == 0 && g.nz % 2 == 0 && g.nx > 4 && g.ny > 4 && g.nz > 4;
 }
 
+// ---- TMA descriptors -------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+    else
+      cudaGetLastError();
+  }
+  return fn;
+}
+// row-major FP64 matrix [rows][cols] with leading dimension ld (doubles); box = {box_cols, box_rows}; 128B swizzle
+bool make_map(CUtensorMap* m, const double* base, long long rows, long long cols, long long ld, int box_cols,
+              int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 8};
+  cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
+  cuuint32_t es[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+const CUtensorMap& nn_map(rt_ctx* c, const double* p) {
+  auto it = c->tmN.find(p);
+  if (it == c->tmN.end()) {
+    CUtensorMap m{};
+    make_map(&m, p, c->N, c->N, c->ldn, BK_HOST, TILE);
+    it = c->tmN.emplace(p, m).first;
+  }
+  return it->second;
+}
+
 // ---- stage timing helpers ------------------------------------------------------------------------
 void stage_begin(rt_ctx* c, int stage) {
   if (!c->timing) return;
@@ -148,7 +197,13 @@ void stage_end(rt_ctx* c) {
 void enqueue_gemm(rt_ctx* c, const double* A0, const double* B0, double a0, const double* A1, const double* B1,
                   double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr, double b2 = 0) {
   GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2};
-  launch_gemm_abt(g, c->st);
+  if (c->use_tma) {
+    const CUtensorMap& mA0 = nn_map(c, A0);
+    const CUtensorMap& mB0 = nn_map(c, B0);
+    launch_gemm_abt_tma(g, mA0, mB0, A1 ? nn_map(c, A1) : mA0, B1 ? nn_map(c, B1) : mB0, c->st);
+  } else {
+    launch_gemm_abt(g, c->st);
+  }
   c->launches += 1;
 }
 
@@ -182,7 +237,8 @@ void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, doub
 
 void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double* rho0) {
   launch_fold_upper(c->N, c->ldn, reP, c->X, c->st);
-  launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
+  if (c->use_tma) launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phi, c->rho_part, c->sms, c->st);
+  else launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
   launch_reduce_rho(c->rho_part, c->dp.npairs, c->Ng, c->gd, c->h, rho0, rho_out, c->d_bsums, c->d_sums, c->st);
   c->launches += 4;
 }
@@ -222,7 +278,8 @@ void enqueue_vcycle(rt_ctx* c, std::vector<MgLevel>& lv, size_t l) {
 }
 
 void enqueue_project(rt_ctx* c, const double* w, const double* eps, double* H) {
-  launch_project(c->pp, c->phi, w, c->d_tiles, c->W, c->st);
+  if (c->use_tma) launch_project_tma(c->pp, c->tmPhiK, w, c->d_tiles, c->W, c->st);
+  else launch_project(c->pp, c->phi, w, c->d_tiles, c->W, c->st);
   launch_project_reduce(c->pp, c->W, eps, c->dvol, H, c->st);
   c->launches += 2;
 }
@@ -452,6 +509,17 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     CKC(cudaMemcpyAsync(c->phi_owned, phi, (size_t)N * Ng * 8, cudaMemcpyHostToDevice, c->st));
     c->phi = c->phi_owned;
   }
+  c->sms = prop.multiProcessorCount;
+  c->use_tma = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && ((reinterpret_cast<uintptr_t>(c->phi) & 15) == 0) &&
+               get_encode_fn() != nullptr;
+  if (c->use_tma) {
+    if (!make_map(&c->tmPhiK, c->phi, N, Ng, Ng, BK_HOST, TILE) || !make_map(&c->tmPhiN, c->phi, N, Ng, Ng, 16, BK_HOST))
+      c->use_tma = false;
+  }
+  if (c->use_tma) {
+    const int e = init_tma_kernels();
+    if (e != 0) FAIL_CREATE(RT_ECUDA, std::string("init_tma_kernels: ") + cudaGetErrorString((cudaError_t)e));
+  }
   const size_t nn = (size_t)N * ldn;
   ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8); ALLOC(c->d_sums, 8);
   ALLOC(c->d_bsums, 5 * 1024);
@@ -459,7 +527,10 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
                      &c->P0r, &c->P0i, &c->P1r, &c->P1i};
   for (double** mp : mats) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
   ALLOC(c->W, (size_t)c->pp.S * nn);
-  ALLOC(c->rho, Ng); ALLOC(c->rho0, Ng); ALLOC(c->vxc0, Ng); ALLOC(c->w, Ng); ALLOC(c->op_u, Ng);
+  ALLOC(c->rho, Ng); ALLOC(c->rho0, Ng); ALLOC(c->vxc0, Ng);
+  ALLOC(c->w, Ng + 16); ALLOC(c->op_u, Ng + 16);      // projection weights: the TMA path reads whole 16-double stages
+  CKC(cudaMemsetAsync(c->w, 0, (size_t)(Ng + 16) * 8, c->st));
+  CKC(cudaMemsetAsync(c->op_u, 0, (size_t)(Ng + 16) * 8, c->st));
   ALLOC(c->rho_part, (size_t)c->dp.npairs * Ng);
   for (size_t l = 0; l < c->lv.size(); ++l) {
     MgLevel& L = c->lv[l];
@@ -638,7 +709,7 @@ int rt_get_info(rt_handle c, int32_t info[8]) {
   info[0] = 2 * c->q + 1;
   info[1] = (int32_t)c->lv.size();
   info[2] = L.gd.nx; info[3] = L.gd.ny; info[4] = L.gd.nz;
-  info[5] = c->gexec ? 1 : 0;
+  info[5] = (c->gexec ? 1 : 0) | (c->use_tma ? 2 : 0);
   info[6] = (int32_t)c->launches_per_step;
   info[7] = c->pp.S;
   return RT_OK;

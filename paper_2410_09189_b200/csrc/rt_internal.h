@@ -1,6 +1,7 @@
 // rt_internal.h -- launcher prototypes shared between the kernel translation units and rt_api.cu.
 // Not part of the public ABI (that is include/rt_tddft.h).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -53,6 +54,18 @@ struct GemmArgs {
 };
 void launch_gemm_abt(const GemmArgs& g, cudaStream_t st);
 size_t gemm_smem_bytes();
+
+// ---- TMA-fed, warp-specialised versions (gemm_tma.cu): default on sm_100a when Phi rows are 16-byte aligned ----
+int    init_tma_kernels();                 // sets the dynamic shared-memory attribute; returns a cudaError_t value
+size_t tma_smem_bytes();
+// tmPhi: Phi [N][Ng] with box {16 k, 128 rows}; w must be readable up to roundup(Ng, 16) doubles
+void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const double* w, const int2* tiles, double* W,
+                        cudaStream_t st);
+// tmP: Pfold [N][N] (ld = ldn) box {16, 128}; tmPhiN: Phi with box {16 r, 16 k-rows}
+void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, const double* phi,
+                        double* rho_part, int sms, cudaStream_t st);
+void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
+                         const CUtensorMap& tmB1, cudaStream_t st);
 
 // ---- elementwise N x N (a2 and series glue) -------------------------------------------------------------
 // first != 0: H1 = 2 H0 - Hm1 first.  X = dt * ((H0 + H1)/2 - sigma I)

@@ -1,0 +1,142 @@
+// tma_core.cuh -- TMA + mbarrier producer/consumer machinery for the FP64 DMMA kernels (sm_100a).
+//
+// One producer thread issues cp.async.bulk.tensor (SASS UTMALDG) loads of hardware-swizzled (SWIZZLE_128B) tiles
+// into a ring of shared-memory stages and arms a "full" mbarrier with the byte count; 8 consumer warps wait on it,
+// run LDS.128 + DMMA.8x8x4 only, and release the stage through an "empty" mbarrier (one arrival per warp).  No
+// CTA-wide barrier and no address arithmetic sits on the MMA warps (the first ncu capture showed 1.4 bookkeeping
+// instructions per DMMA and a per-stage __syncthreads holding the tensor pipe at ~80 %).
+//
+// Shared tile layouts produced by TMA with CU_TENSOR_MAP_SWIZZLE_128B (16-byte chunk index ^= 128-byte-row index & 7):
+//   K-contiguous operand: box {16 doubles (k), 128 rows}  -> [128][16] doubles, chunk ch of row r at ch ^ (r & 7)
+//   N-contiguous operand: 8 boxes {16 doubles (n), 16 k-rows}, box bx covers columns 16 bx .. 16 bx + 15
+//                         -> [8][16][16] doubles, chunk ch of k-row k at ch ^ (k & 7)
+// Conflict-free 128-bit fragment reads need the two rows a quarter-warp touches to differ in bit 2 of (r & 7), so
+// MMA row g of an 8-row block reads shared row perm(g) = (g >> 1) | ((g & 1) << 2); the epilogues undo the permutation.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dmma_core.cuh"
+
+namespace rt {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+// Waits for the phase with the given parity.  A pipeline bug would otherwise hang the GPU until the driver's
+// watchdog fires, so after ~10 s of polling the kernel traps (the launch then fails loudly with a CUDA error).
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  if (mbar_try_wait(bar, parity)) return;
+  const long long t0 = clock64();
+  while (!mbar_try_wait(bar, parity)) {
+    if (clock64() - t0 > 20000000000LL) __trap();
+  }
+}
+__device__ __forceinline__ void fence_barrier_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+// 2-D tiled TMA load: coordinates (c0 = inner/contiguous element index, c1 = row index)
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+// 1-D bulk copy (bytes multiple of 16, both addresses 16-byte aligned)
+__device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+// barrier among the consumer warps only (named barrier 1)
+__device__ __forceinline__ void consumer_sync(int nthreads) {
+  asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+}
+
+__device__ __forceinline__ int perm8(int g) { return (g >> 1) | ((g & 1) << 2); }
+
+// ---- one pipeline stage of MMAs on TMA-swizzled tiles ---------------------------------------------------
+// A, B K-contiguous ([128][16], 128B swizzle).  pg = perm8(lane >> 2), c = lane & 3.
+template <int FA, int FB, bool SCALE>
+__device__ __forceinline__ void mma_stage_kc_tma(double (&acc)[FA][FB][2], const double* __restrict__ smA,
+                                                 const double* __restrict__ smB, const double* __restrict__ wk,
+                                                 int wrow, int wcol, int pg, int c) {
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    const int off = pg * BK + (((c + 4 * half) ^ pg) << 1);
+    double2 af[FA], bf[FB];
+#pragma unroll
+    for (int a = 0; a < FA; ++a) af[a] = *reinterpret_cast<const double2*>(smA + (wrow + 8 * a) * BK + off);
+#pragma unroll
+    for (int b = 0; b < FB; ++b) bf[b] = *reinterpret_cast<const double2*>(smB + (wcol + 8 * b) * BK + off);
+    if (SCALE) {
+      const double2 w = *reinterpret_cast<const double2*>(wk + ((c + 4 * half) << 1));
+#pragma unroll
+      for (int b = 0; b < FB; ++b) { bf[b].x *= w.x; bf[b].y *= w.y; }
+    }
+#pragma unroll
+    for (int a = 0; a < FA; ++a)
+#pragma unroll
+      for (int b = 0; b < FB; ++b) dmma884(acc[a][b][0], acc[a][b][1], af[a].x, bf[b].x);
+#pragma unroll
+    for (int a = 0; a < FA; ++a)
+#pragma unroll
+      for (int b = 0; b < FB; ++b) dmma884(acc[a][b][0], acc[a][b][1], af[a].y, bf[b].y);
+  }
+}
+
+// A K-contiguous, B N-contiguous in 8 boxes of [16 k][16 n].  Lane g = lane >> 2 reads chunk g of box
+// (wcol/16 + t) at k-row k: columns 16 t + 2 g + {0,1} -> n-tiles 2t, 2t+1 (same interleave as dmma_core.cuh).
+template <int FA, int FB>
+__device__ __forceinline__ void mma_stage_nc_tma(double (&acc)[FA][FB][2], const double* __restrict__ smA,
+                                                 const double* __restrict__ smB, int wrow, int wcol, int g, int pg,
+                                                 int c) {
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    const int off = pg * BK + (((c + 4 * half) ^ pg) << 1);
+    double2 af[FA];
+#pragma unroll
+    for (int a = 0; a < FA; ++a) af[a] = *reinterpret_cast<const double2*>(smA + (wrow + 8 * a) * BK + off);
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const int k = 2 * c + 8 * half + e;
+      double2 bf[FB / 2];
+#pragma unroll
+      for (int t = 0; t < FB / 2; ++t)
+        bf[t] = *reinterpret_cast<const double2*>(smB + ((wcol >> 4) + t) * 256 + k * BK + ((g ^ (k & 7)) << 1));
+#pragma unroll
+      for (int a = 0; a < FA; ++a)
+#pragma unroll
+        for (int t = 0; t < FB / 2; ++t) {
+          const double av = e ? af[a].y : af[a].x;
+          dmma884(acc[a][2 * t][0], acc[a][2 * t][1], av, bf[t].x);
+          dmma884(acc[a][2 * t + 1][0], acc[a][2 * t + 1][1], av, bf[t].y);
+        }
+    }
+  }
+}
+
+}  // namespace rt

@@ -61,6 +61,8 @@ WORKLOADS = {
     "24k_twin": Workload("24k_twin", (52, 52, 52), 0.40, 1625, 1500, (-0.5, 0.3), 0.2, 20, 3, 2005, kick=(1e-4, 0, 0)),
     # ragged: odd orbital count, non-cubic grid with three different multigrid depths/coarsest sizes
     "ragged": Workload("ragged", (20, 12, 28), 0.33, 37, 11, (-0.9, 0.4), 0.15, 20, 2, 3001, kick=(2e-3, 1e-3, -1e-3)),
+    # odd everything: Ng = 315 is odd (TMA cannot describe Phi -> cp.async kernels), a single multigrid level
+    "odd": Workload("odd", (9, 5, 7), 0.4, 10, 3, (-0.7, 0.3), 0.2, 20, 2, 3002, kick=(0.05, -0.02, 0.03)),
 }
 
 

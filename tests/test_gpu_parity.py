@@ -246,6 +246,27 @@ def test_device_phi_borrowed_and_device_outputs(B):
     gpu.close()
 
 
+def test_cp_async_fallback_paths(B):
+    """RT_NO_TMA forces the cp.async DMMA kernels; an odd Ng selects them automatically (and has one MG level)."""
+    w, Phi, eps, occ = inputs("tiny")
+    ws = strong_kick(w, 0.1)
+    gpu = B.RTTDDFT(ws.shape, ws.h, Phi, eps, occ, ws.dt, E0=ws.kick, n_vcycles=ws.n_vcycles, tma=False)
+    cpu = O.RTOracle(ws.shape, ws.h, Phi, eps, occ, dt=ws.dt, E0=ws.kick, n_vcycles=ws.n_vcycles)
+    assert not gpu.info()["tma"]
+    check_run(B, gpu, cpu, ws, 10)
+    gpu.close()
+    w, Phi, eps, occ = inputs("odd")
+    gpu, cpu = make_pair(B, w, Phi, eps, occ)
+    assert not gpu.info()["tma"] and gpu.info()["mg_levels"] == 1
+    check_run(B, gpu, cpu, w, 20)
+    gpu.close()
+    # and the default path on an even grid does use TMA
+    w, Phi, eps, occ = inputs("tiny")
+    gpu = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt)
+    assert gpu.info()["tma"]
+    gpu.close()
+
+
 def test_zero_steps_and_initial_state(B):
     w, Phi, eps, occ = inputs("tiny")
     gpu, cpu = make_pair(B, w, Phi, eps, occ)
