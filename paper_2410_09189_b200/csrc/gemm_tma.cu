@@ -32,8 +32,11 @@ constexpr size_t SMEM_W = (size_t)ST * BK * 8;
 constexpr size_t SMEM_RED = (size_t)WM * TILE * 8;
 constexpr size_t SMEM_TOTAL = 1024 + SMEM_TILES + SMEM_W + sizeof(Bars) + SMEM_RED;
 
-__device__ __forceinline__ double* align1024(void* p) {
-  return reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(p) + 1023) & ~uintptr_t(1023));
+// 1024-byte alignment of the tile ring (128B-swizzle atom).  The offset is added to the __shared__ array itself so the
+// compiler keeps the shared address space (fragment reads must be LDS.128, not generic LD).
+__device__ __forceinline__ double* align1024(uint8_t* p) {
+  const uint32_t a = smem_u32(p);
+  return reinterpret_cast<double*>(p + ((1024u - (a & 1023u)) & 1023u));
 }
 
 __device__ __forceinline__ void regs_consumer() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_CONSUMER)); }
@@ -156,7 +159,7 @@ __device__ __forceinline__ DensWork dens_decode(long long L, int npairs, long lo
 __global__ void __launch_bounds__(NTHREADS, 1)
 density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmPhiN,
                    const double* __restrict__ phi, double* __restrict__ rho_part, int N, long long Ng, int ntile,
-                   int npairs, long long nrt, int group_r, long long nwork) {
+                   int npairs, long long nrt, int group_r, long long nwork, int b3d) {
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -189,9 +192,13 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
             const int k0 = j0 + kt * BK;
             double* sA = tilesm + (size_t)slot * STAGE_D;
             tma_load_2d(sA, &tmP, k0, j0, full);                              // Pfold[j0.., k0..]
+            if (b3d) {                                                        // Phi[k0.., r0 .. r0+127] in one op
+              tma_load_3d(sA + TILE_D, &tmPhiN, 0, k0, (int)(r0 >> 4), full);
+            } else {
 #pragma unroll
-            for (int bx = 0; bx < 8; ++bx)                                    // Phi[k0.., r0 + 16 bx ..]
-              tma_load_2d(sA + TILE_D + bx * 256, &tmPhiN, (int)(r0 + 16 * bx), k0, full);
+              for (int bx = 0; bx < 8; ++bx)                                  // Phi[k0.., r0 + 16 bx ..]
+                tma_load_2d(sA + TILE_D + bx * 256, &tmPhiN, (int)(r0 + 16 * bx), k0, full);
+            }
           }
         }
       }
@@ -295,13 +302,13 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
   }
 }
 
-void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, const double* phi,
-                        double* rho_part, int sms, cudaStream_t st) {
+void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, int b3d,
+                        const double* phi, double* rho_part, int sms, cudaStream_t st) {
   const long long ngroups = (p.nrt + p.group_r - 1) / p.group_r;
   const long long nwork = ngroups * p.group_r * p.npairs;
   const long long grid = nwork < sms ? nwork : sms;
   density_tma_kernel<<<(unsigned)grid, NTHREADS, SMEM_TOTAL, st>>>(tmP, tmPhiN, phi, rho_part, p.N, p.Ng, p.ntile,
-                                                                   p.npairs, p.nrt, p.group_r, nwork);
+                                                                   p.npairs, p.nrt, p.group_r, nwork, b3d);
 }
 
 // ======================================================================================================

@@ -62,6 +62,7 @@ struct rt_ctx {
   bool use_tma = false;
   int sms = 148;
   CUtensorMap tmPhiK{}, tmPhiN{};
+  int phiN_3d = 0;
   std::map<const double*, CUtensorMap> tmN;
 
   bool timing = false;
@@ -168,6 +169,19 @@ bool make_map(CUtensorMap* m, const double* base, long long rows, long long cols
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
+// Phi [N][Ng] viewed as {16 (r low), N (k), Ng/16 (r high)}: one box {16, 16, 8} lands in shared memory as 8
+// consecutive [16 k][16 r] sub-tiles, the layout the density kernel's B fragments read
+bool make_map_phi3d(CUtensorMap* m, const double* base, long long N, long long Ng) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn || Ng % 16) return false;
+  cuuint64_t dims[3] = {16, (cuuint64_t)N, (cuuint64_t)(Ng / 16)};
+  cuuint64_t strides[2] = {(cuuint64_t)Ng * 8, 128};
+  cuuint32_t box[3] = {16, 16, 8};
+  cuuint32_t es[3] = {1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 const CUtensorMap& nn_map(rt_ctx* c, const double* p) {
   auto it = c->tmN.find(p);
   if (it == c->tmN.end()) {
@@ -237,7 +251,7 @@ void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, doub
 
 void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double* rho0) {
   launch_fold_upper(c->N, c->ldn, reP, c->X, c->st);
-  if (c->use_tma) launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phi, c->rho_part, c->sms, c->st);
+  if (c->use_tma) launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phiN_3d, c->phi, c->rho_part, c->sms, c->st);
   else launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
   launch_reduce_rho(c->rho_part, c->dp.npairs, c->Ng, c->gd, c->h, rho0, rho_out, c->d_bsums, c->d_sums, c->st);
   c->launches += 4;
@@ -513,8 +527,9 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   c->use_tma = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && ((reinterpret_cast<uintptr_t>(c->phi) & 15) == 0) &&
                get_encode_fn() != nullptr;
   if (c->use_tma) {
-    if (!make_map(&c->tmPhiK, c->phi, N, Ng, Ng, BK_HOST, TILE) || !make_map(&c->tmPhiN, c->phi, N, Ng, Ng, 16, BK_HOST))
-      c->use_tma = false;
+    if (!make_map(&c->tmPhiK, c->phi, N, Ng, Ng, BK_HOST, TILE)) c->use_tma = false;
+    else if (make_map_phi3d(&c->tmPhiN, c->phi, N, Ng)) c->phiN_3d = 1;
+    else if (!make_map(&c->tmPhiN, c->phi, N, Ng, Ng, 16, BK_HOST)) c->use_tma = false;
   }
   if (c->use_tma) {
     const int e = init_tma_kernels();

@@ -61,9 +61,10 @@ size_t tma_smem_bytes();
 // tmPhi: Phi [N][Ng] with box {16 k, 128 rows}; w must be readable up to roundup(Ng, 16) doubles
 void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const double* w, const int2* tiles, double* W,
                         cudaStream_t st);
-// tmP: Pfold [N][N] (ld = ldn) box {16, 128}; tmPhiN: Phi with box {16 r, 16 k-rows}
-void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, const double* phi,
-                        double* rho_part, int sms, cudaStream_t st);
+// tmP: Pfold [N][N] (ld = ldn) box {16, 128}; tmPhiN: Phi with box {16 r, 16 k-rows} (b3d = 0: 8 loads per stage)
+// or, when Ng % 16 == 0, the 3-D view {16 r-low, N k, Ng/16 r-high} with box {16, 16, 8} (b3d = 1: one load)
+void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, int b3d,
+                        const double* phi, double* rho_part, int sms, cudaStream_t st);
 void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
                          const CUtensorMap& tmB1, cudaStream_t st);
 
