@@ -278,11 +278,13 @@ def main():
         sampler = ClockSampler(local) if rank == 0 else None
         l0 = B.rt_get_launch_count(sim.handle)
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.profiler.start()          # no-op unless run under `ncu --profile-from-start off`
         ev0.record(stream)
         for _ in range(args.steps):
             one_step()
         ev1.record(stream)
         torch.cuda.synchronize()
+        torch.cuda.profiler.stop()
         if world > 1:
             dist.barrier()
         ms_total = ev0.elapsed_time(ev1)
@@ -361,10 +363,13 @@ def main():
         per_kernel[k] = {"bound": bound, "ms_per_call": ms, "share": stage_ms[k] / tot_stage if tot_stage else None,
                          "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "work": note}
     traffic = None
-    tfile = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    tfile = os.path.join(ROOT, "profiles", "roofline_traffic.csv")     # per-launch DRAM bytes from ncu --set full
     if os.path.exists(tfile):
+        import csv
         with open(tfile) as f:
-            traffic = json.load(f).get(w.name, {}).get(dom)
+            for row in csv.DictReader(f):
+                if row["workload"] == w.name and row["stage"] == dom:
+                    traffic = float(row["dram_bytes_per_launch"])
     roof = dict(per_kernel[dom])
     roof.update({"kernel": dom, "traffic": traffic,
                  "peak_source": ("FP64 DMMA issue rate measured live by rt_probe_fp64_peak in this run "
