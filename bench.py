@@ -339,8 +339,9 @@ def main():
     N, Ng = w.norb, w.ngrid
     alg = {"Hupdate": ("tensor", N * (N + 1.0) * Ng, "a1 projection project_kernel: N(N+1)Ng flop per launch (symmetric output)"),
            "Rho": ("tensor", 1.0 * N * N * Ng, "a5 density density_kernel: N^2 Ng flop per launch (triangular fold)"),
-           "ELDYN": ("tensor", (2.0 * (info["exp_order"] // 2 + 1) + 16.0) * N ** 3,
-                     "a3+a4 gemm_abt_kernel: (q+1) series GEMMs + 8 for U P U^dagger, 2N^3 each"),
+           "ELDYN": ("tensor", ((info["exp_order"] // 2 + 1) + 12.0) * N ** 3,
+                     "a3+a4 gemm_abt_tma_kernel: (q+1) symmetric-output series GEMMs (N^3 each) + U P U^dagger "
+                     "(2 full dual GEMMs 8N^3 + Hermitian output 4N^3)"),
            "Vh": ("hbm", 167.0 * Ng * 8 / 7 * w.n_vcycles, "a7 V-cycles: 167 B/pt/cycle unfused x 8/7"),
            "XC": ("hbm", 32.0 * Ng, "a8 delta_v_kernel: 32 B/pt")}
     shares = {k: (stage_ms[k] / max(1, stage_calls[k])) for k in stage_ms}

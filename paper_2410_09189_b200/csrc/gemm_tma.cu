@@ -142,24 +142,27 @@ void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const do
 // ======================================================================================================
 // a5 density (persistent)
 // ======================================================================================================
-struct DensWork { int pair; long long rt; bool valid; };
+// Work item = (type, r-tile).  A type is one or two k-segments of one j-tile each (table built on the host,
+// rt_api.cu build_density_types): all types cost about the same number of stages, every type owns one row of the
+// partial-sum array.  Items are rastered in groups of group_r r-tiles x all types, r-tile fastest.
+struct DensWork { int type; long long rt; bool valid; };
 
-__device__ __forceinline__ DensWork dens_decode(long long L, int npairs, long long nrt, int group_r) {
-  const long long per_group = (long long)group_r * npairs;
+__device__ __forceinline__ DensWork dens_decode(long long L, int ntypes, long long nrt, int group_r) {
+  const long long per_group = (long long)group_r * ntypes;
   const long long grp = L / per_group, in = L % per_group;
   const long long r_first = grp * group_r;
   const long long gr_here = (nrt - r_first < group_r) ? (nrt - r_first) : group_r;
   DensWork d;
-  d.pair = (int)(in / gr_here);
+  d.type = (int)(in / gr_here);
   d.rt = r_first + in % gr_here;
-  d.valid = d.pair < npairs && d.rt < nrt;
+  d.valid = d.type < ntypes && d.rt < nrt;
   return d;
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1)
 density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmPhiN,
-                   const double* __restrict__ phi, double* __restrict__ rho_part, int N, long long Ng, int ntile,
-                   int npairs, long long nrt, int group_r, long long nwork, int b3d) {
+                   const double* __restrict__ phi, const DensSeg* __restrict__ segs, double* __restrict__ rho_part,
+                   int N, long long Ng, int ntypes, long long nrt, int group_r, long long nwork, int b3d) {
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -169,27 +172,25 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
   init_bars(bars);
 
   if (warp >= NCONS) {
-    // ===== producer: runs ahead across j-tiles and work items =====
+    // ===== producer: runs ahead across segments and work items =====
     regs_producer();
     if (warp == NCONS && lane == 0) {
       tma_prefetch_desc(&tmP);
       tma_prefetch_desc(&tmPhiN);
       long long it = 0;
       for (long long L = blockIdx.x; L < nwork; L += gridDim.x) {
-        const DensWork wk = dens_decode(L, npairs, nrt, group_r);
+        const DensWork wk = dens_decode(L, ntypes, nrt, group_r);
         if (!wk.valid) continue;
         const long long r0 = wk.rt * TILE;
         for (int which = 0; which < 2; ++which) {
-          const int jt = which == 0 ? wk.pair : ntile - 1 - wk.pair;
-          if (which == 1 && jt <= wk.pair) break;
-          const int j0 = jt * TILE;
-          const int nk = (N - j0 + BK - 1) / BK;
-          for (int kt = 0; kt < nk; ++kt, ++it) {
+          const DensSeg sg = segs[2 * wk.type + which];
+          const int j0 = sg.jt * TILE;
+          for (int i = 0; i < sg.ns; ++i, ++it) {
             const int slot = (int)(it % ST);
             if (it >= ST) mbar_wait(smem_u32(&bars->empty[slot]), (uint32_t)((it / ST) - 1) & 1);
             const uint32_t full = smem_u32(&bars->full[slot]);
             mbar_expect_tx(full, 2 * TILE_BYTES);
-            const int k0 = j0 + kt * BK;
+            const int k0 = j0 + (sg.s0 + sg.dir * i) * BK;
             double* sA = tilesm + (size_t)slot * STAGE_D;
             tma_load_2d(sA, &tmP, k0, j0, full);                              // Pfold[j0.., k0..]
             if (b3d) {                                                        // Phi[k0.., r0 .. r0+127] in one op
@@ -215,7 +216,7 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
   const bool vecF = ((Ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(phi) & 15) == 0);
   long long it = 0;
   for (long long L = blockIdx.x; L < nwork; L += gridDim.x) {
-    const DensWork wk = dens_decode(L, npairs, nrt, group_r);
+    const DensWork wk = dens_decode(L, ntypes, nrt, group_r);
     if (!wk.valid) continue;
     const long long r0 = wk.rt * TILE;
     double colsum[FB / 2][4];
@@ -224,18 +225,17 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
 #pragma unroll
       for (int q = 0; q < 4; ++q) colsum[t][q] = 0.0;
 
-    for (int which = 0; which < 2; ++which) {
-      const int jt = which == 0 ? wk.pair : ntile - 1 - wk.pair;
-      if (which == 1 && jt <= wk.pair) break;
-      const int j0 = jt * TILE;
-      const int nk = (N - j0 + BK - 1) / BK;
+    for (int which = 0; which < 2; ++which) {               // same segment order as the producer
+      const DensSeg sg = segs[2 * wk.type + which];
+      if (sg.ns == 0) continue;
+      const int j0 = sg.jt * TILE;
       double acc[FA][FB][2];
 #pragma unroll
       for (int a = 0; a < FA; ++a)
 #pragma unroll
         for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
 
-      for (int kt = 0; kt < nk; ++kt, ++it) {
+      for (int i = 0; i < sg.ns; ++i, ++it) {
         const int slot = (int)(it % ST);
         mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
         const double* sA = tilesm + (size_t)slot * STAGE_D;
@@ -295,7 +295,7 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
         double v = 0.0;
 #pragma unroll
         for (int m = 0; m < WM; ++m) v += colred[m * TILE + ctid];
-        rho_part[(long long)wk.pair * Ng + r] = v;
+        rho_part[(long long)wk.type * Ng + r] = v;
       }
     }
     consumer_sync(32 * NCONS);
@@ -303,12 +303,12 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
 }
 
 void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, int b3d,
-                        const double* phi, double* rho_part, int sms, cudaStream_t st) {
+                        const double* phi, const DensSeg* segs, double* rho_part, int sms, cudaStream_t st) {
   const long long ngroups = (p.nrt + p.group_r - 1) / p.group_r;
-  const long long nwork = ngroups * p.group_r * p.npairs;
+  const long long nwork = ngroups * p.group_r * p.ntypes;
   const long long grid = nwork < sms ? nwork : sms;
-  density_tma_kernel<<<(unsigned)grid, NTHREADS, SMEM_TOTAL, st>>>(tmP, tmPhiN, phi, rho_part, p.N, p.Ng, p.ntile,
-                                                                   p.npairs, p.nrt, p.group_r, nwork, b3d);
+  density_tma_kernel<<<(unsigned)grid, NTHREADS, SMEM_TOTAL, st>>>(tmP, tmPhiN, phi, segs, rho_part, p.N, p.Ng,
+                                                                   p.ntypes, p.nrt, p.group_r, nwork, b3d);
 }
 
 // ======================================================================================================
@@ -316,6 +316,8 @@ void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUte
 // ======================================================================================================
 struct GemmTmaArgs {
   int N, ldn, nterms;
+  int sym;                 // +1: D is symmetric, -1: antisymmetric -> only tiles ti <= tj are computed and mirrored
+  const int2* tiles;       // upper-triangular tile list (sym != 0)
   double alpha0, alpha1;
   double* D; double* Z1; double beta1; double* Z2; double beta2;
 };
@@ -331,7 +333,9 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   init_bars(bars);
   const int N = ga.N, ldn = ga.ldn;
-  const int i0 = blockIdx.y * TILE, j0 = blockIdx.x * TILE;
+  int i0, j0;
+  if (ga.sym) { const int2 tt = ga.tiles[blockIdx.x]; i0 = tt.x * TILE; j0 = tt.y * TILE; }
+  else { i0 = blockIdx.y * TILE; j0 = blockIdx.x * TILE; }
   const int nk1 = (N + BK - 1) / BK;
   const int nk = ga.nterms * nk1;
 
@@ -381,6 +385,8 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
     if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
   }
   const double fin = (ga.nterms == 2 && ratio != 1.0) ? ga.alpha0 * ratio : ga.alpha0;
+  const bool diag = ga.sym && i0 == j0;
+  const double msign = (double)ga.sym;
 
 #pragma unroll
   for (int a = 0; a < FA; ++a) {
@@ -391,12 +397,20 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
           const int col = j0 + wcol + 8 * b + c + 4 * e;
-          if (col < N) {
+          if (col < N && (!diag || col >= row)) {
             const long long o = (long long)row * ldn + col;
-            const double d = fin * acc[a][b][e];
+            double d = fin * acc[a][b][e];
+            if (ga.sym < 0 && row == col) d = 0.0;
             if (ga.D) ga.D[o] = d;
             if (ga.Z1) ga.Z1[o] += ga.beta1 * d;
             if (ga.Z2) ga.Z2[o] += ga.beta2 * d;
+            if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
+              const long long om = (long long)col * ldn + row;
+              const double dm = msign * d;
+              if (ga.D) ga.D[om] = dm;
+              if (ga.Z1) ga.Z1[om] += ga.beta1 * dm;
+              if (ga.Z2) ga.Z2[om] += ga.beta2 * dm;
+            }
           }
         }
       }
@@ -405,10 +419,11 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
 }
 
 void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
-                         const CUtensorMap& tmB1, cudaStream_t st) {
-  GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2};
+                         const CUtensorMap& tmB1, int sym, const int2* tiles, cudaStream_t st) {
+  GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, sym, tiles, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2};
   const int nt = (g.N + TILE - 1) / TILE;
-  gemm_abt_tma_kernel<<<dim3(nt, nt), NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
+  if (sym) gemm_abt_tma_kernel<<<nt * (nt + 1) / 2, NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
+  else gemm_abt_tma_kernel<<<dim3(nt, nt), NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
 }
 
 int init_tma_kernels() {

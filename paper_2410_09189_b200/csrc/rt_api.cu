@@ -47,6 +47,8 @@ struct rt_ctx {
          *Cm = nullptr, *Sc = nullptr, *Sm = nullptr, *P0r = nullptr, *P0i = nullptr, *P1r = nullptr, *P1i = nullptr,
          *W = nullptr;
   int2* d_tiles = nullptr;
+  DensSeg* d_segs = nullptr;
+  std::vector<DensSeg> segs;
   ProjectPlan pp{};
   DensityPlan dp{};
   // grid arrays
@@ -139,6 +141,35 @@ bool can_coarsen(const GridDims& g) {
   return g.nx % 2 == 0 && g.ny % 2 == 0 && g.nz % 2 == 0 && g.nx > 4 && g.ny > 4 && g.nz > 4;
 }
 
+// ---- a5 work types ---------------------------------------------------------------------------------
+// The triangular fold leaves j-tile jt with the contraction rows k >= jt*TILE, i.e. nk(jt) stages of 16.  Pair
+// (p, ntile-1-p) therefore always costs about (ntile + 1) tiles.  The time line of a pair is: short tile
+// ntile-1-p with k ascending to N, then long tile p with k descending from N (rows around the turn-around are
+// re-read while they are still in L2).  The time line is cut into `nsplit` pieces of equal length; each piece is a
+// work type (<= 2 segments) with its own partial-sum row.  nsplit > 1 puts more CTAs on the same r-tile, so fewer
+// r-tile panels of Phi are in flight: used when the folded P (4 N^2 bytes) is small enough to stay in L2 next to them.
+void build_density_types(int N, int ntile, int nsplit, std::vector<DensSeg>& out) {
+  out.clear();
+  const int npairs = (ntile + 1) / 2;
+  auto nk = [&](int jt) { return (N - jt * TILE + BK_HOST - 1) / BK_HOST; };
+  for (int p = 0; p < npairs; ++p) {
+    const int jb = ntile - 1 - p;
+    const int nkB = jb > p ? nk(jb) : 0, nkA = nk(p);
+    const int tot = nkB + nkA;
+    for (int i = 0; i < nsplit; ++i) {
+      const int t0 = (int)((long long)tot * i / nsplit), t1 = (int)((long long)tot * (i + 1) / nsplit);
+      DensSeg b{jb > p ? jb : p, 0, 0, 1}, a{p, 0, 0, -1};
+      if (t0 < nkB) { b.s0 = t0; b.ns = (t1 < nkB ? t1 : nkB) - t0; }
+      if (t1 > nkB) {
+        const int u0 = (t0 > nkB ? t0 : nkB) - nkB, u1 = t1 - nkB;
+        a.s0 = nkA - 1 - u0; a.ns = u1 - u0;
+      }
+      out.push_back(b);
+      out.push_back(a);
+    }
+  }
+}
+
 // ---- TMA descriptors -------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -208,13 +239,15 @@ void stage_end(rt_ctx* c) {
 }
 
 // ---- the stages ------------------------------------------------------------------------------------
-void enqueue_gemm(rt_ctx* c, const double* A0, const double* B0, double a0, const double* A1, const double* B1,
-                  double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr, double b2 = 0) {
+void enqueue_gemm(rt_ctx* c, int sym, const double* A0, const double* B0, double a0, const double* A1,
+                  const double* B1, double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr,
+                  double b2 = 0) {
   GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2};
   if (c->use_tma) {
     const CUtensorMap& mA0 = nn_map(c, A0);
     const CUtensorMap& mB0 = nn_map(c, B0);
-    launch_gemm_abt_tma(g, mA0, mB0, A1 ? nn_map(c, A1) : mA0, B1 ? nn_map(c, B1) : mB0, c->st);
+    launch_gemm_abt_tma(g, mA0, mB0, A1 ? nn_map(c, A1) : mA0, B1 ? nn_map(c, B1) : mB0, sym, c->d_tiles,
+                        c->st);
   } else {
     launch_gemm_abt(g, c->st);
   }
@@ -224,7 +257,7 @@ void enqueue_gemm(rt_ctx* c, const double* A0, const double* B0, double a0, cons
 // C = cos X, S = sin X for the real symmetric X (H-bar real at Gamma) -> U = C - i S.
 // cos X = sum_k (-1)^k Y^k/(2k)!, sin X = X sum_k (-1)^k Y^k/(2k+1)!, Y = X^2, k <= q.   q + 1 GEMMs.
 void enqueue_expm(rt_ctx* c) {
-  enqueue_gemm(c, c->X, c->X, 1.0, nullptr, nullptr, 0, c->Ya);
+  enqueue_gemm(c, 1, c->X, c->X, 1.0, nullptr, nullptr, 0, c->Ya);
   launch_series_init(c->N, c->ldn, c->Ya, c->Cm, -0.5, c->Sc, -1.0 / 6.0, c->st);
   c->launches += 1;
   double ck = -0.5, sk = -1.0 / 6.0;
@@ -233,27 +266,28 @@ void enqueue_expm(rt_ctx* c) {
     ck = -ck / ((2.0 * k - 1.0) * (2.0 * k));
     sk = -sk / ((2.0 * k) * (2.0 * k + 1.0));
     double* cur = (k < c->q) ? ((k & 1) ? c->Yc : c->Yb) : nullptr;
-    enqueue_gemm(c, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk);
+    enqueue_gemm(c, 1, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk);
     prev = cur;
   }
-  enqueue_gemm(c, c->X, c->Sc, 1.0, nullptr, nullptr, 0, c->Sm);
+  enqueue_gemm(c, 1, c->X, c->Sc, 1.0, nullptr, nullptr, 0, c->Sm);
 }
 
 // P1 = U P0 U^dagger (Eq. 15), U = C - iS, P0 = A + iB (A symmetric, B antisymmetric).
 //   Yr = C A + S B, Yi = C B - S A ; P1r = Yr C - Yi S, P1i = Yr S + Yi C.
 // gemm_abt contracts against B^T: a symmetric right factor is used as is, the antisymmetric one flips the sign.
 void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
-  enqueue_gemm(c, c->Cm, Ar, 1.0, c->Sm, Ai, -1.0, c->Yb);
-  enqueue_gemm(c, c->Cm, Ai, -1.0, c->Sm, Ar, -1.0, c->Yc);
-  enqueue_gemm(c, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, Or);
-  enqueue_gemm(c, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, Oi);
+  enqueue_gemm(c, 0, c->Cm, Ar, 1.0, c->Sm, Ai, -1.0, c->Yb);
+  enqueue_gemm(c, 0, c->Cm, Ai, -1.0, c->Sm, Ar, -1.0, c->Yc);
+  enqueue_gemm(c, 1, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, Or);      // P1 Hermitian: Re symmetric,
+  enqueue_gemm(c, -1, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, Oi);      // Im antisymmetric
 }
 
 void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double* rho0) {
   launch_fold_upper(c->N, c->ldn, reP, c->X, c->st);
-  if (c->use_tma) launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phiN_3d, c->phi, c->rho_part, c->sms, c->st);
+  if (c->use_tma)
+    launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phiN_3d, c->phi, c->d_segs, c->rho_part, c->sms, c->st);
   else launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
-  launch_reduce_rho(c->rho_part, c->dp.npairs, c->Ng, c->gd, c->h, rho0, rho_out, c->d_bsums, c->d_sums, c->st);
+  launch_reduce_rho(c->rho_part, c->use_tma ? c->dp.ntypes : c->dp.npairs, c->Ng, c->gd, c->h, rho0, rho_out, c->d_bsums, c->d_sums, c->st);
   c->launches += 4;
 }
 
@@ -494,7 +528,13 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     p.S = (int)((Ng + kc - 1) / kc);
     DensityPlan& d = c->dp;
     d.N = N; d.Ng = Ng; d.ntile = ntile; d.npairs = (ntile + 1) / 2; d.nrt = (Ng + TILE - 1) / TILE; d.ldn = ldn;
-    int gr = d.npairs >= 12 ? 12 : (sms + d.npairs - 1) / d.npairs;
+    // work types of the TMA kernel: one per pair.  (Cutting the pairs' time lines into several types per r-tile, so
+    // that fewer Phi panels are in flight, was measured on nano: 4 pieces -> 397 ms and 277 GB of DRAM reads against
+    // 364 ms and 191 GB for whole pairs; the extra epilogues and pipeline refills cost more than the locality buys.)
+    const int nsplit = 1;
+    build_density_types(N, ntile, nsplit, c->segs);
+    d.ntypes = (int)(c->segs.size() / 2);
+    int gr = (sms + d.ntypes - 1) / d.ntypes;
     if (gr > d.nrt) gr = (int)d.nrt;
     d.group_r = gr < 1 ? 1 : gr;
   }
@@ -503,7 +543,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   {
     size_t freeb = 0, totalb = 0;
     CKC(cudaMemGetInfo(&freeb, &totalb));
-    double need = 15.0 * N * (double)ldn * 8 + (double)c->pp.S * N * ldn * 8 + (double)c->dp.npairs * Ng * 8 + 12.0 * Ng * 8;
+    double need = 15.0 * N * (double)ldn * 8 + (double)c->pp.S * N * ldn * 8 + (double)c->dp.ntypes * Ng * 8 + 12.0 * Ng * 8;
     if (!(cfg->flags & RT_PHI_DEVICE)) need += (double)N * Ng * 8;
     if (need > (double)freeb) {
       char buf[256];
@@ -546,7 +586,9 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   ALLOC(c->w, Ng + 16); ALLOC(c->op_u, Ng + 16);      // projection weights: the TMA path reads whole 16-double stages
   CKC(cudaMemsetAsync(c->w, 0, (size_t)(Ng + 16) * 8, c->st));
   CKC(cudaMemsetAsync(c->op_u, 0, (size_t)(Ng + 16) * 8, c->st));
-  ALLOC(c->rho_part, (size_t)c->dp.npairs * Ng);
+  ALLOC(c->rho_part, (size_t)c->dp.ntypes * Ng);
+  ALLOC(c->d_segs, c->segs.size());
+  CKC(cudaMemcpyAsync(c->d_segs, c->segs.data(), c->segs.size() * sizeof(DensSeg), cudaMemcpyHostToDevice, c->st));
   for (size_t l = 0; l < c->lv.size(); ++l) {
     MgLevel& L = c->lv[l];
     ALLOC(L.u, L.n); ALLOC(L.tmp, L.n); ALLOC(L.f, L.n); ALLOC(L.r, L.n);

@@ -37,7 +37,11 @@ struct DensityPlan {
   long long nrt;         // r tiles = ceil(Ng / TILE)
   int ldn;
   int group_r;           // raster: r-tiles per supertile column
+  int ntypes;            // TMA kernel: work types per r-tile (each owns one partial row); >= npairs
 };
+// TMA density kernel: one k-segment of j-tile jt: stages s0, s0 + dir, ... (ns of them), stage s covering the
+// contraction rows jt*TILE + 16 s ... + 15.  A work type is two consecutive DensSeg (the second may have ns = 0).
+struct DensSeg { int jt, s0, ns, dir; };
 void launch_density(const DensityPlan& p, const double* phi, const double* Pfold, double* rho_part, cudaStream_t st);
 size_t density_smem_bytes();
 // Pfold[j][i] = 2 P[j][i] (i > j), P[j][j] (i == j), 0 (i < j)
@@ -64,9 +68,11 @@ void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const do
 // tmP: Pfold [N][N] (ld = ldn) box {16, 128}; tmPhiN: Phi with box {16 r, 16 k-rows} (b3d = 0: 8 loads per stage)
 // or, when Ng % 16 == 0, the 3-D view {16 r-low, N k, Ng/16 r-high} with box {16, 16, 8} (b3d = 1: one load)
 void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, int b3d,
-                        const double* phi, double* rho_part, int sms, cudaStream_t st);
+                        const double* phi, const DensSeg* segs, double* rho_part, int sms, cudaStream_t st);
+// sym = +1 / -1: the product is known to be symmetric / antisymmetric (polynomials of the symmetric X commute; P1 is
+// Hermitian): only the upper tiles (list `tiles`, ti <= tj) are computed and the mirror image is written too
 void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
-                         const CUtensorMap& tmB1, cudaStream_t st);
+                         const CUtensorMap& tmB1, int sym, const int2* tiles, cudaStream_t st);
 
 // ---- elementwise N x N (a2 and series glue) -------------------------------------------------------------
 // first != 0: H1 = 2 H0 - Hm1 first.  X = dt * ((H0 + H1)/2 - sigma I)
