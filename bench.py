@@ -218,9 +218,8 @@ def main():
 
     import torch
     import torch.distributed as dist
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2410_09189_b200 import replicas
+    rank, world, local = replicas.rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the RT-TDDFT path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -235,8 +234,7 @@ def main():
     from paper_2410_09189_b200 import binding as B
 
     # inputs: every rank propagates its own seeded system (replicas; seed offset by rank)
-    import dataclasses
-    wr = dataclasses.replace(w, seed=w.seed + 100 * rank)
+    wr = replicas.replica_workload(w, rank)
     big = w.norb * w.ngrid * 8 > 2e9
     t_gen = time.perf_counter()
     if big:
@@ -321,10 +319,7 @@ def main():
         e2e_sec = time.perf_counter() - t0
         charge = B.rt_get_charge(sim.handle)
 
-    tmax = torch.tensor([ms_total, e2e_sec * 1e3], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total, e2e_ms = float(tmax[0]), float(tmax[1])
+    ms_total, e2e_ms = replicas.max_over_ranks([ms_total, e2e_sec * 1e3], device=f"cuda:{local}")
     if rank != 0:
         sim.close()
         if world > 1:
@@ -332,8 +327,8 @@ def main():
         return 0
 
     ms_per_step = ms_total / args.steps
-    value = world * args.steps / (ms_total * 1e-3)
-    e2e_value = world * args.steps / (e2e_ms * 1e-3)
+    value = replicas.whole_job_steps_per_s(args.steps, world, ms_total)
+    e2e_value = replicas.whole_job_steps_per_s(args.steps, world, e2e_ms)
 
     # roofline of the dominant kernel (the stage with the largest share)
     N, Ng = w.norb, w.ngrid

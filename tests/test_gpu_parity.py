@@ -187,6 +187,34 @@ def test_step_parity_strong_kick(B, name, nsteps):
     gpu.close()
 
 
+def test_step_parity_scaled_twins(B):
+    """Scaled-down twins of the two configs too large for a full oracle run: identical structure
+    (random orthonormal orbitals, eps range, occupation ratio, dt, V-cycles, kick), end to end against the oracle.
+    nano_twin: 64^3 x 300 orbitals (3 j-tiles, ragged); 24k_twin: 52^3 x 1,625 orbitals (13 j-tiles, 52 -> 26 -> 13)."""
+    w, Phi, eps, occ = inputs("nano_twin")
+    gpu, cpu = make_pair(B, w, Phi, eps, occ)
+    check_run(B, gpu, cpu, w, 6)
+    gpu.close()
+    _cache.pop("nano_twin")
+    w, Phi, eps, occ = inputs("24k_twin")
+    ws = strong_kick(w, 0.05)
+    gpu, cpu = make_pair(B, ws, Phi, eps, occ)
+    assert gpu.info()["mg_levels"] == 3 and gpu.info()["coarsest"] == (13, 13, 13)
+    check_run(B, gpu, cpu, ws, 2)
+    gpu.close()
+    _cache.pop("24k_twin")
+
+
+def test_step_parity_mid_laser(B):
+    """`mid` config as BASELINE.json states it: 96^3 grid, 512 Gaussian-sum orbitals, Gaussian-envelope laser along z
+    driven through rt_set_field every step (first 3 of its 500 steps; the oracle needs ~10 s per step)."""
+    w, Phi, eps, occ = inputs("mid")
+    gpu, cpu = make_pair(B, w, Phi, eps, occ)
+    check_run(B, gpu, cpu, w, 3, laser=True)
+    gpu.close()
+    _cache.pop("mid")
+
+
 def test_step_parity_laser_set_field(B):
     """rt_set_field path: Gaussian-envelope laser along z (the `mid` config's driver) on the tiny system."""
     w, Phi, eps, occ = inputs("tiny")
