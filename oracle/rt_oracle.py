@@ -273,7 +273,17 @@ class RTOracle:
     """
 
     def __init__(self, shape, h, Phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2,
-                 nu_pre=2, nu_post=2, omega=6.0 / 7.0, hartree=True, xc=True):
+                 nu_pre=2, nu_post=2, omega=6.0 / 7.0, hartree=True, xc=True,
+                 propagator="eigh", dP_thrs=1e-10, max_order=200, H_thrs=0.0, max_hupdates=20):
+        """propagator = "eigh": exact spectral exponential (north_star).  propagator = "commutator": the
+        paper's own series applied to P (Eq. 39, Alg. 1 lines 15-23) until max|dP^(k)| <= dP_thrs
+        (Alg. 1 line 5: 1e-10).  H_thrs > 0 turns the fixed count of Hamiltonian updates into the paper's
+        dynamic loop (Alg. 1 lines 12-13, 24-26; L483): repeat while max|H1 - H1_old| > H_thrs, at most
+        max_hupdates times.  ``last_hupdates``, ``last_H_err``, ``last_orders`` report what the last step did."""
+        assert propagator in ("eigh", "commutator")
+        self.propagator, self.dP_thrs, self.max_order = propagator, float(dP_thrs), int(max_order)
+        self.H_thrs, self.max_hupdates = float(H_thrs), int(max_hupdates)
+        self.last_hupdates, self.last_H_err, self.last_H_errs, self.last_orders = 0, 0.0, [], []
         self.shape = tuple(int(n) for n in shape)
         self.h = float(h)
         self.dVol = self.h ** 3
@@ -310,14 +320,29 @@ class RTOracle:
             dv = dv + vxc_lda(rho) - self.vxc0
         return dv
 
+    def _propagate(self, Hbar):
+        if self.propagator == "eigh":
+            return propagate_eigh(Hbar, self.P0, self.dt)                  # Eq. 15
+        P1, k = propagate_commutator(Hbar, self.P0, self.dt, self.dP_thrs, self.max_order)   # lines 15-23
+        self.last_orders.append(k)
+        return P1
+
     def step(self, nsteps: int = 1):
         for _ in range(nsteps):
             H1 = 2.0 * self.H0 - self.Hm1                                  # Alg. 1 line 11
-            for _it in range(self.m):                                      # lines 13-26, fixed m
+            self.last_orders, self.last_H_errs = [], []
+            it = 0
+            H_err = 2.0 * self.H_thrs                                      # line 12
+            while (it < self.m) if self.H_thrs <= 0.0 else (H_err > self.H_thrs and it < self.max_hupdates):
                 Hbar = 0.5 * (self.H0 + H1)                                # line 14 / Eq. 12
-                P1 = propagate_eigh(Hbar, self.P0, self.dt)                # Eq. 15
+                P1 = self._propagate(Hbar)
                 rho = density(self.Phi, P1.real)                           # Eq. 27
+                H1_old = H1
                 H1 = np.diag(self.eps) + project(self.Phi, self.delta_v(rho), self.dVol)   # line 25
+                H_err = float(np.max(np.abs(H1 - H1_old)))                 # line 24 (after the update, DESIGN R2)
+                self.last_H_errs.append(H_err)
+                it += 1
+            self.last_hupdates, self.last_H_err = it, H_err
             self.rho = rho
             self.Hm1, self.H0, self.P0 = self.H0, H1, P1                   # line 28
             self.t += self.dt

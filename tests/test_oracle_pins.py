@@ -372,3 +372,56 @@ def test_convergence_in_m(tiny_inputs):
     ref = np.max(np.abs(m4))
     assert np.max(np.abs(m2 - m4)) / ref < 1e-3
     assert np.max(np.abs(m2 - m4)) < 0.2 * np.max(np.abs(m1 - m4))
+
+
+# ------------------------------------------------------------------ the paper's own loops (Alg. 1 lines 12-26)
+
+def test_commutator_mode_tracks_exact_propagator(tiny_inputs):
+    """Whole trajectory with the series of Eq. 39 (dP_thrs = 1e-10, Alg. 1 line 5) against the exact spectral
+    propagator: PAPER.md:L426 "arbitrarily close ... subject to the convergence threshold dP_thrs"; and the
+    invariants the series keeps exactly: tr[H,X] = 0 => tr P = N_e, Hermiticity."""
+    a = _make(tiny_inputs, E0=(0.05, 0, 0))
+    b = _make(tiny_inputs, E0=(0.05, 0, 0), propagator="commutator", dP_thrs=1e-10)
+    ne = a.occ.sum()
+    for _ in range(6):
+        a.step(1)
+        b.step(1)
+        assert len(b.last_orders) == 2 and all(3 < k < 40 for k in b.last_orders)
+        assert abs(np.trace(b.P0).real - ne) < 1e-12
+        assert np.max(np.abs(b.P0 - b.P0.conj().T)) < 1e-14
+    # every neglected tail is < dP_thrs per propagation; 12 propagations
+    assert np.max(np.abs(a.P0 - b.P0)) < 12 * 1e-10
+    assert np.max(np.abs(a.dipole() - b.dipole())) < 1e-8
+    tight = _make(tiny_inputs, E0=(0.05, 0, 0), propagator="commutator", dP_thrs=1e-16)
+    tight.step(6)
+    assert np.max(np.abs(a.P0 - tight.P0)) < 2e-13
+
+
+def test_dynamic_hamiltonian_loop(tiny_inputs):
+    """Alg. 1 lines 12-13/24-26 with H_thrs (L351, L483).  (i) the loop stops at the first update whose
+    max|H1 - H1_old| <= H_thrs and never before; (ii) its result agrees with a long fixed-count run to the order of
+    H_thrs; (iii) a larger time step needs at least as many updates, and the later phase needs no more than the
+    initial one (L485: 3, 4, 5, 9 updates for dt = 0.2 ... 2 a.u.t. initially, 1, 2, 3, 6 later)."""
+    thr = 1e-7
+    first, later = [], []
+    for dt in (0.1, 1.0, 4.0):
+        d = _make(tiny_inputs, E0=(0.05, 0, 0), dt=dt, H_thrs=thr, max_hupdates=30)
+        d.step(1)
+        n1 = d.last_hupdates
+        assert 1 <= n1 < 30 and d.last_H_err <= thr
+        assert all(x > thr for x in d.last_H_errs[:-1]) and len(d.last_H_errs) == n1
+        e = _make(tiny_inputs, E0=(0.05, 0, 0), dt=dt, n_hupdates=n1)          # same step, fixed count
+        e.step(1)
+        assert np.array_equal(e.P0, d.P0)
+        f = _make(tiny_inputs, E0=(0.05, 0, 0), dt=dt, n_hupdates=n1 - 1)      # reported error = last change of H1
+        f.step(1)
+        assert abs(np.max(np.abs(e.H0 - f.H0)) - d.last_H_err) < 1e-15
+        ref = _make(tiny_inputs, E0=(0.05, 0, 0), dt=dt, n_hupdates=n1 + 6)
+        ref.step(1)
+        assert np.max(np.abs(ref.P0 - d.P0)) < 50 * thr
+        d.step(3)
+        first.append(n1)
+        later.append(d.last_hupdates)
+    assert first == sorted(first) and first[-1] > first[0]
+    assert later == sorted(later) and later[-1] > later[0]
+    assert all(b <= a for a, b in zip(first, later))
