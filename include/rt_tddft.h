@@ -52,6 +52,12 @@ extern "C" {
 #define RT_NO_TMA     16u   /* use the cp.async versions of the DMMA kernels even where TMA applies (the
                                library falls back to them by itself when Ng is odd or phi is not 16-byte aligned) */
 
+/* rt_config.propagator */
+#define RT_PROP_TAYLOR      0   /* U = exp(-i Hbar dt) by a fixed-degree Taylor polynomial, then P1 = U P0 U^dagger      */
+#define RT_PROP_COMMUTATOR  1   /* the paper's own series applied to P: dP^(k) = (-i dt/k)[Hbar, dP^(k-1)],
+                                   P1 = P0 + sum_k dP^(k) until max|dP^(k)| <= dP_thrs (Eq. 39, Alg. 1 lines
+                                   15-23 L375-L392; real/imaginary split of Eq. 40)                          */
+
 typedef struct rt_ctx* rt_handle;
 
 typedef struct {
@@ -69,6 +75,14 @@ typedef struct {
   uint32_t flags;           /* RT_* flags above                                                              */
   int32_t  device;          /* CUDA device ordinal                                                           */
   void*    stream;          /* cudaStream_t all work is enqueued on (e.g. torch.cuda.current_stream()); NULL = legacy default */
+  /* -- the paper's dynamic loops (Alg. 1 line 5, L351); all zero = the fixed-count step described above -- */
+  int32_t  propagator;      /* RT_PROP_TAYLOR (0) or RT_PROP_COMMUTATOR                                       */
+  int32_t  max_order;       /* commutator series: largest order k; 0 -> from the spectral bound (<= 96)       */
+  double   dP_thrs;         /* commutator series: stop when max|dP^(k)| <= dP_thrs; 0 -> 1e-10                */
+  double   H_thrs;          /* > 0: repeat the Hamiltonian update while max|H1 - H1_old| > H_thrs (Alg. 1 lines
+                               12-13, 24-26; L483) instead of n_hupdates times.  rt_step then synchronises the
+                               host once per update (it reads the 8-byte error norm)                           */
+  int32_t  max_hupdates;    /* bound on the updates per step when H_thrs > 0; 0 -> 20                          */
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
@@ -107,6 +121,10 @@ int rt_get_info(rt_handle h, int32_t info[8]);
 /* Total number of this library's kernel launches enqueued through the handle so far (graph replays count the
  * kernels inside the graph).  HOST. */
 int rt_get_launch_count(rt_handle h, int64_t* n);
+/* What the loops of Alg. 1 did in the most recent step.  HOST: n[0] = Hamiltonian updates (n_hupdates unless
+ * H_thrs > 0), n[1] = orders summed by the commutator series in the last update (0 with RT_PROP_TAYLOR);
+ * err[0] = last max|H1 - H1_old| (0 unless H_thrs > 0), err[1] = last max|dP^(k)|.  Synchronises. */
+int rt_get_convergence(rt_handle h, int32_t n[2], double err[2]);
 /* Text of the last error on this handle (or of the last failed rt_create when h == NULL).  Never NULL. */
 const char* rt_last_error(rt_handle h);
 /* Frees every workspace (not a borrowed phi).  NULL is accepted. */

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "librt_tddft.so")
 
 RT_OK, RT_EINVAL, RT_ENOMEM, RT_ECUDA, RT_ESTATE = 0, -1, -2, -3, -4
 RT_PHI_DEVICE, RT_NO_HARTREE, RT_NO_XC, RT_NO_GRAPH, RT_NO_TMA = 1, 2, 4, 8, 16
+RT_PROP_TAYLOR, RT_PROP_COMMUTATOR = 0, 1
 RT_STAGE_NAMES = ("Hupdate", "Rho", "Vh", "ELDYN", "XC")      # Table 1 of the paper, L543-L547
 RT_STAGE_COUNT = 5
 
@@ -25,7 +26,7 @@ SYMBOLS = (
     "rt_create", "rt_set_field", "rt_step", "rt_get_dipole", "rt_get_density", "rt_get_pmatrix", "rt_get_hmatrix",
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
-    "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak",
+    "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
 )
 
 
@@ -43,6 +44,9 @@ class rt_config(C.Structure):
         ("flags", C.c_uint32),
         ("device", C.c_int32),
         ("stream", C.c_void_p),
+        ("propagator", C.c_int32), ("max_order", C.c_int32),
+        ("dP_thrs", C.c_double), ("H_thrs", C.c_double),
+        ("max_hupdates", C.c_int32),
     ]
 
 
@@ -66,7 +70,7 @@ def _load():
         "rt_get_time": [vp, dp], "rt_get_charge": [vp, dp], "rt_get_info": [vp, dp], "rt_get_launch_count": [vp, i64p],
         "rt_destroy": [vp], "rt_op_project": [vp, dp, dp], "rt_op_density": [vp, dp, dp, dp],
         "rt_op_propagate": [vp, dp, dp, dp, dp, dp], "rt_op_hartree": [vp, dp, dp, i32], "rt_op_vxc": [vp, dp, dp],
-        "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp],
+        "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp], "rt_get_convergence": [vp, dp, dp],
     }
     for name, argtypes in sig.items():
         fn = getattr(lib, name)
@@ -169,6 +173,13 @@ def rt_get_info(h) -> dict:
             "project_split_k": int(a[7])}
 
 
+def rt_get_convergence(h) -> dict:
+    n = np.zeros(2, dtype=np.int32)
+    err = np.zeros(2)
+    _check(h, _lib.rt_get_convergence(h, n.ctypes.data, _ptr(err)))
+    return {"hupdates": int(n[0]), "orders": int(n[1]), "H_err": float(err[0]), "dP_err": float(err[1])}
+
+
 def rt_get_launch_count(h) -> int:
     n = C.c_int64(0)
     _check(h, _lib.rt_get_launch_count(h, C.byref(n)))
@@ -233,8 +244,10 @@ class RTTDDFT:
 
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
                  nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
-                 device=0, stream=None):
+                 device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0):
         cfg = rt_config()
+        cfg.propagator = {"taylor": RT_PROP_TAYLOR, "commutator": RT_PROP_COMMUTATOR}[propagator]
+        cfg.max_order, cfg.dP_thrs, cfg.H_thrs, cfg.max_hupdates = int(max_order), float(dP_thrs), float(H_thrs), int(max_hupdates)
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)
         cfg.h, cfg.norb, cfg.dt = float(h), int(len(eps)), float(dt)
         cfg.n_hupdates, cfg.n_vcycles = int(n_hupdates), int(n_vcycles)
@@ -301,6 +314,9 @@ class RTTDDFT:
 
     def info(self):
         return rt_get_info(self.handle)
+
+    def convergence(self):
+        return rt_get_convergence(self.handle)
 
     def close(self):
         if getattr(self, "handle", None):

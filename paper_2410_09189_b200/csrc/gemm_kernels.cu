@@ -298,6 +298,7 @@ constexpr int GEMM_STAGE = BM * BK + BN * BK;
 
 __global__ void __launch_bounds__(NT, 1)
 gemm_abt_kernel(GemmArgs ga) {
+  if (ga.skip && *ga.skip) return;
   extern __shared__ __align__(16) double smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g = lane >> 2, c = lane & 3;

@@ -320,12 +320,14 @@ struct GemmTmaArgs {
   const int2* tiles;       // upper-triangular tile list (sym != 0)
   double alpha0, alpha1;
   double* D; double* Z1; double beta1; double* Z2; double beta2;
+  const int* skip;         // non-zero -> no-op (orders past convergence of the commutator series)
 };
 
 __global__ void __launch_bounds__(NTHREADS, 1)
 gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmB0,
                     const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmB1,
                     GemmTmaArgs ga) {
+  if (ga.skip && *ga.skip) return;
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -420,7 +422,7 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
 
 void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
                          const CUtensorMap& tmB1, int sym, const int2* tiles, cudaStream_t st) {
-  GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, sym, tiles, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2};
+  GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, sym, tiles, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2, g.skip};
   const int nt = (g.N + TILE - 1) / TILE;
   if (sym) gemm_abt_tma_kernel<<<nt * (nt + 1) / 2, NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
   else gemm_abt_tma_kernel<<<dim3(nt, nt), NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);

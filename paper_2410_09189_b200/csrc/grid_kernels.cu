@@ -401,6 +401,65 @@ void launch_copy5(int N, int ldn, double* d0, const double* s0, double* d1, cons
   copy4_kernel<<<(unsigned)nb, 256, 0, st>>>(n, d0, s0, d1, s1, d2, s2, d3, s3);
 }
 
+// ---------------------------------------------------------------- dynamic-loop error norms (Alg. 1 lines 22, 24)
+__device__ __forceinline__ double block_max(double m) {
+  __shared__ double shm[32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if (lane == 0) shm[warp] = m;
+  __syncthreads();
+  if (warp == 0) {
+    m = lane < (int)(blockDim.x >> 5) ? shm[lane] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  }
+  return m;      // valid in thread 0
+}
+
+__global__ void __launch_bounds__(RB)
+commutator_check_kernel(long long n, const double* __restrict__ a, const double* __restrict__ b, int k, double thrs,
+                        ConvState* __restrict__ cs) {
+  // `done` can only be set by the last block of an EARLIER launch (every block of this one arrives first)
+  if (*reinterpret_cast<volatile int*>(&cs->done)) return;
+  double m = 0.0;
+  for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < n; r += (long long)gridDim.x * RB)
+    m = fmax(m, fmax(fabs(a[r]), fabs(b[r])));
+  m = block_max(m);
+  if (threadIdx.x == 0) {
+    atomicMax(&cs->dP_bits[k], (unsigned long long)__double_as_longlong(m));
+    __threadfence();
+    if (atomicAdd(&cs->arrived[k], 1u) == gridDim.x - 1) {
+      __threadfence();
+      const double err = __longlong_as_double((long long)atomicMax(&cs->dP_bits[k], 0ull));
+      cs->k_used = k;
+      if (!(err > thrs)) cs->done = 1;          // Alg. 1 line 18: while (dP_err > dP_thrs)
+    }
+  }
+}
+static int norm_blocks(long long n) {
+  long long nb = (n + RB * 4 - 1) / (RB * 4);
+  return (int)(nb < 1 ? 1 : (nb > 148 * 8 ? 148 * 8 : nb));
+}
+void launch_commutator_check(int N, int ldn, const double* dPr, const double* dPi, int k, double thrs, ConvState* cs,
+                             cudaStream_t st) {
+  const long long n = (long long)N * ldn;      // padding columns hold zeros
+  commutator_check_kernel<<<norm_blocks(n), RB, 0, st>>>(n, dPr, dPi, k, thrs, cs);
+}
+
+__global__ void __launch_bounds__(RB)
+maxabs_diff_kernel(long long n, const double* __restrict__ a, const double* __restrict__ b, ConvState* __restrict__ cs) {
+  double m = 0.0;
+  for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < n; r += (long long)gridDim.x * RB)
+    m = fmax(m, fabs(a[r] - b[r]));
+  m = block_max(m);
+  if (threadIdx.x == 0) atomicMax(&cs->H_bits, (unsigned long long)__double_as_longlong(m));
+}
+void launch_maxabs_diff(int N, int ldn, const double* A, const double* B, ConvState* cs, cudaStream_t st) {
+  const long long n = (long long)N * ldn;
+  maxabs_diff_kernel<<<norm_blocks(n), RB, 0, st>>>(n, A, B, cs);
+}
+
 __global__ void set_diag_kernel(int N, int ldn, double* __restrict__ M, const double* __restrict__ d) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
   if (j >= ldn) return;

@@ -58,6 +58,20 @@ struct rt_ctx {
 
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t gexec = nullptr;
+  // dynamic-H_thrs mode: one graph per kind of Hamiltonian update (first of a step / later ones)
+  cudaGraph_t graph_upd[2] = {nullptr, nullptr};
+  cudaGraphExec_t gexec_upd[2] = {nullptr, nullptr};
+  int64_t launches_per_upd[2] = {0, 0};
+
+  // the paper's loops (Alg. 1 lines 12-26): commutator series with dP_thrs, Hamiltonian loop with H_thrs
+  int prop = RT_PROP_TAYLOR;
+  int kmax = 0;
+  double dP_thrs = 0, H_thrs = 0;
+  int max_hup = 0;
+  bool dynamic = false;
+  ConvState* d_cs = nullptr;
+  int last_hupdates = 0, last_orders = 0;
+  double last_H_err = 0, last_dP_err = 0;
 
   // TMA descriptors: Phi as a K-contiguous operand (box 16 x 128) and as an N-contiguous one (box 16 x 16);
   // one K-contiguous descriptor per library-owned N x N buffer
@@ -241,8 +255,8 @@ void stage_end(rt_ctx* c) {
 // ---- the stages ------------------------------------------------------------------------------------
 void enqueue_gemm(rt_ctx* c, int sym, const double* A0, const double* B0, double a0, const double* A1,
                   const double* B1, double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr,
-                  double b2 = 0) {
-  GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2};
+                  double b2 = 0, const int* skip = nullptr) {
+  GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2, skip};
   if (c->use_tma) {
     const CUtensorMap& mA0 = nn_map(c, A0);
     const CUtensorMap& mB0 = nn_map(c, B0);
@@ -280,6 +294,40 @@ void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, doub
   enqueue_gemm(c, 0, c->Cm, Ai, -1.0, c->Sm, Ar, -1.0, c->Yc);
   enqueue_gemm(c, 1, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, Or);      // P1 Hermitian: Re symmetric,
   enqueue_gemm(c, -1, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, Oi);      // Im antisymmetric
+}
+
+// The paper's propagator (Eq. 39, Alg. 1 lines 15-23 L375-L392) with S = 1 and Hbar real symmetric (L433):
+//   dP^(k) = (1/k)(Omega dP^(k-1) + dP^(k-1) Omega^dagger) = (-i/k)[X, dP^(k-1)],  X = dt Hbar;  P1 = P0 + sum_k dP^(k)
+// split as in Eq. 40 (L428-L433) with dP = S' + iA':   S'' = (1/k)[X, A'],  A'' = -(1/k)[X, S'].
+// Each commutator is ONE dual-term GEMM whose output is known to be (anti)symmetric, so only the upper tiles are
+// computed and mirrored -- the same 2N^3 flop as the paper's "one multiply + transpose (DGEAM)" form (L434-L438).
+// gemm_abt contracts against B^T:  X A' = -gemm(X, A'),  A' X = gemm(A', X),  X S' = gemm(X, S'),  S' X = gemm(S', X).
+// (X carries the shift -sigma dt I, which commutes with everything.)  The loop `while dP_err > dP_thrs` runs on the
+// device: commutator_check sets cs->done and the GEMMs of the remaining orders (up to kmax) return immediately.
+void enqueue_commutator(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
+  const size_t nn = (size_t)c->N * c->ldn * 8;
+  cudaMemcpyAsync(Or, Ar, nn, cudaMemcpyDeviceToDevice, c->st);               // line 15: P1 <- P0
+  cudaMemcpyAsync(Oi, Ai, nn, cudaMemcpyDeviceToDevice, c->st);
+  const double* pr = Ar;                                                      // line 17 (DESIGN R2): dP <- P0
+  const double* pi = Ai;
+  double* bufs[2][2] = {{c->Yb, c->Yc}, {c->Cm, c->Sm}};
+  const int* skip = &c->d_cs->done;
+  for (int k = 1; k <= c->kmax; ++k) {
+    double* nr = bufs[k & 1][0];
+    double* ni = bufs[k & 1][1];
+    const double s = 1.0 / (double)k;
+    enqueue_gemm(c, 1, c->X, pi, -s, pi, c->X, -s, nr, Or, 1.0, nullptr, 0, skip);    // S'' and P1r += S''  (lines 20-21)
+    enqueue_gemm(c, -1, c->X, pr, -s, pr, c->X, s, ni, Oi, 1.0, nullptr, 0, skip);    // A'' and P1i += A''
+    launch_commutator_check(c->N, c->ldn, nr, ni, k, c->dP_thrs, c->d_cs, c->st);     // line 22
+    c->launches += 1;
+    pr = nr;
+    pi = ni;
+  }
+}
+
+void enqueue_propagate(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
+  if (c->prop == RT_PROP_COMMUTATOR) enqueue_commutator(c, Ar, Ai, Or, Oi);
+  else { enqueue_expm(c); enqueue_upu(c, Ar, Ai, Or, Oi); }
 }
 
 void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double* rho0) {
@@ -332,39 +380,52 @@ void enqueue_project(rt_ctx* c, const double* w, const double* eps, double* H) {
   c->launches += 2;
 }
 
-// One time step, Algorithm 1 lines 10-28.
-void enqueue_step(rt_ctx* c) {
-  for (int it = 0; it < c->m; ++it) {
-    stage_begin(c, RT_STAGE_ELDYN);
-    launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st);   // lines 11, 14
+// One Hamiltonian update, Algorithm 1 lines 14-25 (`it` = 0 also extrapolates H1, line 11).
+void enqueue_update(rt_ctx* c, int it) {
+  stage_begin(c, RT_STAGE_ELDYN);
+  if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);                          // lines 12, 16
+  launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st);     // lines 11, 14
+  c->launches += 1;
+  enqueue_propagate(c, c->P0r, c->P0i, c->P1r, c->P1i);                                        // Eq. 15 / Eq. 39
+  stage_end(c);
+
+  stage_begin(c, RT_STAGE_RHO);
+  enqueue_density(c, c->P1r, c->rho, c->rho0);                                                 // Eq. 27 + line 27
+  stage_end(c);
+
+  if (c->use_h) {
+    stage_begin(c, RT_STAGE_VH);
+    launch_poisson_rhs(c->Ng, c->rho, c->rho0, c->d_sums, c->lv[0].f, c->st);
     c->launches += 1;
-    enqueue_expm(c);
-    enqueue_upu(c, c->P0r, c->P0i, c->P1r, c->P1i);                                            // Eq. 15
-    stage_end(c);
-
-    stage_begin(c, RT_STAGE_RHO);
-    enqueue_density(c, c->P1r, c->rho, c->rho0);                                               // Eq. 27 + line 27
-    stage_end(c);
-
-    if (c->use_h) {
-      stage_begin(c, RT_STAGE_VH);
-      launch_poisson_rhs(c->Ng, c->rho, c->rho0, c->d_sums, c->lv[0].f, c->st);
-      c->launches += 1;
-      for (int v = 0; v < c->n_vc; ++v) enqueue_vcycle(c, c->lv, 0);
-      stage_end(c);
-    }
-
-    stage_begin(c, RT_STAGE_XC);
-    launch_delta_v(c->Ng, c->gd, c->h, c->rho, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->w, c->st);
-    c->launches += 1;
-    stage_end(c);
-
-    stage_begin(c, RT_STAGE_HUPDATE);
-    enqueue_project(c, c->w, c->d_eps, c->H1);                                                 // line 25
+    for (int v = 0; v < c->n_vc; ++v) enqueue_vcycle(c, c->lv, 0);
     stage_end(c);
   }
+
+  stage_begin(c, RT_STAGE_XC);
+  launch_delta_v(c->Ng, c->gd, c->h, c->rho, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->w, c->st);
+  c->launches += 1;
+  stage_end(c);
+
+  stage_begin(c, RT_STAGE_HUPDATE);
+  if (c->dynamic)                                                                              // H1_old <- H1
+    cudaMemcpyAsync(c->Ya, c->H1, (size_t)c->N * c->ldn * 8, cudaMemcpyDeviceToDevice, c->st);
+  enqueue_project(c, c->w, c->d_eps, c->H1);                                                   // line 25
+  if (c->dynamic) {
+    launch_maxabs_diff(c->N, c->ldn, c->H1, c->Ya, c->d_cs, c->st);                            // line 24
+    c->launches += 1;
+  }
+  stage_end(c);
+}
+
+void enqueue_shift(rt_ctx* c) {
   launch_copy5(c->N, c->ldn, c->Hm1, c->H0, c->H0, c->H1, c->P0r, c->P1r, c->P0i, c->P1i, c->st);   // line 28
   c->launches += 1;
+}
+
+// One time step with a fixed number of Hamiltonian updates, Algorithm 1 lines 10-28.
+void enqueue_step(rt_ctx* c) {
+  for (int it = 0; it < c->m; ++it) enqueue_update(c, it);
+  enqueue_shift(c);
 }
 
 int sync_and_check(rt_ctx* c) {
@@ -409,6 +470,10 @@ int rt_destroy(rt_handle c) {
   cudaStreamSynchronize(c->st);
   if (c->gexec) cudaGraphExecDestroy(c->gexec);
   if (c->graph) cudaGraphDestroy(c->graph);
+  for (int i = 0; i < 2; ++i) {
+    if (c->gexec_upd[i]) cudaGraphExecDestroy(c->gexec_upd[i]);
+    if (c->graph_upd[i]) cudaGraphDestroy(c->graph_upd[i]);
+  }
   for (auto& ep : c->ev_used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
   for (auto& ep : c->ev_free) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
   for (void* p : c->allocs) cudaFree(p);
@@ -426,6 +491,11 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   if (cfg->norb < 1) return fail(c, RT_EINVAL, "rt_create: norb must be >= 1");
   if (cfg->n_hupdates < 0 || cfg->n_vcycles < 0 || cfg->nu_pre < 0 || cfg->nu_post < 0 || cfg->exp_order < 0)
     return fail(c, RT_EINVAL, "rt_create: negative iteration count");
+  if (cfg->propagator != RT_PROP_TAYLOR && cfg->propagator != RT_PROP_COMMUTATOR)
+    return fail(c, RT_EINVAL, "rt_create: unknown propagator");
+  if (cfg->max_order < 0 || cfg->max_order > MAX_ORDER || cfg->max_hupdates < 0 || !(cfg->dP_thrs >= 0.0) ||
+      !(cfg->H_thrs >= 0.0))
+    return fail(c, RT_EINVAL, "rt_create: bad max_order / max_hupdates / dP_thrs / H_thrs");
   for (int i = 0; i < cfg->norb; ++i)
     if (!(occ[i] >= 0.0 && occ[i] <= 2.0)) return fail(c, RT_EINVAL, "rt_create: occ must lie in [0, 2]");
 
@@ -481,6 +551,20 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
       while (term > 1e-17 && q < 40) { ++q; term *= theta * theta / ((2.0 * q + 1.0) * (2.0 * q + 2.0)); }
     }
     c->q = q;
+    // the paper's loops: thresholds of Alg. 1 line 5 (L351); kmax from the same spectral bound -- the k-th term of
+    // the commutator series is bounded by max|P0| (2 theta)^k / k!  (||ad_X|| <= 2 ||X||)
+    c->prop = cfg->propagator;
+    c->dP_thrs = cfg->dP_thrs > 0.0 ? cfg->dP_thrs : 1e-10;
+    c->H_thrs = cfg->H_thrs;
+    c->dynamic = cfg->H_thrs > 0.0;
+    c->max_hup = cfg->max_hupdates > 0 ? cfg->max_hupdates : 20;
+    if (cfg->max_order > 0) c->kmax = cfg->max_order;
+    else {
+      int k = 1;
+      double term = 2.0 * 2.0 * theta;
+      while (term > 1e-3 * c->dP_thrs && k < MAX_ORDER) { ++k; term *= 2.0 * theta / k; }
+      c->kmax = k + 2 < MAX_ORDER ? k + 2 : MAX_ORDER;
+    }
   }
 
   // multigrid hierarchy
@@ -578,6 +662,10 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   const size_t nn = (size_t)N * ldn;
   ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8); ALLOC(c->d_sums, 8);
   ALLOC(c->d_bsums, 5 * 1024);
+  if (c->prop == RT_PROP_COMMUTATOR || c->dynamic) {
+    ALLOC(c->d_cs, 1);
+    CKC(cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st));
+  }
   double** mats[] = {&c->Hm1, &c->H0, &c->H1, &c->X, &c->Ya, &c->Yb, &c->Yc, &c->Cm, &c->Sc, &c->Sm,
                      &c->P0r, &c->P0i, &c->P1r, &c->P1i};
   for (double** mp : mats) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
@@ -640,7 +728,8 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   CKC(cudaStreamSynchronize(c->st));
   CKC(cudaGetLastError());
 
-  // capture one step into a CUDA graph (pointers are fixed: line 28 is a copy, not a pointer rotation)
+  // capture one step into a CUDA graph (pointers are fixed: line 28 is a copy, not a pointer rotation).  With
+  // H_thrs > 0 the number of updates is decided on the host, so the unit captured is one Hamiltonian update.
   {
     const int64_t before = c->launches;
     if (c->use_graph) {
@@ -649,19 +738,32 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
       cudaStream_t user = c->st, cap = nullptr;
       CKC(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
       c->st = cap;
-      cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
-      if (e == cudaSuccess) {
-        enqueue_step(c);
-        e = cudaStreamEndCapture(cap, &c->graph);
+      cudaError_t e = cudaSuccess;
+      if (!c->dynamic) {
+        e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) {
+          enqueue_step(c);
+          e = cudaStreamEndCapture(cap, &c->graph);
+        }
+        c->launches_per_step = c->launches - before;
+      } else {
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+          const int64_t b0 = c->launches;
+          e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+          if (e == cudaSuccess) {
+            enqueue_update(c, i);
+            e = cudaStreamEndCapture(cap, &c->graph_upd[i]);
+          }
+          c->launches_per_upd[i] = c->launches - b0;
+        }
       }
       c->st = user;
       cudaStreamDestroy(cap);
       if (e != cudaSuccess) { cudaGetLastError(); FAIL_CREATE(RT_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
-      CKC(cudaGraphInstantiate(&c->gexec, c->graph, 0));
-    } else {
-      // dry count without launching anything is not possible; count on the first real step instead
+      if (c->graph) CKC(cudaGraphInstantiate(&c->gexec, c->graph, 0));
+      for (int i = 0; i < 2; ++i)
+        if (c->graph_upd[i]) CKC(cudaGraphInstantiate(&c->gexec_upd[i], c->graph_upd[i], 0));
     }
-    c->launches_per_step = c->launches - before;
     c->launches = before;
   }
 #undef ALLOC
@@ -684,7 +786,33 @@ int rt_step(rt_handle c, int32_t nsteps) {
   if (nsteps < 0) return fail(c, RT_EINVAL, "rt_step: nsteps < 0");
   CK(cudaSetDevice(c->cfg.device));
   for (int s = 0; s < nsteps; ++s) {
-    if (c->gexec && !c->timing) {
+    if (c->dynamic) {
+      // Alg. 1 lines 12-26: while (H_err > H_thrs).  The decision needs H_err on the host: one 8-byte read and a
+      // stream synchronisation per Hamiltonian update.
+      int it = 0;
+      double herr = 2.0 * c->H_thrs;
+      while (herr > c->H_thrs && it < c->max_hup) {
+        const int kind = it == 0 ? 0 : 1;
+        if (c->gexec_upd[kind] && !c->timing) {
+          CK(cudaGraphLaunch(c->gexec_upd[kind], c->st));
+          c->launches += c->launches_per_upd[kind];
+        } else {
+          enqueue_update(c, kind);
+          CK(cudaGetLastError());
+        }
+        ConvState hs;
+        CK(cudaMemcpyAsync(&hs, c->d_cs, sizeof hs, cudaMemcpyDeviceToHost, c->st));
+        if (int rc = sync_and_check(c)) return rc;
+        memcpy(&herr, &hs.H_bits, 8);
+        c->last_orders = hs.k_used;
+        memcpy(&c->last_dP_err, &hs.dP_bits[hs.k_used], 8);
+        ++it;
+      }
+      enqueue_shift(c);
+      CK(cudaGetLastError());
+      c->last_hupdates = it;
+      c->last_H_err = herr;
+    } else if (c->gexec && !c->timing) {
       CK(cudaGraphLaunch(c->gexec, c->st));
       c->launches += c->launches_per_step;
     } else {
@@ -694,6 +822,27 @@ int rt_step(rt_handle c, int32_t nsteps) {
       CK(cudaGetLastError());
     }
     c->t += c->dt;
+  }
+  return RT_OK;
+}
+
+int rt_get_convergence(rt_handle c, int32_t n[2], double err[2]) {
+  CHECK_HANDLE(c);
+  if (!n || !err) return fail(c, RT_EINVAL, "rt_get_convergence: NULL");
+  CK(cudaSetDevice(c->cfg.device));
+  n[0] = c->dynamic ? c->last_hupdates : c->m;
+  n[1] = 0;
+  err[0] = c->dynamic ? c->last_H_err : 0.0;
+  err[1] = 0.0;
+  if (c->d_cs && c->prop == RT_PROP_COMMUTATOR) {
+    if (c->dynamic) { n[1] = c->last_orders; err[1] = c->last_dP_err; }
+    else {
+      ConvState hs;
+      CK(cudaMemcpyAsync(&hs, c->d_cs, sizeof hs, cudaMemcpyDeviceToHost, c->st));
+      if (int rc = sync_and_check(c)) return rc;
+      n[1] = hs.k_used;
+      memcpy(&err[1], &hs.dP_bits[hs.k_used], 8);
+    }
   }
   return RT_OK;
 }
@@ -836,8 +985,8 @@ int rt_op_propagate(rt_handle c, const double* Hbar, const double* P0re, const d
     stage_begin(c, RT_STAGE_ELDYN);
     launch_hbar(c->N, c->ldn, T[0], T[0], T[0], c->X, c->dt, c->sigma, 0, c->st);   // X = dt (Hbar - sigma I)
     c->launches += 1;
-    enqueue_expm(c);
-    enqueue_upu(c, T[1], T[2], T[3], T[4]);
+    if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);
+    enqueue_propagate(c, T[1], T[2], T[3], T[4]);
     stage_end(c);
     if ((rc = copy_matrix_out(c, T[3], P1re))) break;
     if ((rc = copy_matrix_out(c, T[4], P1im))) break;

@@ -55,6 +55,7 @@ struct GemmArgs {
   double* D;                                            // may be nullptr (only the axpys are wanted)
   double* Z1; double beta1;                             // may be nullptr
   double* Z2; double beta2;
+  const int* skip;                                      // device flag (may be nullptr): non-zero -> the launch is a no-op
 };
 void launch_gemm_abt(const GemmArgs& g, cudaStream_t st);
 size_t gemm_smem_bytes();
@@ -98,6 +99,23 @@ void launch_field(long long Ng, GridDims gd, double h, const double* E, double* 
 // f = 4 pi (rho - rho0 - sums[4]/Ng)      (rho0 may be nullptr: f = 4 pi (rho - sums[4]/Ng))
 void launch_poisson_rhs(long long Ng, const double* rho, const double* rho0, const double* sums, double* f,
                         cudaStream_t st);
+
+// ---- convergence state of the paper's dynamic loops (Alg. 1 lines 12-13, 16-23) ----
+// Lives in device memory; the host reads it only in the dynamic-H_thrs mode and in rt_get_convergence.
+constexpr int MAX_ORDER = 96;
+struct ConvState {
+  unsigned long long dP_bits[MAX_ORDER + 1];   // max|dP^(k)|, bit pattern of a non-negative double (atomicMax)
+  unsigned int arrived[MAX_ORDER + 1];         // blocks of commutator_check that have contributed to order k
+  int done;                                    // dP_err <= dP_thrs reached: the GEMMs of later orders skip themselves
+  int k_used;                                  // orders summed into P1
+  unsigned long long H_bits;                   // max|H1 - H1_old| of this Hamiltonian update
+};
+// after the two GEMMs of order k: dP_err = max(|dPr|, |dPi|) over the matrix; the last block to arrive sets
+// k_used = k and done = (dP_err <= thrs).  A no-op once done is set.
+void launch_commutator_check(int N, int ldn, const double* dPr, const double* dPi, int k, double thrs, ConvState* cs,
+                             cudaStream_t st);
+// cs->H_bits = max |A - B| over the N x N matrices (line 24)
+void launch_maxabs_diff(int N, int ldn, const double* A, const double* B, ConvState* cs, cudaStream_t st);
 
 struct MgLevel {
   GridDims gd; double h; long long n;
