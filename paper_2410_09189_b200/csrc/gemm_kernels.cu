@@ -294,17 +294,20 @@ void launch_fold_upper(int N, int ldn, const double* P, double* Pfold, cudaStrea
 // ======================================================================================================
 // a3/a4 N x N GEMM, D = a0 A0 B0^T + a1 A1 B1^T
 // ======================================================================================================
-constexpr int GEMM_STAGE = BM * BK + BN * BK;
-
-__global__ void __launch_bounds__(NT, 1)
+// Tile variants: 128 x 128 (8 warps, warp tile 64 x 32) for large N; 64 x 64 and 32 x 32 CTA tiles for small N, where
+// 128 x 128 tiles would leave most of the 148 SMs idle (N = 128 is ONE such tile, N = 512 sixteen).
+template <int FA, int FB, int WM, int WN>
+__global__ void __launch_bounds__(32 * WM * WN)
 gemm_abt_kernel(GemmArgs ga) {
+  constexpr int BM = 8 * FA * WM, BN = 8 * FB * WN, NT = 32 * WM * WN;
+  constexpr int GEMM_STAGE = BM * BK + BN * BK;
   if (ga.skip && *ga.skip) return;
   extern __shared__ __align__(16) double smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g = lane >> 2, c = lane & 3;
   const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
   const int N = ga.N, ldn = ga.ldn;
-  const int i0 = blockIdx.y * TILE, j0 = blockIdx.x * TILE;
+  const int i0 = blockIdx.y * BM, j0 = blockIdx.x * BN;
   const int nk1 = (N + BK - 1) / BK;
   const int nk = ga.A1 ? 2 * nk1 : nk1;
 
@@ -377,16 +380,24 @@ gemm_abt_kernel(GemmArgs ga) {
   }
 }
 
-size_t gemm_smem_bytes() { return (size_t)STAGES * GEMM_STAGE * sizeof(double); }
+size_t gemm_smem_bytes() { return (size_t)STAGES * (BM * BK + BN * BK) * sizeof(double); }
 
-void launch_gemm_abt(const GemmArgs& g, cudaStream_t st) {
+template <int FA_, int FB_, int WM_, int WN_>
+static void launch_gemm_variant(const GemmArgs& g, cudaStream_t st) {
+  constexpr int bm = 8 * FA_ * WM_, bn = 8 * FB_ * WN_;
+  const size_t smem = (size_t)STAGES * (bm + bn) * BK * sizeof(double);
   static bool attr = false;
   if (!attr) {
-    cudaFuncSetAttribute(gemm_abt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem_bytes());
+    cudaFuncSetAttribute(gemm_abt_kernel<FA_, FB_, WM_, WN_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr = true;
   }
-  const int nt = (g.N + TILE - 1) / TILE;
-  gemm_abt_kernel<<<dim3(nt, nt), NT, gemm_smem_bytes(), st>>>(g);
+  gemm_abt_kernel<FA_, FB_, WM_, WN_><<<dim3((g.N + bn - 1) / bn, (g.N + bm - 1) / bm), 32 * WM_ * WN_, smem, st>>>(g);
+}
+
+void launch_gemm_abt(const GemmArgs& g, cudaStream_t st) {
+  if (g.N <= GEMM_SMALL_N32) launch_gemm_variant<2, 2, 2, 2>(g, st);          // 32 x 32 tiles, 4 warps
+  else if (g.N <= GEMM_SMALL_N) launch_gemm_variant<4, 2, 2, 4>(g, st);        // 64 x 64 tiles, 8 warps
+  else launch_gemm_variant<FA, FB, WM, WN>(g, st);                             // 128 x 128 tiles
 }
 
 }  // namespace rt

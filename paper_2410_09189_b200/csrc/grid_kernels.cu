@@ -2,8 +2,7 @@
 //
 //   a6  reduce_rho      : rho = sum of the density kernel's partials, fused dipole / charge reduction
 //                         (Alg. 1 line 27) with a fixed-order second stage (bit-reproducible).
-//   a7  multigrid       : periodic 7-point Poisson, V(nu1,nu2) cycles, weighted Jacobi, full weighting,
-//                         trilinear prolongation, exact separable solve on the coarsest level ("Vh", L545; DESIGN R6).
+//   a7  poisson_rhs     : right-hand side of the Poisson solve (the multigrid cycle itself is in mg_kernels.cu).
 //   a8  delta_v / vxc   : Slater exchange + PZ81 correlation and the dV assembly ("exchange/correlation", L547).
 //   a2  hbar etc.       : Alg. 1 lines 11, 14, 28 on N x N matrices.
 #include "rt_internal.h"
@@ -184,175 +183,6 @@ poisson_rhs_kernel(long long Ng, const double* __restrict__ rho, const double* _
 void launch_poisson_rhs(long long Ng, const double* rho, const double* rho0, const double* sums, double* f,
                         cudaStream_t st) {
   poisson_rhs_kernel<<<nblk(Ng), RB, 0, st>>>(Ng, rho, rho0, sums, f);
-}
-
-__device__ __forceinline__ void idx3(long long r, GridDims gd, int& ix, int& iy, int& iz) {
-  const long long nyz = (long long)gd.ny * gd.nz;
-  ix = (int)(r / nyz);
-  const int rem = (int)(r - (long long)ix * nyz);
-  iy = rem / gd.nz;
-  iz = rem - iy * gd.nz;
-}
-
-__device__ __forceinline__ double nb_sum(const double* __restrict__ u, GridDims gd, int ix, int iy, int iz) {
-  const long long nyz = (long long)gd.ny * gd.nz;
-  const int xm = ix == 0 ? gd.nx - 1 : ix - 1, xp = ix == gd.nx - 1 ? 0 : ix + 1;
-  const int ym = iy == 0 ? gd.ny - 1 : iy - 1, yp = iy == gd.ny - 1 ? 0 : iy + 1;
-  const int zm = iz == 0 ? gd.nz - 1 : iz - 1, zp = iz == gd.nz - 1 ? 0 : iz + 1;
-  const long long row = (long long)iy * gd.nz, pl = (long long)ix * nyz;
-  return u[xm * nyz + row + iz] + u[xp * nyz + row + iz] + u[pl + (long long)ym * gd.nz + iz] +
-         u[pl + (long long)yp * gd.nz + iz] + u[pl + row + zm] + u[pl + row + zp];
-}
-
-// u_out = (1 - omega) u + (omega / 6) (h^2 f + sum_nb u)
-__global__ void __launch_bounds__(RB)
-jacobi_kernel(GridDims gd, long long n, double h2, double omega, const double* __restrict__ u,
-              const double* __restrict__ f, double* __restrict__ out) {
-  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
-  if (r >= n) return;
-  int ix, iy, iz;
-  idx3(r, gd, ix, iy, iz);
-  out[r] = (1.0 - omega) * u[r] + (omega / 6.0) * (h2 * f[r] + nb_sum(u, gd, ix, iy, iz));
-}
-void launch_jacobi(const MgLevel& L, const double* uin, double* uout, double omega, cudaStream_t st) {
-  jacobi_kernel<<<nblk(L.n), RB, 0, st>>>(L.gd, L.n, L.h * L.h, omega, uin, L.f, uout);
-}
-
-// r = f - (6 u - sum_nb u)/h^2
-__global__ void __launch_bounds__(RB)
-residual_kernel(GridDims gd, long long n, double inv_h2, const double* __restrict__ u, const double* __restrict__ f,
-                double* __restrict__ res) {
-  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
-  if (r >= n) return;
-  int ix, iy, iz;
-  idx3(r, gd, ix, iy, iz);
-  res[r] = f[r] - (6.0 * u[r] - nb_sum(u, gd, ix, iy, iz)) * inv_h2;
-}
-void launch_residual(const MgLevel& L, cudaStream_t st) {
-  residual_kernel<<<nblk(L.n), RB, 0, st>>>(L.gd, L.n, 1.0 / (L.h * L.h), L.u, L.f, L.r);
-}
-
-// full weighting (1/4,1/2,1/4)^3, coarse I <-> fine 2I
-__global__ void __launch_bounds__(RB)
-restrict_kernel(GridDims gf, GridDims gc, long long nc, const double* __restrict__ res, double* __restrict__ fc) {
-  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
-  if (r >= nc) return;
-  int I, J, K;
-  idx3(r, gc, I, J, K);
-  const long long nyz = (long long)gf.ny * gf.nz;
-  double s = 0.0;
-#pragma unroll
-  for (int a = -1; a <= 1; ++a) {
-    int x = 2 * I + a; x = x < 0 ? x + gf.nx : (x >= gf.nx ? x - gf.nx : x);
-    const double wa = a == 0 ? 0.5 : 0.25;
-    double sy = 0.0;
-#pragma unroll
-    for (int b = -1; b <= 1; ++b) {
-      int y = 2 * J + b; y = y < 0 ? y + gf.ny : (y >= gf.ny ? y - gf.ny : y);
-      const double wb = b == 0 ? 0.5 : 0.25;
-      const double* p = res + x * nyz + (long long)y * gf.nz;
-      const int z0 = 2 * K;
-      const int zm = z0 == 0 ? gf.nz - 1 : z0 - 1, zp = z0 + 1 >= gf.nz ? z0 + 1 - gf.nz : z0 + 1;
-      sy += wb * (0.25 * p[zm] + 0.5 * p[z0] + 0.25 * p[zp]);
-    }
-    s += wa * sy;
-  }
-  fc[r] = s;
-}
-void launch_restrict(const MgLevel& fine, const MgLevel& coarse, cudaStream_t st) {
-  restrict_kernel<<<nblk(coarse.n), RB, 0, st>>>(fine.gd, coarse.gd, coarse.n, fine.r, coarse.f);
-}
-
-// trilinear prolongation, added to the fine solution
-__global__ void __launch_bounds__(RB)
-prolong_add_kernel(GridDims gf, GridDims gc, long long nf, const double* __restrict__ ec, double* __restrict__ u) {
-  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
-  if (r >= nf) return;
-  int ix, iy, iz;
-  idx3(r, gf, ix, iy, iz);
-  const int I0 = ix >> 1, J0 = iy >> 1, K0 = iz >> 1;
-  const int I1 = (ix & 1) ? (I0 + 1 == gc.nx ? 0 : I0 + 1) : I0;
-  const int J1 = (iy & 1) ? (J0 + 1 == gc.ny ? 0 : J0 + 1) : J0;
-  const int K1 = (iz & 1) ? (K0 + 1 == gc.nz ? 0 : K0 + 1) : K0;
-  const long long nyz = (long long)gc.ny * gc.nz;
-  auto at = [&](int I, int J, int K) { return ec[I * nyz + (long long)J * gc.nz + K]; };
-  // 0.5 (a + b) with a == b on even points reproduces the injected value exactly
-  const double z00 = 0.5 * (at(I0, J0, K0) + at(I0, J0, K1));
-  const double z01 = 0.5 * (at(I0, J1, K0) + at(I0, J1, K1));
-  const double z10 = 0.5 * (at(I1, J0, K0) + at(I1, J0, K1));
-  const double z11 = 0.5 * (at(I1, J1, K0) + at(I1, J1, K1));
-  const double y0 = 0.5 * (z00 + z01), y1 = 0.5 * (z10 + z11);
-  u[r] += 0.5 * (y0 + y1);
-}
-void launch_prolong_add(const MgLevel& coarse, const MgLevel& fine, cudaStream_t st) {
-  prolong_add_kernel<<<nblk(fine.n), RB, 0, st>>>(fine.gd, coarse.gd, fine.n, coarse.u, fine.u);
-}
-
-__global__ void __launch_bounds__(RB) zero_kernel(double* __restrict__ p, long long n) {
-  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
-  if (r < n) p[r] = 0.0;
-}
-void launch_zero(double* p, long long n, cudaStream_t st) { zero_kernel<<<nblk(n), RB, 0, st>>>(p, n); }
-
-// Exact solve on the coarsest level in the zero-mean subspace: u = (Qx x Qy x Qz) L^+ (Qx x Qy x Qz)^T f with
-// the real orthonormal eigenvectors of the periodic 1-D operator (columns of Q) and eigenvalues lx+ly+lz.
-// One CTA; two global scratch buffers (L.r and L.tmp) ping-pong between the six axis passes.
-__global__ void __launch_bounds__(1024)
-coarse_solve_kernel(GridDims gd, const double* __restrict__ f, double* __restrict__ u, double* __restrict__ s0,
-                    double* __restrict__ s1, const double* __restrict__ Qx, const double* __restrict__ Qy,
-                    const double* __restrict__ Qz, const double* __restrict__ lx, const double* __restrict__ ly,
-                    const double* __restrict__ lz) {
-  const int nx = gd.nx, ny = gd.ny, nz = gd.nz;
-  const int n = nx * ny * nz;
-  const int tid = threadIdx.x, nt = blockDim.x;
-  // forward: contract each axis with Q^T  (out[a] = sum_i Q[i][a] in[i])
-  for (int o = tid; o < n; o += nt) {                    // x axis: f -> s0
-    const int a = o / (ny * nz), rest = o % (ny * nz);
-    double s = 0.0;
-    for (int i = 0; i < nx; ++i) s += Qx[i * nx + a] * f[i * ny * nz + rest];
-    s0[o] = s;
-  }
-  __syncthreads();
-  for (int o = tid; o < n; o += nt) {                    // y axis: s0 -> s1
-    const int a = o / (ny * nz), b = (o / nz) % ny, k = o % nz;
-    double s = 0.0;
-    for (int j = 0; j < ny; ++j) s += Qy[j * ny + b] * s0[(a * ny + j) * nz + k];
-    s1[o] = s;
-  }
-  __syncthreads();
-  for (int o = tid; o < n; o += nt) {                    // z axis + divide by the eigenvalue: s1 -> s0
-    const int a = o / (ny * nz), b = (o / nz) % ny, cc = o % nz;
-    double s = 0.0;
-    for (int k = 0; k < nz; ++k) s += Qz[k * nz + cc] * s1[(a * ny + b) * nz + k];
-    const double lam = lx[a] + ly[b] + lz[cc];
-    s0[o] = (a == 0 && b == 0 && cc == 0) ? 0.0 : s / lam;
-  }
-  __syncthreads();
-  // backward: contract each axis with Q  (out[i] = sum_a Q[i][a] in[a])
-  for (int o = tid; o < n; o += nt) {                    // z: s0 -> s1
-    const int a = o / (ny * nz), b = (o / nz) % ny, k = o % nz;
-    double s = 0.0;
-    for (int cc = 0; cc < nz; ++cc) s += Qz[k * nz + cc] * s0[(a * ny + b) * nz + cc];
-    s1[o] = s;
-  }
-  __syncthreads();
-  for (int o = tid; o < n; o += nt) {                    // y: s1 -> s0
-    const int a = o / (ny * nz), j = (o / nz) % ny, k = o % nz;
-    double s = 0.0;
-    for (int b = 0; b < ny; ++b) s += Qy[j * ny + b] * s1[(a * ny + b) * nz + k];
-    s0[o] = s;
-  }
-  __syncthreads();
-  for (int o = tid; o < n; o += nt) {                    // x: s0 -> u
-    const int i = o / (ny * nz), rest = o % (ny * nz);
-    double s = 0.0;
-    for (int a = 0; a < nx; ++a) s += Qx[i * nx + a] * s0[a * ny * nz + rest];
-    u[o] = s;
-  }
-}
-void launch_coarse_solve(const MgLevel& L, const double* Qx, const double* Qy, const double* Qz, const double* lx,
-                         const double* ly, const double* lz, cudaStream_t st) {
-  coarse_solve_kernel<<<1, 1024, 0, st>>>(L.gd, L.f, L.u, L.r, L.tmp, Qx, Qy, Qz, lx, ly, lz);
 }
 
 // ---------------------------------------------------------------------------------------------- a2 and glue

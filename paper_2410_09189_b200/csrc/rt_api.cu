@@ -257,7 +257,7 @@ void enqueue_gemm(rt_ctx* c, int sym, const double* A0, const double* B0, double
                   const double* B1, double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr,
                   double b2 = 0, const int* skip = nullptr) {
   GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2, skip};
-  if (c->use_tma) {
+  if (c->use_tma && c->N > GEMM_SMALL_N) {
     const CUtensorMap& mA0 = nn_map(c, A0);
     const CUtensorMap& mB0 = nn_map(c, B0);
     launch_gemm_abt_tma(g, mA0, mB0, A1 ? nn_map(c, A1) : mA0, B1 ? nn_map(c, B1) : mB0, sym, c->d_tiles,
@@ -339,38 +339,11 @@ void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double
   c->launches += 4;
 }
 
-void enqueue_smooth(rt_ctx* c, const MgLevel& L, int n) {
-  const double* in = L.u;
-  double* out = L.tmp;
-  for (int s = 0; s < n; ++s) {
-    launch_jacobi(L, in, out, c->omega, c->st);
-    c->launches += 1;
-    const double* t = in; in = out; out = const_cast<double*>(t);
-  }
-  if (n & 1) {   // odd sweep count: result sits in tmp, bring it home
-    cudaMemcpyAsync(L.u, L.tmp, (size_t)L.n * sizeof(double), cudaMemcpyDeviceToDevice, c->st);
-  }
-}
-
-void enqueue_vcycle(rt_ctx* c, std::vector<MgLevel>& lv, size_t l) {
-  MgLevel& L = lv[l];
-  if (l + 1 == lv.size()) {
-    launch_coarse_solve(L, c->Qx, c->Qy, c->Qz, c->lx, c->ly, c->lz, c->st);
-    c->launches += 1;
-    return;
-  }
-  enqueue_smooth(c, L, c->nu1);
-  launch_residual(L, c->st);
-  launch_restrict(L, lv[l + 1], c->st);
-  c->launches += 2;
-  if (l + 2 < lv.size()) {        // zero initial guess (the exact coarsest solve overwrites u)
-    launch_zero(lv[l + 1].u, lv[l + 1].n, c->st);
-    c->launches += 1;
-  }
-  enqueue_vcycle(c, lv, l + 1);
-  launch_prolong_add(lv[l + 1], L, c->st);
-  c->launches += 1;
-  enqueue_smooth(c, L, c->nu2);
+// a7: one Poisson solve on the hierarchy `lv` (lv[0].u is warm-started), right-hand side from rho - rho0
+void enqueue_poisson(rt_ctx* c, const std::vector<MgLevel>& lv, int n_vc, const double* rho, const double* rho0) {
+  MgSolveArgs s{lv.data(), (int)lv.size(), n_vc, c->nu1, c->nu2, c->omega, c->Qx, c->Qy, c->Qz, c->lx, c->ly, c->lz,
+                rho, rho0, c->d_sums};
+  c->launches += launch_mg_solve(s, c->st);
 }
 
 void enqueue_project(rt_ctx* c, const double* w, const double* eps, double* H) {
@@ -395,9 +368,7 @@ void enqueue_update(rt_ctx* c, int it) {
 
   if (c->use_h) {
     stage_begin(c, RT_STAGE_VH);
-    launch_poisson_rhs(c->Ng, c->rho, c->rho0, c->d_sums, c->lv[0].f, c->st);
-    c->launches += 1;
-    for (int v = 0; v < c->n_vc; ++v) enqueue_vcycle(c, c->lv, 0);
+    enqueue_poisson(c, c->lv, c->n_vc, c->rho, c->rho0);
     stage_end(c);
   }
 
@@ -654,6 +625,11 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     if (!make_map(&c->tmPhiK, c->phi, N, Ng, Ng, BK_HOST, TILE)) c->use_tma = false;
     else if (make_map_phi3d(&c->tmPhiN, c->phi, N, Ng)) c->phiN_3d = 1;
     else if (!make_map(&c->tmPhiN, c->phi, N, Ng, Ng, 16, BK_HOST)) c->use_tma = false;
+  }
+  if (c->use_h) {
+    if ((int)c->lv.size() > MG_MAX_LEVELS) FAIL_CREATE(RT_EINVAL, "rt_create: too many multigrid levels");
+    const int e = init_mg_kernels();
+    if (e != 0) FAIL_CREATE(RT_ECUDA, std::string("init_mg_kernels: ") + cudaGetErrorString((cudaError_t)e));
   }
   if (c->use_tma) {
     const int e = init_tma_kernels();
@@ -1011,9 +987,8 @@ int rt_op_hartree(rt_handle c, double* vh, const double* drho, int32_t n_vc) {
   lv[0].u = c->op_u;
   stage_begin(c, RT_STAGE_VH);
   launch_sum_only(c->w, c->Ng, c->d_bsums, c->d_sums, c->st);
-  launch_poisson_rhs(c->Ng, c->w, nullptr, c->d_sums, lv[0].f, c->st);
-  c->launches += 3;
-  for (int v = 0; v < n_vc; ++v) enqueue_vcycle(c, lv, 0);
+  c->launches += 2;
+  enqueue_poisson(c, lv, n_vc, c->w, nullptr);
   stage_end(c);
   CK(cudaMemcpyAsync(vh, c->op_u, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
   if (int rc = sync_and_check(c)) return rc;

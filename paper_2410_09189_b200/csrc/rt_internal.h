@@ -57,6 +57,9 @@ struct GemmArgs {
   double* Z2; double beta2;
   const int* skip;                                      // device flag (may be nullptr): non-zero -> the launch is a no-op
 };
+// N <= GEMM_SMALL_N32: 32 x 32 CTA tiles; N <= GEMM_SMALL_N: 64 x 64; above: 128 x 128 (rt_api.cu sends N > GEMM_SMALL_N
+// to the TMA-fed kernel when TMA is available)
+constexpr int GEMM_SMALL_N32 = 512, GEMM_SMALL_N = 1536;
 void launch_gemm_abt(const GemmArgs& g, cudaStream_t st);
 size_t gemm_smem_bytes();
 
@@ -121,15 +124,20 @@ struct MgLevel {
   GridDims gd; double h; long long n;
   double* u; double* tmp; double* f; double* r;     // solution, ping-pong scratch, rhs, residual
 };
-void launch_jacobi(const MgLevel& L, const double* uin, double* uout, double omega, cudaStream_t st);
-void launch_residual(const MgLevel& L, cudaStream_t st);                        // L.r = L.f - A L.u
-void launch_restrict(const MgLevel& fine, const MgLevel& coarse, cudaStream_t st);   // coarse.f = R fine.r
-void launch_prolong_add(const MgLevel& coarse, const MgLevel& fine, cudaStream_t st); // fine.u += P coarse.u
-void launch_zero(double* p, long long n, cudaStream_t st);
-// exact zero-mean solve on the coarsest level: u = Q L^+ Q^T f, separable real eigenbasis (Qx,Qy,Qz; inverse
-// eigenvalue tables ilx, ily, ilz hold the 1-D eigenvalues).  One CTA.
-void launch_coarse_solve(const MgLevel& L, const double* Qx, const double* Qy, const double* Qz, const double* lx,
-                         const double* ly, const double* lz, cudaStream_t st);
+// One Poisson solve (a7): rhs = 4 pi (rho - rho0 - sums[4]/n), then n_vc V(nu1,nu2) cycles on lv[0].u (warm start).
+// Levels with at most MG_CLUSTER_MAX_PTS points run inside one thread-block-cluster kernel per cycle; larger levels
+// use shared-memory tile kernels (mg_kernels.cu).  Returns the number of kernels enqueued.
+constexpr int MG_MAX_LEVELS = 12;
+constexpr long long MG_CLUSTER_MAX_PTS = 32768;
+struct MgSolveArgs {
+  const MgLevel* lv; int nlev;
+  int n_vc, nu1, nu2; double omega;
+  const double *Qx, *Qy, *Qz, *lx, *ly, *lz;     // eigenbasis of the coarsest level (exact zero-mean solve)
+  const double* rho; const double* rho0;         // rho0 may be nullptr
+  const double* sums;                            // sums[4] = sum(rho - rho0)
+};
+int init_mg_kernels();                           // dynamic shared-memory attributes; returns a cudaError_t value
+int launch_mg_solve(const MgSolveArgs& s, cudaStream_t st);
 // block sums of drho for rt_op_hartree (mean removal): sums[4] = sum(drho)
 void launch_sum_only(const double* v, long long n, double* bsums, double* sums, cudaStream_t st);
 
