@@ -3,13 +3,16 @@
 // says "multigrid", Table 1 "Vh" L545).
 //
 // Two kinds of kernels:
-//   * levels with more than MG_CLUSTER_MAX_PTS points: shared-memory tiles with halos, 3 launches per level per cycle
+//   * large levels: shared-memory tiles with halos, 3 launches per level per cycle
 //       mg_smooth_kernel<false>  : nu (1 or 2) Jacobi sweeps fused; the tile is loaded once with a halo of nu
 //       mg_resid_restrict_kernel : residual on a (2c+1)^3 fine patch kept in shared memory, full weighting -> coarse rhs
 //       mg_smooth_kernel<true>   : u + P e (coarse patch staged in shared memory) followed by the post-sweeps
-//   * all smaller levels: ONE launch of mg_cluster_kernel per cycle (or per solve when the finest level is small):
-//       a thread-block cluster of 8 CTAs walks down and up the hierarchy, phases separated by the hardware cluster
-//       barrier (~0.2 us, flushes L1) instead of kernel boundaries (~2 us each); arrays stay in L2.
+//   * the levels from which the rest of the hierarchy fits one CTA's shared memory (<= 200 KB: 16^3 and below, 13^3):
+//       ONE launch of mg_coarse_kernel<true> per cycle (per solve when even the finest level fits): a single CTA walks
+//       down and up the hierarchy on shared-memory arrays, phases separated by __syncthreads (~0.1 us) instead of
+//       kernel boundaries (~2 us).  A coarsest level too large for that (a grid that cannot be halved) is solved by
+//       mg_coarse_kernel<false>: a cluster of 8 CTAs on global memory, phases separated by the cluster barrier
+//       (measured ~2 us per phase including the L2 round trips, so it is only the fallback).
 // Every value is computed with the same formula and operand order as before the fusion (one thread per output).
 #include "rt_internal.h"
 
@@ -29,13 +32,26 @@ __device__ __forceinline__ int wrapi(int i, int n) {
   i %= n;
   return i < 0 ? i + n : i;
 }
-__device__ __forceinline__ void decode3(int i, int ny, int nz, int& x, int& y, int& z) {
-  const int nyz = ny * nz;
-  x = i / nyz;
-  const int rem = i - x * nyz;
-  y = rem / nz;
-  z = rem - y * nz;
-}
+// Linear index -> (x, y, z) of a box with y-z extents (ny, nz) without integer division: q = floor(i / d) as
+// umulhi(i, ceil(2^32 / d)), exact for i, d < 2^16 (every box here has fewer than 2^16 points; the division was the
+// bottleneck of the first version of these kernels: ~100 instructions per point against ~15 of useful work).
+struct Dec3 {
+  int ny, nz, nyz;
+  unsigned myz, mz;
+  __host__ __device__ static Dec3 make(int ny_, int nz_) {      // two 64-bit divisions: done on the host or once per CTA
+    Dec3 d;
+    d.ny = ny_; d.nz = nz_; d.nyz = ny_ * nz_;
+    d.myz = d.nyz > 1 ? (unsigned)((0x100000000ull + (unsigned)d.nyz - 1) / (unsigned)d.nyz) : 0u;
+    d.mz = nz_ > 1 ? (unsigned)((0x100000000ull + (unsigned)nz_ - 1) / (unsigned)nz_) : 0u;
+    return d;
+  }
+  __device__ __forceinline__ void operator()(int i, int& x, int& y, int& z) const {
+    x = nyz > 1 ? (int)__umulhi((unsigned)i, myz) : i;
+    const int rem = i - x * nyz;
+    y = nz > 1 ? (int)__umulhi((unsigned)rem, mz) : rem;
+    z = rem - y * nz;
+  }
+};
 
 // ------------------------------------------------------------------------------------------- tile kernels
 struct SmoothArgs {
@@ -49,6 +65,7 @@ struct SmoothArgs {
   const double* f;
   const double* ec;      // PROLONG: coarse-level correction
   double* uout;
+  Dec3 decA, decB, decC, decI;   // halo box, halo-1 box, coarse patch, interior
 };
 
 // out = (1 - omega) c + (omega / 6) (h^2 f + neighbours), neighbours summed x-, x+, y-, y+, z-, z+
@@ -68,10 +85,14 @@ __global__ void __launch_bounds__(MG_THREADS) mg_smooth_kernel(const SmoothArgs 
   const int nB = (H == 2) ? (rx - 2) * (ry - 2) * (rz - 2) : 0;
   // coarse patch (PROLONG): covers fine coordinates [x0 - H, x0 + bx + H)
   const int cx = PROLONG ? (rx / 2 + 2) : 0, cy = PROLONG ? (ry / 2 + 2) : 0, cz = PROLONG ? (rz / 2 + 2) : 0;
+  // f on the box of the first sweep (halo H-1), loaded in the same round trip as u
+  const int fx = rx - 2, fy = ry - 2, fz = rz - 2;
+  const int nF = H > 0 ? fx * fy * fz : 0;
   double* A = sm;
   double* B = A + nA;
   double* C = B + nB;
-  int* xs = reinterpret_cast<int*>(C + cx * cy * cz);
+  double* F = C + cx * cy * cz;
+  int* xs = reinterpret_cast<int*>(F + nF);
   int* ys = xs + rx;
   int* zs = ys + ry;
 
@@ -90,18 +111,20 @@ __global__ void __launch_bounds__(MG_THREADS) mg_smooth_kernel(const SmoothArgs 
   if (PROLONG) {
     c0x = (x0 - H) >> 1; c0y = (y0 - H) >> 1; c0z = (z0 - H) >> 1;      // arithmetic shift = floor
     const int ncx = a.gc.nx, ncy = a.gc.ny, ncz = a.gc.nz;
+    const Dec3 decC = a.decC;
     for (int i = tid; i < cx * cy * cz; i += MG_THREADS) {
       int lx, ly, lz;
-      decode3(i, cy, cz, lx, ly, lz);
+      decC(i, lx, ly, lz);
       C[i] = a.ec[((long long)wrapi(c0x + lx, ncx) * ncy + wrapi(c0y + ly, ncy)) * ncz + wrapi(c0z + lz, ncz)];
     }
   }
   __syncthreads();
 
   // load the tile with its halo (periodic wrap); PROLONG: add the trilinear interpolation of the coarse patch
+  const Dec3 decA = a.decA;
   for (int i = tid; i < nA; i += MG_THREADS) {
     int lx, ly, lz;
-    decode3(i, ry, rz, lx, ly, lz);
+    decA(i, lx, ly, lz);
     double v = a.uin ? a.uin[((long long)xs[lx] * ny + ys[ly]) * nz + zs[lz]] : 0.0;
     if (PROLONG) {
       const int X = x0 - H + lx, Y = y0 - H + ly, Z = z0 - H + lz;
@@ -118,22 +141,29 @@ __global__ void __launch_bounds__(MG_THREADS) mg_smooth_kernel(const SmoothArgs 
     }
     A[i] = v;
   }
+  if (H > 0) {
+    const Dec3 decF = a.decB;
+    for (int i = tid; i < nF; i += MG_THREADS) {
+      int lx, ly, lz;
+      decF(i, lx, ly, lz);
+      F[i] = a.f[((long long)xs[lx + 1] * ny + ys[ly + 1]) * nz + zs[lz + 1]];
+    }
+  }
   __syncthreads();
 
   if (H == 2) {       // first sweep: halo-1 region, stays in shared memory
-    const int dy = ry - 2, dz = rz - 2;
+    const Dec3 decB = a.decB;
     for (int i = tid; i < nB; i += MG_THREADS) {
       int lx, ly, lz;
-      decode3(i, dy, dz, lx, ly, lz);
-      const double fv = a.f[((long long)xs[lx + 1] * ny + ys[ly + 1]) * nz + zs[lz + 1]];
-      B[i] = jacobi_point(A, ry, rz, ((lx + 1) * ry + ly + 1) * rz + lz + 1, fv, a.h2, a.omega);
+      decB(i, lx, ly, lz);
+      B[i] = jacobi_point(A, ry, rz, ((lx + 1) * ry + ly + 1) * rz + lz + 1, F[i], a.h2, a.omega);
     }
     __syncthreads();
   }
   if (H == 0) {       // no sweep: u + P e only
     for (int i = tid; i < nA; i += MG_THREADS) {
       int lx, ly, lz;
-      decode3(i, ry, rz, lx, ly, lz);
+      decA(i, lx, ly, lz);
       const int X = x0 + lx, Y = y0 + ly, Z = z0 + lz;
       if (X >= nx || Y >= ny || Z >= nz) continue;
       a.uout[((long long)X * ny + Y) * nz + Z] = A[i];
@@ -142,13 +172,16 @@ __global__ void __launch_bounds__(MG_THREADS) mg_smooth_kernel(const SmoothArgs 
     const double* S = (H == 2) ? B : A;
     const int sy = ry - (H == 2 ? 2 : 0), sz = rz - (H == 2 ? 2 : 0);
     const int nI = a.bx * a.by * a.bz;
+    const Dec3 decI = a.decI;
     for (int i = tid; i < nI; i += MG_THREADS) {
       int lx, ly, lz;
-      decode3(i, a.by, a.bz, lx, ly, lz);
+      decI(i, lx, ly, lz);
       const int X = x0 + lx, Y = y0 + ly, Z = z0 + lz;
       if (X >= nx || Y >= ny || Z >= nz) continue;
       const long long g = ((long long)X * ny + Y) * nz + Z;
-      a.uout[g] = jacobi_point(S, sy, sz, ((lx + 1) * sy + ly + 1) * sz + lz + 1, a.f[g], a.h2, a.omega);
+      // f of the interior point: offset 1 inside the halo-1 box when H == 2, the box itself when H == 1
+      const double fv = (H == 2) ? F[((lx + 1) * fy + ly + 1) * fz + lz + 1] : F[(lx * fy + ly) * fz + lz];
+      a.uout[g] = jacobi_point(S, sy, sz, ((lx + 1) * sy + ly + 1) * sz + lz + 1, fv, a.h2, a.omega);
     }
   }
 }
@@ -157,6 +190,7 @@ size_t smooth_smem_bytes(int bx, int by, int bz, int H, bool prolong) {
   const int rx = bx + 2 * H, ry = by + 2 * H, rz = bz + 2 * H;
   size_t d = (size_t)rx * ry * rz + (H == 2 ? (size_t)(rx - 2) * (ry - 2) * (rz - 2) : 0);
   if (prolong) d += (size_t)(rx / 2 + 2) * (ry / 2 + 2) * (rz / 2 + 2);
+  if (H > 0) d += (size_t)(rx - 2) * (ry - 2) * (rz - 2);
   return d * 8 + (size_t)(rx + ry + rz) * 4 + 16;
 }
 
@@ -168,6 +202,7 @@ struct ResRestArgs {
   const double* u;
   const double* f;
   double* fc;
+  Dec3 decU, decQ, decT;         // u box, residual box, coarse tile
 };
 
 // coarse rhs = R (f - A u): residual on the (2c+1)^3 fine patch around the coarse tile, then (1/4,1/2,1/4)^3
@@ -191,25 +226,30 @@ __global__ void __launch_bounds__(MG_THREADS) mg_resid_restrict_kernel(const Res
   for (int i = tid; i < uy; i += MG_THREADS) ys[i] = wrapi(2 * C0y - 2 + i, ny);
   for (int i = tid; i < uz; i += MG_THREADS) zs[i] = wrapi(2 * C0z - 2 + i, nz);
   __syncthreads();
+  const Dec3 decU = a.decU, decQ = a.decQ, decT = a.decT;
   for (int i = tid; i < ux * uy * uz; i += MG_THREADS) {
     int lx, ly, lz;
-    decode3(i, uy, uz, lx, ly, lz);
+    decU(i, lx, ly, lz);
     U[i] = a.u[((long long)xs[lx] * ny + ys[ly]) * nz + zs[lz]];
+  }
+  for (int i = tid; i < qx * qy * qz; i += MG_THREADS) {      // f on the residual box, same round trip
+    int lx, ly, lz;
+    decQ(i, lx, ly, lz);
+    R[i] = a.f[((long long)xs[lx + 1] * ny + ys[ly + 1]) * nz + zs[lz + 1]];
   }
   __syncthreads();
   for (int i = tid; i < qx * qy * qz; i += MG_THREADS) {
     int lx, ly, lz;
-    decode3(i, qy, qz, lx, ly, lz);
+    decQ(i, lx, ly, lz);
     const int o = ((lx + 1) * uy + ly + 1) * uz + lz + 1, px = uy * uz;
     const double nb = U[o - px] + U[o + px] + U[o - uz] + U[o + uz] + U[o - 1] + U[o + 1];
-    const double fv = a.f[((long long)xs[lx + 1] * ny + ys[ly + 1]) * nz + zs[lz + 1]];
-    R[i] = fv - (6.0 * U[o] - nb) * a.inv_h2;
+    R[i] = R[i] - (6.0 * U[o] - nb) * a.inv_h2;
   }
   __syncthreads();
   const int ncx = a.gc.nx, ncy = a.gc.ny, ncz = a.gc.nz;
   for (int i = tid; i < a.cbx * a.cby * a.cbz; i += MG_THREADS) {
     int I, J, K;
-    decode3(i, a.cby, a.cbz, I, J, K);
+    decT(i, I, J, K);
     if (C0x + I >= ncx || C0y + J >= ncy || C0z + K >= ncz) continue;
     double s = 0.0;
 #pragma unroll
@@ -252,10 +292,15 @@ struct ClusterArgs {
   const double* sums;
 };
 
-struct ClusterCtx {
-  cg::cluster_group cl;
+// Phase barrier of the coarse kernel.  SMEM: one CTA, every array in shared memory, __syncthreads.
+// !SMEM: a cluster of CL_SIZE CTAs on arrays in global memory (L2), hardware cluster barrier (flushes L1).
+template <bool SMEM>
+struct CoarseCtx {
   int gtid, gthreads;
-  __device__ __forceinline__ void sync() { __threadfence(); cl.sync(); }
+  __device__ __forceinline__ void sync() {
+    if (SMEM) __syncthreads();
+    else { __threadfence(); cg::this_cluster().sync(); }
+  }
 };
 
 __device__ __forceinline__ double nb_sum_g(const double* u, const GridDims& gd, int ix, int iy, int iz) {
@@ -268,36 +313,39 @@ __device__ __forceinline__ double nb_sum_g(const double* u, const GridDims& gd, 
          u[pl + row + zm] + u[pl + row + zp];
 }
 
-__device__ void cl_jacobi(ClusterCtx& c, const MgLevel& L, const double* in, double* out, double omega) {
+template <class Ctx>
+__device__ void cl_jacobi(Ctx& c, const MgLevel& L, const Dec3& dec, const double* in, double* out, double omega) {
   const int n = (int)L.n;
   const double h2 = L.h * L.h;
   for (int r = c.gtid; r < n; r += c.gthreads) {
     if (!in) { out[r] = (1.0 - omega) * 0.0 + (omega / 6.0) * (h2 * L.f[r] + 0.0); continue; }
     int ix, iy, iz;
-    decode3(r, L.gd.ny, L.gd.nz, ix, iy, iz);
+    dec(r, ix, iy, iz);
     out[r] = (1.0 - omega) * in[r] + (omega / 6.0) * (h2 * L.f[r] + nb_sum_g(in, L.gd, ix, iy, iz));
   }
   c.sync();
 }
 
-__device__ void cl_residual(ClusterCtx& c, const MgLevel& L, const double* u) {
+template <class Ctx>
+__device__ void cl_residual(Ctx& c, const MgLevel& L, const Dec3& dec, const double* u) {
   const int n = (int)L.n;
   const double inv_h2 = 1.0 / (L.h * L.h);
   for (int r = c.gtid; r < n; r += c.gthreads) {
     int ix, iy, iz;
-    decode3(r, L.gd.ny, L.gd.nz, ix, iy, iz);
+    dec(r, ix, iy, iz);
     L.r[r] = L.f[r] - (6.0 * u[r] - nb_sum_g(u, L.gd, ix, iy, iz)) * inv_h2;
   }
   c.sync();
 }
 
-__device__ void cl_restrict(ClusterCtx& c, const MgLevel& F, const MgLevel& Cc) {
+template <class Ctx>
+__device__ void cl_restrict(Ctx& c, const MgLevel& F, const MgLevel& Cc, const Dec3& dec) {
   const int nc = (int)Cc.n;
-  const GridDims gf = F.gd, gc = Cc.gd;
+  const GridDims gf = F.gd;
   const int nyz = gf.ny * gf.nz;
   for (int r = c.gtid; r < nc; r += c.gthreads) {
     int I, J, K;
-    decode3(r, gc.ny, gc.nz, I, J, K);
+    dec(r, I, J, K);
     double s = 0.0;
 #pragma unroll
     for (int a = -1; a <= 1; ++a) {
@@ -320,13 +368,15 @@ __device__ void cl_restrict(ClusterCtx& c, const MgLevel& F, const MgLevel& Cc) 
   c.sync();
 }
 
-__device__ void cl_prolong_add(ClusterCtx& c, const MgLevel& Cc, const double* ec, const MgLevel& F, double* u) {
+template <class Ctx>
+__device__ void cl_prolong_add(Ctx& c, const MgLevel& Cc, const double* ec, const MgLevel& F, const Dec3& dec,
+                               double* u) {
   const int nf = (int)F.n;
-  const GridDims gf = F.gd, gc = Cc.gd;
+  const GridDims gc = Cc.gd;
   const int nyz = gc.ny * gc.nz;
   for (int r = c.gtid; r < nf; r += c.gthreads) {
     int ix, iy, iz;
-    decode3(r, gf.ny, gf.nz, ix, iy, iz);
+    dec(r, ix, iy, iz);
     const int I0 = ix >> 1, J0 = iy >> 1, K0 = iz >> 1;
     const int I1 = (ix & 1) ? (I0 + 1 == gc.nx ? 0 : I0 + 1) : I0;
     const int J1 = (iy & 1) ? (J0 + 1 == gc.ny ? 0 : J0 + 1) : J0;
@@ -345,28 +395,33 @@ __device__ void cl_prolong_add(ClusterCtx& c, const MgLevel& Cc, const double* e
 // Exact solve on the coarsest level in the zero-mean subspace: u = (Qx x Qy x Qz) L^+ (Qx x Qy x Qz)^T f with the
 // real orthonormal eigenvectors of the periodic 1-D operator (columns of Q) and eigenvalues lx + ly + lz.
 // Six axis passes through the scratch arrays L.r and L.tmp.
-__device__ void cl_coarse_solve(ClusterCtx& c, const MgLevel& L, const ClusterArgs& a, double* u) {
+template <class Ctx>
+__device__ void cl_coarse_solve(Ctx& c, const MgLevel& L, const Dec3& dec, const ClusterArgs& a, double* u) {
   const int nx = L.gd.nx, ny = L.gd.ny, nz = L.gd.nz;
   const int n = nx * ny * nz;
   const double* f = L.f;
   double* s0 = L.r;
   double* s1 = L.tmp;
   for (int o = c.gtid; o < n; o += c.gthreads) {                    // x: f -> s0, contract with Q^T
-    const int q = o / (ny * nz), rest = o % (ny * nz);
+    int q, b_, k_;
+    dec(o, q, b_, k_);
+    const int rest = o - q * ny * nz;
     double s = 0.0;
     for (int i = 0; i < nx; ++i) s += a.Qx[i * nx + q] * f[i * ny * nz + rest];
     s0[o] = s;
   }
   c.sync();
   for (int o = c.gtid; o < n; o += c.gthreads) {                    // y: s0 -> s1
-    const int q = o / (ny * nz), b = (o / nz) % ny, k = o % nz;
+    int q, b, k;
+    dec(o, q, b, k);
     double s = 0.0;
     for (int j = 0; j < ny; ++j) s += a.Qy[j * ny + b] * s0[(q * ny + j) * nz + k];
     s1[o] = s;
   }
   c.sync();
   for (int o = c.gtid; o < n; o += c.gthreads) {                    // z and the division: s1 -> s0
-    const int q = o / (ny * nz), b = (o / nz) % ny, cc = o % nz;
+    int q, b, cc;
+    dec(o, q, b, cc);
     double s = 0.0;
     for (int k = 0; k < nz; ++k) s += a.Qz[k * nz + cc] * s1[(q * ny + b) * nz + k];
     const double lam = a.lx[q] + a.ly[b] + a.lz[cc];
@@ -374,21 +429,25 @@ __device__ void cl_coarse_solve(ClusterCtx& c, const MgLevel& L, const ClusterAr
   }
   c.sync();
   for (int o = c.gtid; o < n; o += c.gthreads) {                    // back, z: s0 -> s1, contract with Q
-    const int q = o / (ny * nz), b = (o / nz) % ny, k = o % nz;
+    int q, b, k;
+    dec(o, q, b, k);
     double s = 0.0;
     for (int cc = 0; cc < nz; ++cc) s += a.Qz[k * nz + cc] * s0[(q * ny + b) * nz + cc];
     s1[o] = s;
   }
   c.sync();
   for (int o = c.gtid; o < n; o += c.gthreads) {                    // y: s1 -> s0
-    const int q = o / (ny * nz), j = (o / nz) % ny, k = o % nz;
+    int q, j, k;
+    dec(o, q, j, k);
     double s = 0.0;
     for (int b = 0; b < ny; ++b) s += a.Qy[j * ny + b] * s1[(q * ny + b) * nz + k];
     s0[o] = s;
   }
   c.sync();
   for (int o = c.gtid; o < n; o += c.gthreads) {                    // x: s0 -> u
-    const int i = o / (ny * nz), rest = o % (ny * nz);
+    int i, b_, k_;
+    dec(o, i, b_, k_);
+    const int rest = o - i * ny * nz;
     double s = 0.0;
     for (int q = 0; q < nx; ++q) s += a.Qx[i * nx + q] * s0[q * ny * nz + rest];
     u[o] = s;
@@ -396,36 +455,63 @@ __device__ void cl_coarse_solve(ClusterCtx& c, const MgLevel& L, const ClusterAr
   c.sync();
 }
 
-__global__ void __cluster_dims__(CL_SIZE, 1, 1) __launch_bounds__(CL_THREADS)
-mg_cluster_kernel(const __grid_constant__ ClusterArgs a) {
-  ClusterCtx c{cg::this_cluster(), 0, 0};
-  c.gtid = (int)c.cl.block_rank() * CL_THREADS + threadIdx.x;
-  c.gthreads = CL_SIZE * CL_THREADS;
+// Shared-memory footprint of levels l0.. of a hierarchy (u, tmp, f, r per level)
+__host__ __device__ inline size_t coarse_smem_doubles(const MgLevel* lv, int nlev) {
+  size_t d = 0;
+  for (int l = 0; l < nlev; ++l) d += 4 * (size_t)lv[l].n;
+  return d;
+}
+
+template <bool SMEM>
+__global__ void __launch_bounds__(CL_THREADS) mg_coarse_kernel(const __grid_constant__ ClusterArgs a) {
+  extern __shared__ __align__(16) double sm[];
+  __shared__ MgLevel slv[MG_MAX_LEVELS];
+  __shared__ Dec3 sdec[MG_MAX_LEVELS];
+  CoarseCtx<SMEM> c{(int)threadIdx.x, CL_THREADS};
+  if (!SMEM) {
+    c.gtid = (int)cg::this_cluster().block_rank() * CL_THREADS + threadIdx.x;
+    c.gthreads = CL_SIZE * CL_THREADS;
+  }
   const int last = a.nlev - 1;
+  if (threadIdx.x == 0) {
+    double* p = sm;
+    for (int l = 0; l < a.nlev; ++l) {
+      MgLevel L = a.lv[l];
+      if (SMEM) { L.u = p; L.tmp = p + L.n; L.f = p + 2 * L.n; L.r = p + 3 * L.n; p += 4 * L.n; }
+      slv[l] = L;
+    }
+  }
+  if ((int)threadIdx.x < a.nlev) sdec[threadIdx.x] = Dec3::make(a.lv[threadIdx.x].gd.ny, a.lv[threadIdx.x].gd.nz);
+  __syncthreads();
+  const MgLevel& G0 = a.lv[0];          // level 0 in global memory (input / output of the SMEM variant)
 
   if (a.do_rhs) {
-    const MgLevel& L = a.lv[0];
+    const MgLevel& L = slv[0];
     const int n = (int)L.n;
     const double mean = a.sums[4] / (double)n;
     for (int r = c.gtid; r < n; r += c.gthreads) {
       const double d = a.rho0 ? a.rho[r] - a.rho0[r] : a.rho[r];
       L.f[r] = 4.0 * 3.14159265358979323846 * (d - mean);
     }
-    c.sync();
+  } else if (SMEM) {
+    for (int r = c.gtid; r < (int)G0.n; r += c.gthreads) slv[0].f[r] = G0.f[r];
   }
+  if (SMEM && !a.zero_guess)
+    for (int r = c.gtid; r < (int)G0.n; r += c.gthreads) slv[0].u[r] = G0.u[r];
+  c.sync();
 
   // where each level's current solution lives (u or tmp); sweeps ping-pong between the two
   double* cur[MG_MAX_LEVELS];
-  for (int l = 0; l < a.nlev; ++l) cur[l] = a.lv[l].u;
+  for (int l = 0; l < a.nlev; ++l) cur[l] = slv[l].u;
 
   for (int cyc = 0; cyc < a.ncycles; ++cyc) {
     for (int l = 0; l < last; ++l) {
-      const MgLevel& L = a.lv[l];
+      const MgLevel& L = slv[l];
       bool zero = (l > 0) || (a.zero_guess && cyc == 0);
       for (int s = 0; s < a.nu1; ++s) {
         // zero guess: nothing is read, so start in the buffer from which the remaining sweeps end in u
         double* out = zero ? (((a.nu1 - 1 + a.nu2) & 1) ? L.tmp : L.u) : (cur[l] == L.u ? L.tmp : L.u);
-        cl_jacobi(c, L, zero ? nullptr : cur[l], out, a.omega);
+        cl_jacobi(c, L, sdec[l], zero ? nullptr : cur[l], out, a.omega);
         cur[l] = out;
         zero = false;
       }
@@ -434,25 +520,23 @@ mg_cluster_kernel(const __grid_constant__ ClusterArgs a) {
         cur[l] = L.u;
         c.sync();
       }
-      cl_residual(c, L, cur[l]);
-      cl_restrict(c, L, a.lv[l + 1]);
+      cl_residual(c, L, sdec[l], cur[l]);
+      cl_restrict(c, L, slv[l + 1], sdec[l + 1]);
     }
-    cl_coarse_solve(c, a.lv[last], a, a.lv[last].u);
-    cur[last] = a.lv[last].u;
+    cl_coarse_solve(c, slv[last], sdec[last], a, slv[last].u);
+    cur[last] = slv[last].u;
     for (int l = last - 1; l >= 0; --l) {
-      const MgLevel& L = a.lv[l];
-      cl_prolong_add(c, a.lv[l + 1], cur[l + 1], L, cur[l]);
+      const MgLevel& L = slv[l];
+      cl_prolong_add(c, slv[l + 1], cur[l + 1], L, sdec[l], cur[l]);
       for (int s = 0; s < a.nu2; ++s) {
         double* out = cur[l] == L.u ? L.tmp : L.u;
-        cl_jacobi(c, L, cur[l], out, a.omega);
+        cl_jacobi(c, L, sdec[l], cur[l], out, a.omega);
         cur[l] = out;
       }
     }
   }
-  if (cur[0] != a.lv[0].u) {
-    const MgLevel& L = a.lv[0];
-    for (int r = c.gtid; r < (int)L.n; r += c.gthreads) L.u[r] = cur[0][r];
-  }
+  if (SMEM || cur[0] != G0.u)
+    for (int r = c.gtid; r < (int)G0.n; r += c.gthreads) G0.u[r] = cur[0][r];
 }
 
 }  // namespace
@@ -466,7 +550,16 @@ int tile_edge(int n, int bmax) {            // equal tiles of at most bmax point
 }
 
 struct TileGeom { int bx, by, bz, tx, ty, tz; };
+// Largest tile is (mx, my, mz); on small levels the tile is halved (x, y, then z, in turn) until there are at least
+// ~148 CTAs or the tile is down to 256 points: these launches are latency-bound, so more SMs in flight is what counts.
 TileGeom make_geom(const GridDims& g, int mx, int my, int mz) {
+  for (int turn = 0; turn < 12; ++turn) {
+    const long long nt = (long long)((g.nx + mx - 1) / mx) * ((g.ny + my - 1) / my) * ((g.nz + mz - 1) / mz);
+    if (nt >= 148 || mx * my * mz <= 256) break;
+    if (turn % 3 == 0 && mx > 2) mx /= 2;
+    else if (turn % 3 == 1 && my > 2) my /= 2;
+    else if (turn % 3 == 2 && mz > 8) mz /= 2;
+  }
   TileGeom t;
   t.bx = tile_edge(g.nx, mx); t.by = tile_edge(g.ny, my); t.bz = tile_edge(g.nz, mz);
   t.tx = (g.nx + t.bx - 1) / t.bx; t.ty = (g.ny + t.by - 1) / t.by; t.tz = (g.nz + t.bz - 1) / t.bz;
@@ -483,6 +576,13 @@ void launch_smooth(const MgLevel& L, const MgLevel* coarse, const double* ec, co
   a.bx = t.bx; a.by = t.by; a.bz = t.bz; a.tx = t.tx; a.ty = t.ty; a.tz = t.tz;
   a.nsweep = nsweep; a.h2 = L.h * L.h; a.omega = omega;
   a.uin = uin; a.f = L.f; a.ec = ec; a.uout = uout;
+  {
+    const int H = nsweep, ry = t.by + 2 * H, rz = t.bz + 2 * H;
+    a.decA = Dec3::make(ry, rz);
+    a.decB = Dec3::make(ry > 2 ? ry - 2 : 1, rz > 2 ? rz - 2 : 1);
+    a.decC = Dec3::make(ry / 2 + 2, rz / 2 + 2);
+    a.decI = Dec3::make(t.by, t.bz);
+  }
   const unsigned grid = (unsigned)(t.tx * t.ty * t.tz);
   const size_t smem = smooth_smem_bytes(t.bx, t.by, t.bz, nsweep, ec != nullptr);
   if (ec) mg_smooth_kernel<true><<<grid, MG_THREADS, smem, st>>>(a);
@@ -496,17 +596,37 @@ void launch_resid_restrict(const MgLevel& F, const MgLevel& C, const double* u, 
   a.cbx = t.bx; a.cby = t.by; a.cbz = t.bz; a.tx = t.tx; a.ty = t.ty; a.tz = t.tz;
   a.inv_h2 = 1.0 / (F.h * F.h);
   a.u = u; a.f = F.f; a.fc = C.f;
+  a.decU = Dec3::make(2 * t.by + 3, 2 * t.bz + 3);
+  a.decQ = Dec3::make(2 * t.by + 1, 2 * t.bz + 1);
+  a.decT = Dec3::make(t.by, t.bz);
   mg_resid_restrict_kernel<<<(unsigned)(t.tx * t.ty * t.tz), MG_THREADS, resrest_smem_bytes(t.bx, t.by, t.bz), st>>>(a);
 }
 
-void launch_cluster(const MgSolveArgs& s, int l0, int ncycles, int zero_guess, int do_rhs, cudaStream_t st) {
+constexpr size_t COARSE_SMEM_MAX = 200 * 1024;     // bytes of level arrays the single-CTA kernel may hold
+
+bool fits_smem(const MgSolveArgs& s, int l0) {
+  return coarse_smem_doubles(s.lv + l0, s.nlev - l0) * 8 <= COARSE_SMEM_MAX;
+}
+
+// levels l0.. : single CTA on shared memory when they fit, else the 8-CTA cluster on global memory
+void launch_coarse(const MgSolveArgs& s, int l0, int ncycles, int zero_guess, int do_rhs, cudaStream_t st) {
   ClusterArgs a{};
   a.nlev = s.nlev - l0; a.ncycles = ncycles; a.zero_guess = zero_guess;
   a.nu1 = s.nu1; a.nu2 = s.nu2; a.omega = s.omega;
   for (int l = l0; l < s.nlev; ++l) a.lv[l - l0] = s.lv[l];
   a.Qx = s.Qx; a.Qy = s.Qy; a.Qz = s.Qz; a.lx = s.lx; a.ly = s.ly; a.lz = s.lz;
   a.do_rhs = do_rhs; a.rho = s.rho; a.rho0 = s.rho0; a.sums = s.sums;
-  mg_cluster_kernel<<<CL_SIZE, CL_THREADS, 0, st>>>(a);
+  if (fits_smem(s, l0)) {
+    mg_coarse_kernel<true><<<1, CL_THREADS, coarse_smem_doubles(a.lv, a.nlev) * 8, st>>>(a);
+  } else {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(CL_SIZE); cfg.blockDim = dim3(CL_THREADS); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CL_SIZE; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, mg_coarse_kernel<false>, a);
+  }
 }
 
 struct BigCycle {
@@ -536,7 +656,7 @@ struct BigCycle {
     launch_resid_restrict(L, s.lv[l + 1], cur[l], st);
     ++launches;
     if (l + 1 == lc) {
-      launch_cluster(s, lc, 1, 1, 0, st);
+      launch_coarse(s, lc, 1, 1, 0, st);
       ++launches;
       cur[l + 1] = s.lv[l + 1].u;
     } else {
@@ -559,14 +679,18 @@ int init_mg_kernels() {
     e = cudaFuncSetAttribute(mg_smooth_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(mg_resid_restrict_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(mg_coarse_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)COARSE_SMEM_MAX);
   return (int)e;
 }
 
 int launch_mg_solve(const MgSolveArgs& s, cudaStream_t st) {
+  // lc = first level from which the rest of the hierarchy fits one CTA's shared memory; if even the coarsest level
+  // does not, the levels above it use the tile kernels and the exact solve runs on the cluster
   int lc = 0;
-  while (lc < s.nlev - 1 && s.lv[lc].n > MG_CLUSTER_MAX_PTS) ++lc;
+  while (lc < s.nlev - 1 && !fits_smem(s, lc)) ++lc;
   if (lc == 0) {           // the whole hierarchy is small: rhs + every cycle in one launch
-    launch_cluster(s, 0, s.n_vc, 0, 1, st);
+    launch_coarse(s, 0, s.n_vc, 0, 1, st);
     return 1;
   }
   launch_poisson_rhs(s.lv[0].n, s.rho, s.rho0, s.sums, s.lv[0].f, st);

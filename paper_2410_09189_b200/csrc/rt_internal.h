@@ -125,10 +125,9 @@ struct MgLevel {
   double* u; double* tmp; double* f; double* r;     // solution, ping-pong scratch, rhs, residual
 };
 // One Poisson solve (a7): rhs = 4 pi (rho - rho0 - sums[4]/n), then n_vc V(nu1,nu2) cycles on lv[0].u (warm start).
-// Levels with at most MG_CLUSTER_MAX_PTS points run inside one thread-block-cluster kernel per cycle; larger levels
-// use shared-memory tile kernels (mg_kernels.cu).  Returns the number of kernels enqueued.
+// The coarse end of the hierarchy runs inside one single-CTA shared-memory kernel per cycle; larger levels use
+// shared-memory tile kernels (mg_kernels.cu).  Returns the number of kernels enqueued.
 constexpr int MG_MAX_LEVELS = 12;
-constexpr long long MG_CLUSTER_MAX_PTS = 32768;
 struct MgSolveArgs {
   const MgLevel* lv; int nlev;
   int n_vc, nu1, nu2; double omega;

@@ -1,4 +1,4 @@
-"""GPU parity of the a7 Poisson solve (tile kernels + thread-block-cluster kernel, mg_kernels.cu) against the oracle's
+"""GPU parity of the a7 Poisson solve (tile kernels + single-CTA / cluster coarse kernel, mg_kernels.cu) against the oracle's
 V-cycle (oracle/rt_oracle.py hartree_mg, DESIGN R6) on grids chosen to hit every path: one / two levels on the
 shared-memory tile kernels with ragged tiles, hierarchies that live entirely in the cluster kernel, a grid that cannot
 be coarsened at all (exact solve only), and sweep counts other than V(2,2)."""
@@ -36,8 +36,11 @@ GRIDS = [
     ((40, 36, 72), "one tile level (ragged y tiles), coarsest 10x9x18"),
     ((96, 48, 64), "two tile levels, cluster below"),
     ((104, 52, 26), "24k-like factors: 104 -> 52 -> 26 -> 13 in x"),
-    ((32, 32, 32), "exactly the cluster limit"),
-    ((20, 12, 28), "all in the cluster kernel"),
+    ((32, 32, 32), "one tile level, 16^3 and below in the single-CTA shared-memory kernel"),
+    ((20, 12, 28), "one tile level (6720 points do not fit shared memory with their coarse levels)"),
+    ((16, 12, 20), "whole hierarchy (rhs + all cycles) in ONE single-CTA launch"),
+    ((27, 20, 16), "cannot be coarsened and too large for shared memory: cluster kernel on global memory"),
+    ((54, 40, 32), "tile level above a coarsest level that needs the cluster kernel"),
     ((9, 5, 7), "no coarsening: exact solve only"),
     ((6, 6, 66), "thin grid: tile halo wraps onto the tile itself"),
 ]
@@ -61,7 +64,7 @@ def test_vcycles_match_oracle(B, shape, why):
 
 
 @pytest.mark.parametrize("nu", [(1, 1), (3, 2), (0, 2), (2, 0), (1, 4)])
-@pytest.mark.parametrize("shape", [(40, 36, 72), (20, 12, 28)])
+@pytest.mark.parametrize("shape", [(40, 36, 72), (16, 12, 20), (54, 40, 32)])
 def test_sweep_counts(B, shape, nu):
     h = 0.35
     Phi, eps, occ = tiny_system(shape, h)
