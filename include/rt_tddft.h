@@ -83,6 +83,10 @@ typedef struct {
                                12-13, 24-26; L483) instead of n_hupdates times.  rt_step then synchronises the
                                host once per update (it reads the 8-byte error norm)                           */
   int32_t  max_hupdates;    /* bound on the updates per step when H_thrs > 0; 0 -> 20                          */
+  /* -- grid-slab sharding (the paper's own decomposition): this handle owns the x-planes
+   *    [slab_x0, slab_x0 + slab_nx) of the nx*ny*nz grid and `phi` holds only those: [norb][slab_nx*ny*nz].
+   *    slab_nx = 0: the whole grid (single GPU; every entry point above).  slab_nx > 0: see rt_slab_* below.   */
+  int32_t  slab_x0, slab_nx;
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
@@ -147,6 +151,36 @@ int rt_op_propagate(rt_handle h, const double* Hbar, const double* P0re, const d
 int rt_op_hartree(rt_handle h, double* vh, const double* drho, int32_t n_vc);
 /* a8 "exchange/correlation": vxc[Ng] = Slater + PZ81 potential of rho[Ng] (EITHER). */
 int rt_op_vxc(rt_handle h, const double* rho, double* vxc);
+
+/* ---- grid-slab sharding: one handle per rank, phases separated by the two exchanges of the method --------
+ * The grid contractions are local to a slab (a5: rho on the slab; a1: a partial sum of dH over the slab, L424);
+ * the N x N propagator (a2-a4) and the O(Ng) Poisson / xc stages (a7, a8) are replicated on every rank.  Between the
+ * phases the CALLER combines two library-owned device buffers across ranks with a SUM all-reduce (NCCL through
+ * torch.distributed in paper_2410_09189_b200/slab.py):
+ *   xchg_rho [Ng + 8]    : rho on the full grid (each rank writes its slab, zeros elsewhere) followed by the five
+ *                          partial sums { sum rho, sum x rho, sum y rho, sum z rho, sum (rho - rho0) } + 3 pad
+ *   xchg_H   [norb*ldn]  : partial H1 = dVol Phi_slab diag(dV) Phi_slab^T (+ diag(eps) on the rank with slab_x0 = 0)
+ * A handle created with slab_nx > 0 accepts rt_slab_*, the getters and rt_set_field; rt_step and rt_op_* return
+ * RT_ESTATE.  Sequence (every rank, same order):
+ *   rt_create                      -> local rho0 slab in xchg_rho, partial H(t=0) in xchg_H
+ *   [all-reduce xchg_rho, xchg_H]     rt_slab_phase(h, RT_SLAB_INIT, 0)
+ *   per time step, for it = 0 .. m-1:
+ *     rt_slab_phase(h, RT_SLAB_PROPAGATE, it)  (a2-a5, a6 partial)   [all-reduce xchg_rho]
+ *     rt_slab_phase(h, RT_SLAB_POTENTIAL, it)  (a7, a8, a1 partial)  [all-reduce xchg_H]
+ *   rt_slab_phase(h, RT_SLAB_SHIFT, 0)         (Alg. 1 line 28)
+ * Phases enqueue on the handle's stream and do not synchronise; the collectives must run on the same stream (or be
+ * ordered after it). */
+#define RT_SLAB_INIT      0
+#define RT_SLAB_PROPAGATE 1
+#define RT_SLAB_POTENTIAL 2
+#define RT_SLAB_SHIFT     3
+typedef struct {
+  double* xchg_rho;  int64_t xchg_rho_count;   /* DEVICE, Ng + 8 doubles                          */
+  double* xchg_H;    int64_t xchg_H_count;     /* DEVICE, norb * ldn doubles (ldn = norb rounded up to 8) */
+  int64_t slab_offset, slab_count;             /* this rank's range of grid points inside xchg_rho */
+} rt_slab_buffers;
+int rt_slab_get_buffers(rt_handle h, rt_slab_buffers* out);
+int rt_slab_phase(rt_handle h, int32_t phase, int32_t it);
 
 /* ---- per-stage timing (CUDA events on the launching stream) ------------------------------------
  * Stage ids follow Table 1 (L543-L547) plus the rest of the step. */

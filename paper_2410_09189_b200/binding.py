@@ -27,7 +27,10 @@ SYMBOLS = (
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
+    "rt_slab_get_buffers", "rt_slab_phase",
 )
+
+RT_SLAB_INIT, RT_SLAB_PROPAGATE, RT_SLAB_POTENTIAL, RT_SLAB_SHIFT = 0, 1, 2, 3
 
 
 class rt_config(C.Structure):
@@ -47,7 +50,13 @@ class rt_config(C.Structure):
         ("propagator", C.c_int32), ("max_order", C.c_int32),
         ("dP_thrs", C.c_double), ("H_thrs", C.c_double),
         ("max_hupdates", C.c_int32),
+        ("slab_x0", C.c_int32), ("slab_nx", C.c_int32),
     ]
+
+
+class rt_slab_buffers(C.Structure):
+    _fields_ = [("xchg_rho", C.c_void_p), ("xchg_rho_count", C.c_int64), ("xchg_H", C.c_void_p),
+                ("xchg_H_count", C.c_int64), ("slab_offset", C.c_int64), ("slab_count", C.c_int64)]
 
 
 class RTError(RuntimeError):
@@ -71,6 +80,7 @@ def _load():
         "rt_destroy": [vp], "rt_op_project": [vp, dp, dp], "rt_op_density": [vp, dp, dp, dp],
         "rt_op_propagate": [vp, dp, dp, dp, dp, dp], "rt_op_hartree": [vp, dp, dp, i32], "rt_op_vxc": [vp, dp, dp],
         "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp], "rt_get_convergence": [vp, dp, dp],
+        "rt_slab_get_buffers": [vp, C.POINTER(rt_slab_buffers)], "rt_slab_phase": [vp, i32, i32],
     }
     for name, argtypes in sig.items():
         fn = getattr(lib, name)
@@ -237,6 +247,16 @@ def rt_probe_fp64_peak(device=0):
     return a.value, b.value
 
 
+def rt_slab_get_buffers(h) -> rt_slab_buffers:
+    b = rt_slab_buffers()
+    _check(h, _lib.rt_slab_get_buffers(h, C.byref(b)))
+    return b
+
+
+def rt_slab_phase(h, phase: int, it: int = 0):
+    _check(h, _lib.rt_slab_phase(h, int(phase), int(it)))
+
+
 # ---- convenience wrapper (the call a user makes) -------------------------------------------------------
 
 class RTTDDFT:
@@ -244,8 +264,12 @@ class RTTDDFT:
 
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
                  nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
-                 device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0):
+                 device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0,
+                 slab=None):
+        """``slab = (x0, nx_local)``: the handle owns those x-planes and ``phi`` is [norb][nx_local*ny*nz]
+        (rt_slab_* entry points; see slab.py)."""
         cfg = rt_config()
+        cfg.slab_x0, cfg.slab_nx = (int(slab[0]), int(slab[1])) if slab else (0, 0)
         cfg.propagator = {"taylor": RT_PROP_TAYLOR, "commutator": RT_PROP_COMMUTATOR}[propagator]
         cfg.max_order, cfg.dP_thrs, cfg.H_thrs, cfg.max_hupdates = int(max_order), float(dP_thrs), float(H_thrs), int(max_hupdates)
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)

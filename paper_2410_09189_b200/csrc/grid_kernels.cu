@@ -46,7 +46,7 @@ int reduce_rho_blocks(long long Ng) {
 }
 
 __global__ void __launch_bounds__(RB)
-reduce_rho_kernel(const double* __restrict__ part, int nparts, long long Ng, GridDims gd, double h,
+reduce_rho_kernel(const double* __restrict__ part, int nparts, long long Ng, GridDims gd, double h, int x0,
                   const double* __restrict__ rho0, double* __restrict__ rho, double* __restrict__ bsums) {
   __shared__ double sh[RB / 32][5];
   double v[5] = {0, 0, 0, 0, 0};
@@ -56,9 +56,10 @@ reduce_rho_kernel(const double* __restrict__ part, int nparts, long long Ng, Gri
     double s = 0.0;
     for (int p = 0; p < nparts; ++p) s += part[(long long)p * Ng + r];
     rho[r] = s;
-    const int ix = (int)(r / nyz);
-    const int rem = (int)(r - (long long)ix * nyz);
+    const int ixl = (int)(r / nyz);                  // plane inside the slab; x0 = first plane of the slab
+    const int rem = (int)(r - (long long)ixl * nyz);
     const int iy = rem / gd.nz, iz = rem - iy * gd.nz;
+    const int ix = ixl + x0;
     v[0] += s;
     v[1] += ((double)ix - cx) * h * s;
     v[2] += ((double)iy - cy) * h * s;
@@ -81,10 +82,10 @@ __global__ void final_sums_kernel(const double* __restrict__ bsums, int nb, int 
   if (lane == 0) sums[q] = s;
 }
 
-void launch_reduce_rho(const double* rho_part, int nparts, long long Ng, GridDims gd, double h, const double* rho0,
-                       double* rho, double* bsums, double* sums, cudaStream_t st) {
+void launch_reduce_rho(const double* rho_part, int nparts, long long Ng, GridDims gd, double h, int x0,
+                       const double* rho0, double* rho, double* bsums, double* sums, cudaStream_t st) {
   const int nb = reduce_rho_blocks(Ng);
-  reduce_rho_kernel<<<nb, RB, 0, st>>>(rho_part, nparts, Ng, gd, h, rho0, rho, bsums);
+  reduce_rho_kernel<<<nb, RB, 0, st>>>(rho_part, nparts, Ng, gd, h, x0, rho0, rho, bsums);
   final_sums_kernel<<<1, 32 * 5, 0, st>>>(bsums, nb, 5, sums);
 }
 

@@ -24,7 +24,12 @@ struct EventPair { cudaEvent_t a, b; int stage; };
 struct rt_ctx {
   rt_config cfg{};
   int N = 0, ldn = 0;
-  long long Ng = 0;
+  long long Ng = 0;              // points of the whole grid
+  long long Ngl = 0;             // points this handle's Phi covers (= Ng unless the handle is a grid slab)
+  long long slab_off = 0;        // first grid point of the slab
+  int x0 = 0;                    // first x-plane of the slab
+  bool slab = false;
+  int slab_state = 0;            // 0: waiting for RT_SLAB_INIT, 1: ready
   GridDims gd{};
   double h = 0, dvol = 0, dt = 0, sigma = 0, omega = 0;
   int m = 2, n_vc = 0, nu1 = 2, nu2 = 2, q = 0;           // q: cos/sinc polynomial degree in Y = X^2
@@ -335,7 +340,8 @@ void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double
   if (c->use_tma)
     launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phiN_3d, c->phi, c->d_segs, c->rho_part, c->sms, c->st);
   else launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
-  launch_reduce_rho(c->rho_part, c->use_tma ? c->dp.ntypes : c->dp.npairs, c->Ng, c->gd, c->h, rho0, rho_out, c->d_bsums, c->d_sums, c->st);
+  launch_reduce_rho(c->rho_part, c->use_tma ? c->dp.ntypes : c->dp.npairs, c->Ngl, c->gd, c->h, c->x0, rho0, rho_out,
+                    c->d_bsums, c->d_sums, c->st);
   c->launches += 4;
 }
 
@@ -353,8 +359,18 @@ void enqueue_project(rt_ctx* c, const double* w, const double* eps, double* H) {
   c->launches += 2;
 }
 
-// One Hamiltonian update, Algorithm 1 lines 14-25 (`it` = 0 also extrapolates H1, line 11).
-void enqueue_update(rt_ctx* c, int it) {
+// H = diag(eps) + dVol Phi diag(w) Phi^T with w = c->w (whole grid).  A slab handle contracts over its own grid
+// points only (the partial sum of PAPER.md:L424; the slab of w is first copied to the 16-byte aligned op_u) and only
+// the rank that owns plane 0 adds diag(eps), so that the all-reduce of the partial matrices gives H.
+void enqueue_project_dv(rt_ctx* c, double* H) {
+  if (!c->slab) { enqueue_project(c, c->w, c->d_eps, H); return; }
+  cudaMemcpyAsync(c->op_u, c->w + c->slab_off, (size_t)c->Ngl * 8, cudaMemcpyDeviceToDevice, c->st);
+  enqueue_project(c, c->op_u, c->x0 == 0 ? c->d_eps : nullptr, H);
+}
+
+// First half of a Hamiltonian update, Algorithm 1 lines 14-23 + Eq. 27 (`it` = 0 also extrapolates H1, line 11):
+// mean Hamiltonian, propagation, density of this handle's grid points (+ partial dipole / charge sums).
+void enqueue_update_propagate(rt_ctx* c, int it) {
   stage_begin(c, RT_STAGE_ELDYN);
   if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);                          // lines 12, 16
   launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st);     // lines 11, 14
@@ -363,9 +379,14 @@ void enqueue_update(rt_ctx* c, int it) {
   stage_end(c);
 
   stage_begin(c, RT_STAGE_RHO);
-  enqueue_density(c, c->P1r, c->rho, c->rho0);                                                 // Eq. 27 + line 27
+  if (c->slab) cudaMemsetAsync(c->rho, 0, (size_t)(c->Ng + 8) * 8, c->st);                     // other ranks' slabs
+  enqueue_density(c, c->P1r, c->rho + c->slab_off, c->rho0 + c->slab_off);                     // Eq. 27 + line 27
   stage_end(c);
+}
 
+// Second half, lines 24-25: potential update on the whole grid from the (complete) density, then the projection
+// over this handle's grid points.
+void enqueue_update_potential(rt_ctx* c) {
   if (c->use_h) {
     stage_begin(c, RT_STAGE_VH);
     enqueue_poisson(c, c->lv, c->n_vc, c->rho, c->rho0);
@@ -380,12 +401,17 @@ void enqueue_update(rt_ctx* c, int it) {
   stage_begin(c, RT_STAGE_HUPDATE);
   if (c->dynamic)                                                                              // H1_old <- H1
     cudaMemcpyAsync(c->Ya, c->H1, (size_t)c->N * c->ldn * 8, cudaMemcpyDeviceToDevice, c->st);
-  enqueue_project(c, c->w, c->d_eps, c->H1);                                                   // line 25
+  enqueue_project_dv(c, c->H1);                                                                // line 25
   if (c->dynamic) {
     launch_maxabs_diff(c->N, c->ldn, c->H1, c->Ya, c->d_cs, c->st);                            // line 24
     c->launches += 1;
   }
   stage_end(c);
+}
+
+void enqueue_update(rt_ctx* c, int it) {
+  enqueue_update_propagate(c, it);
+  enqueue_update_potential(c);
 }
 
 void enqueue_shift(rt_ctx* c) {
@@ -464,6 +490,10 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     return fail(c, RT_EINVAL, "rt_create: negative iteration count");
   if (cfg->propagator != RT_PROP_TAYLOR && cfg->propagator != RT_PROP_COMMUTATOR)
     return fail(c, RT_EINVAL, "rt_create: unknown propagator");
+  if (cfg->slab_nx < 0 || cfg->slab_x0 < 0 || (cfg->slab_nx > 0 && cfg->slab_x0 + cfg->slab_nx > cfg->nx))
+    return fail(c, RT_EINVAL, "rt_create: slab [slab_x0, slab_x0 + slab_nx) must lie inside [0, nx)");
+  if (cfg->slab_nx > 0 && cfg->H_thrs > 0.0)
+    return fail(c, RT_EINVAL, "rt_create: the dynamic H_thrs loop is driven by rt_step and is not available on a slab handle");
   if (cfg->max_order < 0 || cfg->max_order > MAX_ORDER || cfg->max_hupdates < 0 || !(cfg->dP_thrs >= 0.0) ||
       !(cfg->H_thrs >= 0.0))
     return fail(c, RT_EINVAL, "rt_create: bad max_order / max_hupdates / dP_thrs / H_thrs");
@@ -486,6 +516,13 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   c->ldn = roundup(c->N, 8);
   c->gd = GridDims{cfg->nx, cfg->ny, cfg->nz};
   c->Ng = (long long)cfg->nx * cfg->ny * cfg->nz;
+  c->Ngl = c->Ng;
+  if (cfg->slab_nx > 0) {
+    c->slab = true;
+    c->x0 = cfg->slab_x0;
+    c->Ngl = (long long)cfg->slab_nx * cfg->ny * cfg->nz;
+    c->slab_off = (long long)cfg->slab_x0 * cfg->ny * cfg->nz;
+  }
   c->h = cfg->h;
   c->dvol = cfg->h * cfg->h * cfg->h;
   c->dt = cfg->dt;
@@ -499,7 +536,8 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   c->use_graph = !(cfg->flags & RT_NO_GRAPH);
   c->st = reinterpret_cast<cudaStream_t>(cfg->stream);
   const int N = c->N, ldn = c->ldn;
-  const long long Ng = c->Ng;
+  const long long Ng = c->Ngl;      // grid points of this handle's Phi: what the plans and Phi descriptors see
+  const long long NgF = c->Ng;      // the whole grid: every O(Ng) array and the Poisson / xc stages
 
 #define FAIL_CREATE(code, msg) do { int rc_ = fail(nullptr, (code), (msg)); rt_destroy(c); return rc_; } while (0)
 #define CKC(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); cudaGetLastError(); FAIL_CREATE(RT_ECUDA, m_); } } while (0)
@@ -598,7 +636,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   {
     size_t freeb = 0, totalb = 0;
     CKC(cudaMemGetInfo(&freeb, &totalb));
-    double need = 15.0 * N * (double)ldn * 8 + (double)c->pp.S * N * ldn * 8 + (double)c->dp.ntypes * Ng * 8 + 12.0 * Ng * 8;
+    double need = 15.0 * N * (double)ldn * 8 + (double)c->pp.S * N * ldn * 8 + (double)c->dp.ntypes * Ng * 8 + 12.0 * NgF * 8;
     if (!(cfg->flags & RT_PHI_DEVICE)) need += (double)N * Ng * 8;
     if (need > (double)freeb) {
       char buf[256];
@@ -636,7 +674,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     if (e != 0) FAIL_CREATE(RT_ECUDA, std::string("init_tma_kernels: ") + cudaGetErrorString((cudaError_t)e));
   }
   const size_t nn = (size_t)N * ldn;
-  ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8); ALLOC(c->d_sums, 8);
+  ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8);
   ALLOC(c->d_bsums, 5 * 1024);
   if (c->prop == RT_PROP_COMMUTATOR || c->dynamic) {
     ALLOC(c->d_cs, 1);
@@ -646,10 +684,13 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
                      &c->P0r, &c->P0i, &c->P1r, &c->P1i};
   for (double** mp : mats) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
   ALLOC(c->W, (size_t)c->pp.S * nn);
-  ALLOC(c->rho, Ng); ALLOC(c->rho0, Ng); ALLOC(c->vxc0, Ng);
-  ALLOC(c->w, Ng + 16); ALLOC(c->op_u, Ng + 16);      // projection weights: the TMA path reads whole 16-double stages
-  CKC(cudaMemsetAsync(c->w, 0, (size_t)(Ng + 16) * 8, c->st));
-  CKC(cudaMemsetAsync(c->op_u, 0, (size_t)(Ng + 16) * 8, c->st));
+  // rho and the five sums share one allocation: it is the first exchange buffer of the slab mode
+  ALLOC(c->rho, NgF + 8); ALLOC(c->rho0, NgF); ALLOC(c->vxc0, NgF);
+  c->d_sums = c->rho + NgF;
+  CKC(cudaMemsetAsync(c->rho, 0, (size_t)(NgF + 8) * 8, c->st));
+  ALLOC(c->w, NgF + 16); ALLOC(c->op_u, NgF + 16);    // projection weights: the TMA path reads whole 16-double stages
+  CKC(cudaMemsetAsync(c->w, 0, (size_t)(NgF + 16) * 8, c->st));
+  CKC(cudaMemsetAsync(c->op_u, 0, (size_t)(NgF + 16) * 8, c->st));
   ALLOC(c->rho_part, (size_t)c->dp.ntypes * Ng);
   ALLOC(c->d_segs, c->segs.size());
   CKC(cudaMemcpyAsync(c->d_segs, c->segs.data(), c->segs.size() * sizeof(DensSeg), cudaMemcpyHostToDevice, c->st));
@@ -688,15 +729,21 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
 
   // initial state (Alg. 1 lines 7-8): P0 = diag(occ); rho0; vxc0; H0 = H-1 = diag(eps) + Proj(E0.r)
   launch_set_diag(N, ldn, c->P0r, c->d_occ, c->st);
-  enqueue_density(c, c->P0r, c->rho0, nullptr);
-  CKC(cudaMemcpyAsync(c->rho, c->rho0, (size_t)Ng * 8, cudaMemcpyDeviceToDevice, c->st));
-  launch_vxc(Ng, c->rho0, c->vxc0, c->st);
-  launch_field(Ng, c->gd, c->h, c->d_E, c->w, c->st);
-  enqueue_project(c, c->w, c->d_eps, c->H0);
-  CKC(cudaMemcpyAsync(c->Hm1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
-  CKC(cudaMemcpyAsync(c->H1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
-  // sums[4] currently holds sum(rho0) (rho0 pointer was NULL): the induced charge at t = 0 is zero
-  CKC(cudaMemsetAsync(c->d_sums + 4, 0, 8, c->st));
+  launch_field(NgF, c->gd, c->h, c->d_E, c->w, c->st);
+  if (!c->slab) {
+    enqueue_density(c, c->P0r, c->rho0, nullptr);
+    CKC(cudaMemcpyAsync(c->rho, c->rho0, (size_t)Ng * 8, cudaMemcpyDeviceToDevice, c->st));
+    launch_vxc(Ng, c->rho0, c->vxc0, c->st);
+    enqueue_project(c, c->w, c->d_eps, c->H0);
+    CKC(cudaMemcpyAsync(c->Hm1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
+    CKC(cudaMemcpyAsync(c->H1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
+    // sums[4] currently holds sum(rho0) (rho0 pointer was NULL): the induced charge at t = 0 is zero
+    CKC(cudaMemsetAsync(c->d_sums + 4, 0, 8, c->st));
+  } else {
+    // slab: the local pieces go to the exchange buffers; RT_SLAB_INIT finishes after the caller's all-reduce
+    enqueue_density(c, c->P0r, c->rho + c->slab_off, nullptr);
+    enqueue_project_dv(c, c->H1);
+  }
   {
     double z8[8] = {0, 0, 0, 0, 0, 0, 0, 0};                  // E(t_1) defaults to 0 (DESIGN R5)
     CKC(cudaMemcpyAsync(c->d_E, z8, sizeof z8, cudaMemcpyHostToDevice, c->st));
@@ -708,7 +755,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   // H_thrs > 0 the number of updates is decided on the host, so the unit captured is one Hamiltonian update.
   {
     const int64_t before = c->launches;
-    if (c->use_graph) {
+    if (c->use_graph && !c->slab) {
       // capture on a private stream (the caller's may be the legacy default stream, which cannot capture);
       // the instantiated graph is replayed on the caller's stream
       cudaStream_t user = c->st, cap = nullptr;
@@ -759,6 +806,7 @@ int rt_set_field(rt_handle c, const double E[3]) {
 
 int rt_step(rt_handle c, int32_t nsteps) {
   CHECK_HANDLE(c);
+  if (c->slab) return fail(c, RT_ESTATE, "rt_step: slab handle -- drive it with rt_slab_phase");
   if (nsteps < 0) return fail(c, RT_EINVAL, "rt_step: nsteps < 0");
   CK(cudaSetDevice(c->cfg.device));
   for (int s = 0; s < nsteps; ++s) {
@@ -907,6 +955,7 @@ int rt_get_launch_count(rt_handle c, int64_t* n) {
 // ---- per-stage entry points ------------------------------------------------------------------------
 int rt_op_project(rt_handle c, const double* v, double* out) {
   CHECK_HANDLE(c);
+  if (c->slab) return fail(c, RT_ESTATE, "rt_op_project: not available on a slab handle");
   if (!v || !out) return fail(c, RT_EINVAL, "rt_op_project: NULL");
   CK(cudaSetDevice(c->cfg.device));
   CK(cudaMemcpyAsync(c->op_u, v, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
@@ -919,6 +968,7 @@ int rt_op_project(rt_handle c, const double* v, double* out) {
 
 int rt_op_density(rt_handle c, const double* reP, double* rho, double sums[5]) {
   CHECK_HANDLE(c);
+  if (c->slab) return fail(c, RT_ESTATE, "rt_op_density: not available on a slab handle");
   if (!reP || !rho) return fail(c, RT_EINVAL, "rt_op_density: NULL");
   CK(cudaSetDevice(c->cfg.device));
   if (int rc = copy_matrix_in(c, reP, c->Ya)) return rc;
@@ -941,6 +991,7 @@ int rt_op_density(rt_handle c, const double* reP, double* rho, double sums[5]) {
 int rt_op_propagate(rt_handle c, const double* Hbar, const double* P0re, const double* P0im, double* P1re,
                     double* P1im) {
   CHECK_HANDLE(c);
+  if (c->slab) return fail(c, RT_ESTATE, "rt_op_propagate: not available on a slab handle");
   if (!Hbar || !P0re || !P0im || !P1re || !P1im) return fail(c, RT_EINVAL, "rt_op_propagate: NULL");
   CK(cudaSetDevice(c->cfg.device));
   // scratch: H1 <- Hbar (as both H0 and H1 of launch_hbar), P1r/P1i <- P0 ; outputs in Hm1-free buffers
@@ -975,6 +1026,7 @@ int rt_op_propagate(rt_handle c, const double* Hbar, const double* P0re, const d
 
 int rt_op_hartree(rt_handle c, double* vh, const double* drho, int32_t n_vc) {
   CHECK_HANDLE(c);
+  if (c->slab) return fail(c, RT_ESTATE, "rt_op_hartree: not available on a slab handle");
   if (!vh || !drho || n_vc < 0) return fail(c, RT_EINVAL, "rt_op_hartree: bad argument");
   if (!c->use_h) return fail(c, RT_EINVAL, "rt_op_hartree: handle created with RT_NO_HARTREE");
   CK(cudaSetDevice(c->cfg.device));
@@ -998,6 +1050,7 @@ int rt_op_hartree(rt_handle c, double* vh, const double* drho, int32_t n_vc) {
 
 int rt_op_vxc(rt_handle c, const double* rho, double* vxc) {
   CHECK_HANDLE(c);
+  if (c->slab) return fail(c, RT_ESTATE, "rt_op_vxc: not available on a slab handle");
   if (!rho || !vxc) return fail(c, RT_EINVAL, "rt_op_vxc: NULL");
   CK(cudaSetDevice(c->cfg.device));
   CK(cudaMemcpyAsync(c->op_u, rho, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
@@ -1007,6 +1060,57 @@ int rt_op_vxc(rt_handle c, const double* rho, double* vxc) {
   stage_end(c);
   CK(cudaMemcpyAsync(vxc, c->w, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
   return sync_and_check(c);
+}
+
+// ---- grid-slab sharding -----------------------------------------------------------------------------
+int rt_slab_get_buffers(rt_handle c, rt_slab_buffers* out) {
+  CHECK_HANDLE(c);
+  if (!out) return fail(c, RT_EINVAL, "rt_slab_get_buffers: NULL");
+  if (!c->slab) return fail(c, RT_ESTATE, "rt_slab_get_buffers: handle was created without a slab");
+  out->xchg_rho = c->rho;
+  out->xchg_rho_count = c->Ng + 8;
+  out->xchg_H = c->H1;
+  out->xchg_H_count = (int64_t)c->N * c->ldn;
+  out->slab_offset = c->slab_off;
+  out->slab_count = c->Ngl;
+  return RT_OK;
+}
+
+int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
+  CHECK_HANDLE(c);
+  if (!c->slab) return fail(c, RT_ESTATE, "rt_slab_phase: handle was created without a slab");
+  CK(cudaSetDevice(c->cfg.device));
+  const size_t nn = (size_t)c->N * c->ldn * 8;
+  switch (phase) {
+    case RT_SLAB_INIT:            // xchg_rho holds rho0 of the whole grid, xchg_H holds H(t = 0)  (Alg. 1 lines 7-8)
+      if (c->slab_state != 0) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT already done");
+      CK(cudaMemcpyAsync(c->rho0, c->rho, (size_t)c->Ng * 8, cudaMemcpyDeviceToDevice, c->st));
+      launch_vxc(c->Ng, c->rho0, c->vxc0, c->st);
+      c->launches += 1;
+      CK(cudaMemcpyAsync(c->H0, c->H1, nn, cudaMemcpyDeviceToDevice, c->st));
+      CK(cudaMemcpyAsync(c->Hm1, c->H1, nn, cudaMemcpyDeviceToDevice, c->st));
+      CK(cudaMemsetAsync(c->d_sums + 4, 0, 8, c->st));       // induced charge at t = 0
+      c->slab_state = 1;
+      break;
+    case RT_SLAB_PROPAGATE:
+      if (c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
+      if (it < 0) return fail(c, RT_EINVAL, "rt_slab_phase: it < 0");
+      enqueue_update_propagate(c, it);
+      break;
+    case RT_SLAB_POTENTIAL:
+      if (c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
+      enqueue_update_potential(c);
+      break;
+    case RT_SLAB_SHIFT:
+      if (c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
+      enqueue_shift(c);
+      c->t += c->dt;
+      break;
+    default:
+      return fail(c, RT_EINVAL, "rt_slab_phase: unknown phase");
+  }
+  CK(cudaGetLastError());
+  return RT_OK;
 }
 
 int rt_timing_enable(rt_handle c, int32_t enable) {

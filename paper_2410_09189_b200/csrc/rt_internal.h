@@ -92,8 +92,10 @@ void launch_set_diag(int N, int ldn, double* M, const double* diag, cudaStream_t
 // ---- grid kernels (a6, a7, a8) ---------------------------------------------------------------------------
 // rho[r] = sum_p rho_part[p][r]; block partial sums of {rho, x rho, y rho, z rho, rho - rho0} -> bsums[nb][5]
 int  reduce_rho_blocks(long long Ng);
-void launch_reduce_rho(const double* rho_part, int nparts, long long Ng, GridDims gd, double h, const double* rho0,
-                       double* rho, double* bsums, double* sums, cudaStream_t st);
+// Ng points starting at x-plane x0 of the grid gd (a grid slab; x0 = 0 and Ng = nx*ny*nz for the whole grid); part,
+// rho0, rho point at the first point of the slab
+void launch_reduce_rho(const double* rho_part, int nparts, long long Ng, GridDims gd, double h, int x0,
+                       const double* rho0, double* rho, double* bsums, double* sums, cudaStream_t st);
 // w[r] = (hartree ? VH : 0) + (xc ? vxc(rho) - vxc0 : 0) + E.x(r)
 void launch_delta_v(long long Ng, GridDims gd, double h, const double* rho, const double* vxc0, const double* VH,
                     const double* E, int use_h, int use_xc, double* w, cudaStream_t st);

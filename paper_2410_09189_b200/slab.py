@@ -1,0 +1,123 @@
+"""Grid-slab sharding of the RT-TDDFT step over ranks (one process per GPU) -- plumbing only.
+
+The paper's own decomposition: the real-space grid is cut into slabs of x-planes, each rank holds
+all N orbitals on its slab.  The two grid contractions are local to a slab -- a5 gives rho on the slab, a1 gives a
+partial sum of dH over the slab ("partial sums ... followed by a reduction", L424) -- while the N x N propagator
+(a2-a4) and the O(Ng) Poisson / xc stages (a7, a8) are replicated.  Per Hamiltonian update there are exactly two
+exchange steps, both SUM all-reduces of library-owned device buffers (include/rt_tddft.h, rt_slab_*):
+
+    xchg_rho [Ng + 8]   rho on the whole grid (every rank writes its slab, zeros elsewhere -- so the sum is an
+                        all-gather that also works for slabs of different sizes and gives bit-identical copies on
+                        every rank) followed by the partial dipole / charge sums
+    xchg_H   [N * ldn]  partial H1 (the rank owning plane 0 adds diag(eps))
+
+All arithmetic runs in the CUDA library; this module only orders the phases and calls torch.distributed (NCCL over
+NVLink/NVSwitch on GPUs).  `SlabStepper` is written against a small backend interface so that the host logic can be
+covered on CPU (gloo, world_size 2) with a backend assembled from other pieces in tests/.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def slab_partition(nx: int, world: int):
+    """Contiguous x-plane ranges [(x0, n), ...], sizes differing by at most one; needs 1 <= world <= nx."""
+    if not (1 <= world <= nx):
+        raise ValueError(f"cannot cut {nx} x-planes into {world} slabs")
+    base, extra = divmod(nx, world)
+    out, x0 = [], 0
+    for r in range(world):
+        n = base + (1 if r < extra else 0)
+        out.append((x0, n))
+        x0 += n
+    return out
+
+
+class _DevicePointer:
+    """Exposes a raw device allocation through __cuda_array_interface__ so torch can wrap it without a copy."""
+
+    def __init__(self, ptr: int, count: int):
+        self.__cuda_array_interface__ = {"shape": (int(count),), "typestr": "<f8", "data": (int(ptr), False),
+                                         "version": 2, "strides": None}
+
+
+def device_view(ptr: int, count: int, device: int):
+    import torch
+    return torch.as_tensor(_DevicePointer(ptr, count), device=torch.device("cuda", device))
+
+
+class DistComm:
+    """SUM all-reduce through torch.distributed (NCCL on GPUs, gloo in the CPU tests)."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+
+    def all_reduce_sum(self, t):
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
+
+
+class CudaSlabBackend:
+    """One rt_handle created with a slab; the exchange buffers as torch views of the library's device memory."""
+
+    def __init__(self, shape, h, phi_slab, eps, occ, dt, slab, device=0, stream=None, **kw):
+        from . import binding as B
+        self.B = B
+        self.sim = B.RTTDDFT(shape, h, phi_slab, eps, occ, dt, slab=slab, device=device, stream=stream, **kw)
+        b = B.rt_slab_get_buffers(self.sim.handle)
+        self.xchg_rho = device_view(b.xchg_rho, b.xchg_rho_count, device)
+        self.xchg_H = device_view(b.xchg_H, b.xchg_H_count, device)
+        self.slab_offset, self.slab_count = int(b.slab_offset), int(b.slab_count)
+
+    def phase(self, phase: int, it: int = 0):
+        self.B.rt_slab_phase(self.sim.handle, phase, it)
+
+    def set_field(self, E):
+        self.sim.set_field(E)
+
+    def dipole(self):
+        return self.sim.dipole()
+
+    def density(self):
+        return self.sim.density()
+
+    def close(self):
+        self.sim.close()
+
+
+class SlabStepper:
+    """Runs Algorithm 1 lines 10-28 on one rank of a slab-sharded system: phases of the backend interleaved with the
+    two all-reduces.  Every rank must call the same methods in the same order."""
+
+    INIT, PROPAGATE, POTENTIAL, SHIFT = 0, 1, 2, 3       # include/rt_tddft.h RT_SLAB_*
+
+    def __init__(self, backend, comm, n_hupdates: int = 2):
+        self.backend, self.comm, self.m = backend, comm, int(n_hupdates)
+        # rt_create left the local rho0 slab and the partial H(t = 0) in the exchange buffers
+        comm.all_reduce_sum(backend.xchg_rho)
+        comm.all_reduce_sum(backend.xchg_H)
+        backend.phase(self.INIT, 0)
+        self.exchanges = 2
+
+    def step(self, nsteps: int = 1):
+        b, c = self.backend, self.comm
+        for _ in range(int(nsteps)):
+            for it in range(self.m):
+                b.phase(self.PROPAGATE, it)          # a2-a5 (+ a6 partial sums) on the slab
+                c.all_reduce_sum(b.xchg_rho)         # exchange 1: rho of the whole grid + dipole / charge sums
+                b.phase(self.POTENTIAL, it)          # a7, a8 on the whole grid, a1 over the slab
+                c.all_reduce_sum(b.xchg_H)           # exchange 2: H1 = sum of the partial projections
+                self.exchanges += 2
+            b.phase(self.SHIFT, 0)                   # line 28
+
+    def set_field(self, E):
+        self.backend.set_field(E)
+
+    def dipole(self) -> np.ndarray:
+        return self.backend.dipole()
+
+    def density(self) -> np.ndarray:
+        return self.backend.density()
+
+    def close(self):
+        self.backend.close()

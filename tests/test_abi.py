@@ -31,12 +31,13 @@ def test_header_symbols_exported(built):
 def test_config_struct_layout(built):
     from paper_2410_09189_b200 import binding
     # values printed by a C program (sizeof / offsetof on include/rt_tddft.h, x86-64 SysV ABI)
-    assert ctypes.sizeof(binding.rt_config) == 144
+    assert ctypes.sizeof(binding.rt_config) == 152 and ctypes.sizeof(binding.rt_slab_buffers) == 48
     assert binding.rt_config.dt.offset == 32 and binding.rt_config.E0.offset == 72
     assert binding.rt_config.flags.offset == 96 and binding.rt_config.stream.offset == 104
     assert binding.rt_config.propagator.offset == 112 and binding.rt_config.max_order.offset == 116
     assert binding.rt_config.dP_thrs.offset == 120 and binding.rt_config.H_thrs.offset == 128
     assert binding.rt_config.max_hupdates.offset == 136
+    assert binding.rt_config.slab_x0.offset == 140 and binding.rt_config.slab_nx.offset == 144
 
 
 def test_no_cpu_fallback(built):
