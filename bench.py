@@ -196,7 +196,9 @@ def workload_config(w, args):
             "n_hupdates": w.n_hupdates, "n_vcycles": w.n_vcycles, "phi_gb": round(w.norb * w.ngrid * 8 / 1e9, 2),
             "l2": "inputs larger than L2 (Phi streamed twice per Hamiltonian update)" if w.norb * w.ngrid * 8 > 2.5e8
             else "L2 flushed between timed steps is not possible inside a CUDA graph: working set fits L2 (stated)",
-            "parallelism": "replicas only" if args.gpus > 1 else "single GPU"}
+            "parallelism": (f"grid slabs over {args.gpus} rank(s), 2 all-reduces per Hamiltonian update"
+                            if getattr(args, "parallel", "replicas") == "slabs" else
+                            "replicas only" if args.gpus > 1 else "single GPU")}
 
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
@@ -208,6 +210,10 @@ def main():
     ap.add_argument("--config", default="nano")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: replicas = one independent system per rank (weak scaling, no data-path collective; "
+                         "default); slabs = ONE system cut into grid slabs over the ranks (strong scaling, two NCCL "
+                         "all-reduces per Hamiltonian update; paper_2410_09189_b200/slab.py)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
 
@@ -223,8 +229,14 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the RT-TDDFT path has no CPU fallback")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    slabs = args.parallel == "slabs"
+    if world > 1 or slabs:
+        if slabs and world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", str(29400 + os.getpid() % 500))
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     from paper_2410_09189_b200.build import build
     if rank == 0:
@@ -234,10 +246,23 @@ def main():
     from paper_2410_09189_b200 import binding as B
 
     # inputs: every rank propagates its own seeded system (replicas; seed offset by rank)
-    wr = replicas.replica_workload(w, rank)
+    wr = replicas.replica_workload(w, rank) if not slabs else w
     big = w.norb * w.ngrid * 8 > 2e9
     t_gen = time.perf_counter()
-    if big:
+    slab = None
+    if slabs:
+        from paper_2410_09189_b200 import slab as S
+        from paper_2410_09189_b200.workloads import make_inputs_device_slab
+        slab = S.slab_partition(w.shape[0], world)[rank]
+        comm = S.DistComm()
+        nyz = w.shape[1] * w.shape[2]
+        if big:
+            phi, eps, occ, ortho_err = make_inputs_device_slab(w, slab, rank, comm.all_reduce_sum, device=f"cuda:{local}")
+        else:
+            Phi, eps, occ = make_inputs_numpy(w)
+            phi = torch.from_numpy(np.ascontiguousarray(Phi[:, slab[0] * nyz:(slab[0] + slab[1]) * nyz])).to(f"cuda:{local}")
+            ortho_err = float(np.max(np.abs(w.dvol * Phi @ Phi.T - np.eye(w.norb))))
+    elif big:
         phi, eps, occ, ortho_err = make_inputs_device(wr, device=f"cuda:{local}")
     else:
         Phi, eps, occ = make_inputs_numpy(wr)
@@ -249,13 +274,21 @@ def main():
     stream = torch.cuda.Stream(device=local)
     E0 = w.kick if not w.laser else w.E_of_t(0.0)
     with torch.cuda.stream(stream):
-        sim = B.RTTDDFT(w.shape, w.h, phi, eps, occ, w.dt, E0=E0, n_hupdates=w.n_hupdates, n_vcycles=w.n_vcycles,
-                        device=local, stream=stream.cuda_stream)
+        if slabs:
+            backend = S.CudaSlabBackend(w.shape, w.h, phi, eps, occ, w.dt, slab, device=local,
+                                        stream=stream.cuda_stream, E0=E0, n_hupdates=w.n_hupdates,
+                                        n_vcycles=w.n_vcycles)
+            stepper = S.SlabStepper(backend, comm, n_hupdates=w.n_hupdates)
+            sim = backend.sim                   # the rt_handle owner: getters, timing and launch counts
+            sim.step = stepper.step             # rt_step is not available on a slab handle
+        else:
+            sim = B.RTTDDFT(w.shape, w.h, phi, eps, occ, w.dt, E0=E0, n_hupdates=w.n_hupdates,
+                            n_vcycles=w.n_vcycles, device=local, stream=stream.cuda_stream)
         info = sim.info()
         peak_dmma, peak_dfma = B.rt_probe_fp64_peak(local)
 
         # stage events inside the timed region when a step is long enough that they cost nothing
-        stage_in_timed = w.norb * w.norb * w.ngrid > 1e12
+        stage_in_timed = w.norb * w.norb * w.ngrid > 1e12 or slabs
         step_no = [0]
 
         def one_step():
@@ -322,23 +355,26 @@ def main():
     ms_total, e2e_ms = replicas.max_over_ranks([ms_total, e2e_sec * 1e3], device=f"cuda:{local}")
     if rank != 0:
         sim.close()
-        if world > 1:
+        if world > 1 or slabs:
             dist.destroy_process_group()
         return 0
 
     ms_per_step = ms_total / args.steps
-    value = replicas.whole_job_steps_per_s(args.steps, world, ms_total)
-    e2e_value = replicas.whole_job_steps_per_s(args.steps, world, e2e_ms)
+    jobs = 1 if slabs else world                 # slabs: all ranks advance ONE system (strong scaling)
+    value = replicas.whole_job_steps_per_s(args.steps, jobs, ms_total)
+    e2e_value = replicas.whole_job_steps_per_s(args.steps, jobs, e2e_ms)
 
     # roofline of the dominant kernel (the stage with the largest share)
     N, Ng = w.norb, w.ngrid
+    if slabs:                                    # rank 0's share of the two grid contractions
+        Ng = slab[1] * w.shape[1] * w.shape[2]
     alg = {"Hupdate": ("tensor", N * (N + 1.0) * Ng, "a1 projection project_kernel: N(N+1)Ng flop per launch (symmetric output)"),
            "Rho": ("tensor", 1.0 * N * N * Ng, "a5 density density_kernel: N^2 Ng flop per launch (triangular fold)"),
            "ELDYN": ("tensor", ((info["exp_order"] // 2 + 1) + 12.0) * N ** 3,
                      "a3+a4 gemm_abt_tma_kernel: (q+1) symmetric-output series GEMMs (N^3 each) + U P U^dagger "
                      "(2 full dual GEMMs 8N^3 + Hermitian output 4N^3)"),
-           "Vh": ("hbm", 167.0 * Ng * 8 / 7 * w.n_vcycles, "a7 V-cycles: 167 B/pt/cycle unfused x 8/7"),
-           "XC": ("hbm", 32.0 * Ng, "a8 delta_v_kernel: 32 B/pt")}
+           "Vh": ("hbm", 167.0 * w.ngrid * 8 / 7 * w.n_vcycles, "a7 V-cycles: 167 B/pt/cycle unfused x 8/7"),
+           "XC": ("hbm", 32.0 * w.ngrid, "a8 delta_v_kernel: 32 B/pt")}
     shares = {k: (stage_ms[k] / max(1, stage_calls[k])) for k in stage_ms}
     tot_stage = sum(stage_ms.values())
     dom = max(stage_ms, key=lambda k: stage_ms[k])
@@ -401,8 +437,8 @@ def main():
                    "sample": f"{n} full oracle steps on the whole workload"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": workload_config(w, args), "clocks": clocks,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if slabs else "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(w, args), "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 24, "d2h_bytes_per_step": 24 + 8 * w.ngrid,
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches), "roofline": roof, "per_kernel": per_kernel, "cpu_baseline": cpu,
@@ -412,7 +448,7 @@ def main():
             "setup_s": {"inputs": t_gen}}
     print(json.dumps(line))
     sim.close()
-    if world > 1:
+    if world > 1 or slabs:
         dist.destroy_process_group()
     return 0
 

@@ -157,3 +157,43 @@ def make_inputs_device(w: Workload, device="cuda", tile: int = 16384, passes: in
     del G
     eps, occ = eigenvalues_occ(w)
     return Phi, eps, occ, err
+
+
+def make_inputs_device_slab(w: Workload, slab, rank: int, all_reduce_sum, device="cuda", tile: int = 16384,
+                            passes: int = 2):
+    """Grid-slab version of make_inputs_device: this rank generates and keeps only the x-planes `slab = (x0, n)` of
+    Phi ([N][n*ny*nz]); the Gram matrix of the Cholesky-QR passes is summed over ranks with `all_reduce_sum(tensor)`
+    (in place), so every rank applies the same L^-1 to its slab.  Philox stream: seed + 1009 * rank."""
+    import torch
+    N = w.norb
+    ngl = slab[1] * w.shape[1] * w.shape[2]
+    gen = torch.Generator(device=device)
+    gen.manual_seed(w.seed + 1009 * rank)
+    Phi = torch.empty((N, ngl), dtype=torch.float64, device=device)
+    rows = max(1, (1 << 27) // ngl)
+    for r0 in range(0, N, rows):
+        Phi[r0:min(N, r0 + rows)].normal_(generator=gen)
+    Phi.mul_(1.0 / math.sqrt(w.ngrid * w.dvol))
+
+    def gram():
+        G = torch.zeros((N, N), dtype=torch.float64, device=device)
+        for c0 in range(0, ngl, tile):
+            blk = Phi[:, c0:c0 + tile]
+            G.addmm_(blk, blk.T, alpha=w.dvol)
+        all_reduce_sum(G)
+        return G
+
+    for _ in range(passes):
+        G = gram()
+        Lc = torch.linalg.cholesky(G)
+        del G
+        for c0 in range(0, ngl, tile):
+            blk = Phi[:, c0:c0 + tile]
+            blk.copy_(torch.linalg.solve_triangular(Lc, blk, upper=False))
+        del Lc
+    G = gram()
+    G.diagonal().sub_(1.0)
+    err = float(G.abs().max())
+    del G
+    eps, occ = eigenvalues_occ(w)
+    return Phi, eps, occ, err
