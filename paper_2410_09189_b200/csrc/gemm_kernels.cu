@@ -27,16 +27,18 @@ constexpr int PROJ_STAGE = BM * BK + BN * BK + BK;     // doubles per stage: A t
 
 __global__ void __launch_bounds__(NT, 1)
 project_kernel(const double* __restrict__ phi, const double* __restrict__ w, const int2* __restrict__ tiles,
-               double* __restrict__ W, int N, long long Ng, int T, long long kchunk, int ldn) {
+               double* __restrict__ W, const ProjectPlan pl) {
   extern __shared__ __align__(16) double smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g = lane >> 2, c = lane & 3;
   const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
-  const int s = blockIdx.x / T, t = blockIdx.x % T;
-  const int2 tt = tiles[t];
+  const int N = pl.N, ldn = pl.ldn;
+  const long long Ng = pl.Ng;
+  const ProjBlock pb = project_decode(blockIdx.x, pl);
+  const int s = pb.s;
+  const int2 tt = tiles[pb.t];
   const int i0 = tt.x * TILE, j0 = tt.y * TILE;
-  const long long kbeg = (long long)s * kchunk;
-  const long long kend = (kbeg + kchunk < Ng) ? kbeg + kchunk : Ng;
+  const long long kbeg = pb.kbeg, kend = pb.kend;
   const int nk = (int)((kend - kbeg + BK - 1) / BK);
   const bool vec = ((Ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(phi) & 15) == 0);
 
@@ -98,7 +100,7 @@ project_kernel(const double* __restrict__ phi, const double* __restrict__ w, con
 }
 
 __global__ void project_reduce_kernel(const double* __restrict__ W, const double* __restrict__ eps, double scale,
-                                      double* __restrict__ H, int N, int ldn, int S) {
+                                      double* __restrict__ H, int N, int ldn, int S, int Sd) {
   // one thread per (i, j) with j >= i; fixed summation order over the splits
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int i = blockIdx.y;
@@ -106,7 +108,8 @@ __global__ void project_reduce_kernel(const double* __restrict__ W, const double
   const long long slab = (long long)N * ldn;
   const double* p = W + (long long)i * ldn + j;
   double sum = 0.0;
-  for (int s = 0; s < S; ++s) sum += p[(long long)s * slab];
+  const int ns = (i / TILE == j / TILE) ? Sd : S;        // diagonal tiles have their own split count
+  for (int s = 0; s < ns; ++s) sum += p[(long long)s * slab];
   double v = scale * sum;
   if (i == j && eps) v += eps[i];
   H[(long long)i * ldn + j] = v;
@@ -122,13 +125,13 @@ void launch_project(const ProjectPlan& p, const double* phi, const double* w, co
     cudaFuncSetAttribute(project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)project_smem_bytes());
     attr = true;
   }
-  project_kernel<<<p.T * p.S, NT, project_smem_bytes(), st>>>(phi, w, tiles, W, p.N, p.Ng, p.T, p.kchunk, p.ldn);
+  project_kernel<<<p.grid(), NT, project_smem_bytes(), st>>>(phi, w, tiles, W, p);
 }
 
 void launch_project_reduce(const ProjectPlan& p, const double* W, const double* eps, double scale, double* H,
                            cudaStream_t st) {
   dim3 grid((p.N + 127) / 128, p.N);
-  project_reduce_kernel<<<grid, 128, 0, st>>>(W, eps, scale, H, p.N, p.ldn, p.S);
+  project_reduce_kernel<<<grid, 128, 0, st>>>(W, eps, scale, H, p.N, p.ldn, p.S, p.Sd);
 }
 
 // ======================================================================================================

@@ -61,8 +61,7 @@ __device__ __forceinline__ void init_bars(Bars* bars) {
 // ======================================================================================================
 __global__ void __launch_bounds__(NTHREADS, 1)
 project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __restrict__ w,
-                   const int2* __restrict__ tiles, double* __restrict__ W, int N, long long Ng, int T,
-                   long long kchunk, int ldn) {
+                   const int2* __restrict__ tiles, double* __restrict__ W, const ProjectPlan pl) {
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -70,11 +69,12 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   init_bars(bars);
 
-  const int s = blockIdx.x / T, t = blockIdx.x % T;
-  const int2 tt = tiles[t];
+  const int N = pl.N, ldn = pl.ldn;
+  const ProjBlock pb = project_decode(blockIdx.x, pl);
+  const int s = pb.s;
+  const int2 tt = tiles[pb.t];
   const int i0 = tt.x * TILE, j0 = tt.y * TILE;
-  const long long kbeg = (long long)s * kchunk;
-  const long long kend = (kbeg + kchunk < Ng) ? kbeg + kchunk : Ng;
+  const long long kbeg = pb.kbeg, kend = pb.kend;
   const int nk = (int)((kend - kbeg + BK - 1) / BK);
 
   if (warp >= NCONS) {
@@ -100,20 +100,41 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
   // ===== consumers =====
   regs_consumer();
   const int g = lane >> 2, c = lane & 3, pg = perm8(g);
-  const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
+  // Diagonal tile of the symmetric output: only 8 x 8 blocks on or above the diagonal are needed (project_reduce reads
+  // j >= i), 136 of the CTA's 256.  The warp roles (wm, wn) are permuted so that every scheduler partition
+  // (warp % 4) gets 32-36 of them instead of 10-58: {(0,2),(1,0)}, {(0,3),(1,1)}, {(0,1),(1,2)}, {(0,0),(1,3)}.
+  const bool diag = i0 == j0;
+  const int role = diag ? ((warp < 4) ? ((0x0132 >> (4 * warp)) & 15) : warp) : warp;
+  const int wrow = (role / WN) * (8 * FA), wcol = (role % WN) * (8 * FB);
+  // blocks on or above the diagonal, as row counts for the two column halves of the warp tile (rounded up to a
+  // rectangle): (0,0), (1,2): rows < 2 | 4 ; (0,1), (1,3): rows < 6 | 8 ; (0,2), (0,3): all ; (1,0), (1,1): none
+  const int dlt = (wcol - wrow) / 8;
   double acc[FA][FB][2];
 #pragma unroll
   for (int a = 0; a < FA; ++a)
 #pragma unroll
     for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
 
-  for (int kt = 0; kt < nk; ++kt) {
-    const int slot = kt % ST;
-    mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
-    const double* sA = tilesm + (size_t)slot * STAGE_D;
-    mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
-    __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+  if (!diag) {
+    for (int kt = 0; kt < nk; ++kt) {
+      const int slot = kt % ST;
+      mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
+      const double* sA = tilesm + (size_t)slot * STAGE_D;
+      mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+    }
+  } else {
+    for (int kt = 0; kt < nk; ++kt) {
+      const int slot = kt % ST;
+      mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
+      const double* sA = tilesm + (size_t)slot * STAGE_D;
+      if (dlt >= 8) mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+      else if (dlt == 4) mma_stage_kc_tma<FA, FB, true, 6, 8>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+      else if (dlt == 0) mma_stage_kc_tma<FA, FB, true, 2, 4>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+    }
   }
 
   // epilogue: raw partial sums into slab s.  MMA row g <-> tile row perm8(g); tile col n' <-> perm8(n')
@@ -136,7 +157,7 @@ size_t tma_smem_bytes() { return SMEM_TOTAL; }
 
 void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const double* w, const int2* tiles, double* W,
                         cudaStream_t st) {
-  project_tma_kernel<<<p.T * p.S, NTHREADS, SMEM_TOTAL, st>>>(tmPhi, w, tiles, W, p.N, p.Ng, p.T, p.kchunk, p.ldn);
+  project_tma_kernel<<<p.grid(), NTHREADS, SMEM_TOTAL, st>>>(tmPhi, w, tiles, W, p);
 }
 
 // ======================================================================================================
@@ -239,7 +260,15 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
         const int slot = (int)(it % ST);
         mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
         const double* sA = tilesm + (size_t)slot * STAGE_D;
-        mma_stage_nc_tma<FA, FB>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
+        // stage sidx holds the contraction rows k = j0 + 16 sidx ...: inside the diagonal block (sidx < 8) the fold is
+        // upper triangular, Pfold[j][k] = 0 for k < j, so row block a of this warp is all zeros in half `half` of the
+        // stage unless 8 (wrow/8 + a) <= 16 sidx + 8 half + 7
+        // (both halves of a stage then need the same even number of row blocks: na = 2 sidx + 2 - wrow/8)
+        const int na = 2 * (sg.s0 + sg.dir * i) + 2 - wrow / 8;
+        if (na >= 8) mma_stage_nc_tma<FA, FB>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
+        else if (na == 6) mma_stage_nc_tma<FA, FB, 6>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
+        else if (na == 4) mma_stage_nc_tma<FA, FB, 4>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
+        else if (na == 2) mma_stage_nc_tma<FA, FB, 2>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
       }

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <queue>
 #include <string>
 #include <vector>
 
@@ -597,28 +598,52 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   {
     ProjectPlan& p = c->pp;
     p.N = N; p.Ng = Ng; p.ntile = ntile; p.T = ntile * (ntile + 1) / 2; p.ldn = ldn;
-    // split-K factor: enough CTAs for >= 2 waves when the tile count is small, and T*S chosen to fill whole
-    // waves of one CTA per SM (wave quantisation was 14% of the first nano profile at S = 2: 380 CTAs = 2.57 waves)
+    p.Toff = ntile * (ntile - 1) / 2;
+    // Split-K factors.  One CTA per SM, CTAs handed out in block order: the plan is the (S, Sd) whose greedy schedule
+    // on `sms` machines finishes first.  Cost model in pipeline stages (16 grid points of one 128 x 128 tile): an
+    // off-diagonal CTA costs kchunk/16, a diagonal one diag_cost * kchunk_d/16 (the TMA kernel issues 160 of the 256
+    // 8 x 8 blocks of a diagonal tile; measured ~0.65), plus a fixed prologue/epilogue per CTA and a term per split for
+    // the second-stage reduction.  (Wave quantisation was 14 % of the first nano profile at S = 2.)
     const int sms = prop.multiProcessorCount;
+    const bool tma_likely = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && get_encode_fn() != nullptr;
+    const double diag_cost = tma_likely ? 0.65 : 1.0;
+    // one stage ~ 2.1 us on one SM; the reduction reads one N x ldn slab per split at ~3 TB/s
+    const double cta_ovh = 8.0, split_ovh = (double)N * ldn * 8.0 / 3.0e12 / 2.1e-6;
     const long long kmin = 16 * 8;
     long long smax = (Ng + kmin - 1) / kmin;
     if (smax > 4 * sms) smax = 4 * sms;
     const double slab_bytes = (double)N * ldn * 8;
     while (smax > 1 && smax * slab_bytes > 2.0e9) --smax;          // workspace cap
-    long long S = 1;
-    double best = -1.0;
+    auto chunk_of = [&](long long S_) { long long kc = (Ng + S_ - 1) / S_; return (kc + 15) / 16 * 16; };
+    auto makespan = [&](long long n1, double c1, long long n2, double c2) {
+      std::priority_queue<double, std::vector<double>, std::greater<double>> q;
+      for (int i = 0; i < sms; ++i) q.push(0.0);
+      double end = 0.0;
+      for (long long j = 0; j < n1 + n2; ++j) {
+        const double t = q.top() + (j < n1 ? c1 : c2);
+        q.pop();
+        q.push(t);
+        if (t > end) end = t;
+      }
+      return end;
+    };
+    double best = 1e300;
+    p.S = p.Sd = 1;
+    p.kchunk = p.kchunk_d = chunk_of(1);
     for (long long s = 1; s <= smax; ++s) {
-      const long long ctas = (long long)p.T * s;
-      if (ctas < 2LL * sms && s < smax) continue;                   // want at least two waves of work
-      const long long waves = (ctas + sms - 1) / sms;
-      const double eff = (double)ctas / (double)(waves * sms);
-      if (eff > best + 1e-9) { best = eff; S = s; }
-      if (eff > 0.985) break;
+      const long long kc = chunk_of(s);
+      const long long S_ = (Ng + kc - 1) / kc;
+      if (S_ != s) continue;                                       // same chunk as a smaller s
+      const long long sd0 = (long long)std::llround(diag_cost * (double)s);
+      for (long long sd = sd0 - 1; sd <= sd0 + 1; ++sd) {
+        if (sd < 1 || sd > s) continue;
+        const long long kd = chunk_of(sd);
+        const long long Sd_ = (Ng + kd - 1) / kd;
+        const double obj = makespan(S_ * p.Toff, kc / 16.0 + cta_ovh, Sd_ * ntile, diag_cost * kd / 16.0 + cta_ovh) +
+                           split_ovh * (double)(p.Toff > 0 ? S_ : Sd_);
+        if (obj < best - 1e-9) { best = obj; p.S = (int)S_; p.kchunk = kc; p.Sd = (int)Sd_; p.kchunk_d = kd; }
+      }
     }
-    long long kc = (Ng + S - 1) / S;
-    kc = (kc + 15) / 16 * 16;
-    p.kchunk = kc;
-    p.S = (int)((Ng + kc - 1) / kc);
     DensityPlan& d = c->dp;
     d.N = N; d.Ng = Ng; d.ntile = ntile; d.npairs = (ntile + 1) / 2; d.nrt = (Ng + TILE - 1) / TILE; d.ldn = ldn;
     // work types of the TMA kernel: one per pair.  (Cutting the pairs' time lines into several types per r-tile, so
@@ -701,8 +726,9 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   }
   {
     std::vector<int2> tiles;
-    for (int ti = 0; ti < ntile; ++ti)
-      for (int tj = ti; tj < ntile; ++tj) tiles.push_back(make_int2(ti, tj));
+    for (int ti = 0; ti < ntile; ++ti)                    // off-diagonal tiles first, then the diagonal (ProjectPlan)
+      for (int tj = ti + 1; tj < ntile; ++tj) tiles.push_back(make_int2(ti, tj));
+    for (int ti = 0; ti < ntile; ++ti) tiles.push_back(make_int2(ti, ti));
     ALLOC(c->d_tiles, tiles.size());
     CKC(cudaMemcpyAsync(c->d_tiles, tiles.data(), tiles.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
     CKC(cudaStreamSynchronize(c->st));

@@ -12,15 +12,35 @@ constexpr int TILE = 128;        // CTA tile edge of the DMMA kernels (orbital i
 struct GridDims { int nx, ny, nz; };
 
 // ---- a1 projection: W[s][i][j] = sum_{r in chunk s} phi_i(r) w(r) phi_j(r) for upper tiles (ti <= tj) -----
+// The tile list holds the Toff = ntile (ntile - 1) / 2 off-diagonal tiles first, then the ntile diagonal ones.  Blocks
+// [0, S Toff) are (split s, off-diagonal tile t), s-major; blocks [S Toff, S Toff + Sd ntile) are the diagonal tiles,
+// which the TMA kernel computes at ~0.65 of the cost of a full tile (blocks below the diagonal are not issued) and
+// which therefore get fewer, longer splits, so that every CTA costs about the same.
 struct ProjectPlan {
   int N;                 // orbitals
   long long Ng;          // grid points (contraction length), also the leading dimension of Phi
   int ntile;             // ceil(N / TILE)
   int T;                 // number of upper-triangular tiles
-  int S;                 // split-K factor
+  int Toff;              // off-diagonal tiles
+  int S;                 // split-K factor of the off-diagonal tiles
   long long kchunk;      // grid points per split (multiple of 16)
+  int Sd;                // split-K factor of the diagonal tiles (<= S)
+  long long kchunk_d;
   int ldn;               // leading dimension of the N x N outputs
+  int grid() const { return S * Toff + Sd * ntile; }
 };
+struct ProjBlock { int s, t; long long kbeg, kend; };
+#ifdef __CUDACC__
+__device__ __forceinline__ ProjBlock project_decode(int b, const ProjectPlan& p) {
+  ProjBlock r;
+  long long kc;
+  if (b < p.S * p.Toff) { r.s = b / p.Toff; r.t = b - r.s * p.Toff; kc = p.kchunk; }
+  else { const int bb = b - p.S * p.Toff; r.s = bb / p.ntile; r.t = p.Toff + (bb - r.s * p.ntile); kc = p.kchunk_d; }
+  r.kbeg = (long long)r.s * kc;
+  r.kend = (r.kbeg + kc < p.Ng) ? r.kbeg + kc : p.Ng;
+  return r;
+}
+#endif
 void launch_project(const ProjectPlan& p, const double* phi, const double* w, const int2* tiles, double* W,
                     cudaStream_t st);
 // H[i][j] = scale * sum_s W[s][i][j] (+ eps_i if i == j and eps != nullptr), mirrored to the lower triangle.

@@ -85,16 +85,21 @@ __device__ __forceinline__ int perm8(int g) { return (g >> 1) | ((g & 1) << 2); 
 
 // ---- one pipeline stage of MMAs on TMA-swizzled tiles ---------------------------------------------------
 // A, B K-contiguous ([128][16], 128B swizzle).  pg = perm8(lane >> 2), c = lane & 3.
-template <int FA, int FB, bool SCALE>
+// NA0 / NA1: number of row blocks (from the top of the warp tile) computed for the column blocks b < FB/2 / b >= FB/2.
+// On a diagonal CTA tile of a symmetric product the 8 x 8 blocks strictly below the diagonal are never read; a
+// PREDICATED-off DMMA still costs its statically scheduled issue slot (measured: no gain), so the skipped blocks are
+// removed at compile time and the kernel branches between a few instantiations.
+template <int FA, int FB, bool SCALE, int NA0 = FA, int NA1 = FA>
 __device__ __forceinline__ void mma_stage_kc_tma(double (&acc)[FA][FB][2], const double* __restrict__ smA,
                                                  const double* __restrict__ smB, const double* __restrict__ wk,
                                                  int wrow, int wcol, int pg, int c) {
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
     const int off = pg * BK + (((c + 4 * half) ^ pg) << 1);
+    constexpr int NAM = NA0 > NA1 ? NA0 : NA1;
     double2 af[FA], bf[FB];
 #pragma unroll
-    for (int a = 0; a < FA; ++a) af[a] = *reinterpret_cast<const double2*>(smA + (wrow + 8 * a) * BK + off);
+    for (int a = 0; a < NAM; ++a) af[a] = *reinterpret_cast<const double2*>(smA + (wrow + 8 * a) * BK + off);
 #pragma unroll
     for (int b = 0; b < FB; ++b) bf[b] = *reinterpret_cast<const double2*>(smB + (wcol + 8 * b) * BK + off);
     if (SCALE) {
@@ -105,17 +110,21 @@ __device__ __forceinline__ void mma_stage_kc_tma(double (&acc)[FA][FB][2], const
 #pragma unroll
     for (int a = 0; a < FA; ++a)
 #pragma unroll
-      for (int b = 0; b < FB; ++b) dmma884(acc[a][b][0], acc[a][b][1], af[a].x, bf[b].x);
+      for (int b = 0; b < FB; ++b)
+        if (a < (b < FB / 2 ? NA0 : NA1)) dmma884(acc[a][b][0], acc[a][b][1], af[a].x, bf[b].x);
 #pragma unroll
     for (int a = 0; a < FA; ++a)
 #pragma unroll
-      for (int b = 0; b < FB; ++b) dmma884(acc[a][b][0], acc[a][b][1], af[a].y, bf[b].y);
+      for (int b = 0; b < FB; ++b)
+        if (a < (b < FB / 2 ? NA0 : NA1)) dmma884(acc[a][b][0], acc[a][b][1], af[a].y, bf[b].y);
   }
 }
 
 // A K-contiguous, B N-contiguous in 8 boxes of [16 k][16 n].  Lane g = lane >> 2 reads chunk g of box
 // (wcol/16 + t) at k-row k: columns 16 t + 2 g + {0,1} -> n-tiles 2t, 2t+1 (same interleave as dmma_core.cuh).
-template <int FA, int FB>
+// NA: number of row blocks (from the top of the warp tile) that are computed.  On the diagonal block of the upper-
+// triangular fold the A fragments of the lower row blocks are all zeros (compile-time removal: see above).
+template <int FA, int FB, int NA = FA>
 __device__ __forceinline__ void mma_stage_nc_tma(double (&acc)[FA][FB][2], const double* __restrict__ smA,
                                                  const double* __restrict__ smB, int wrow, int wcol, int g, int pg,
                                                  int c) {
@@ -124,7 +133,7 @@ __device__ __forceinline__ void mma_stage_nc_tma(double (&acc)[FA][FB][2], const
     const int off = pg * BK + (((c + 4 * half) ^ pg) << 1);
     double2 af[FA];
 #pragma unroll
-    for (int a = 0; a < FA; ++a) af[a] = *reinterpret_cast<const double2*>(smA + (wrow + 8 * a) * BK + off);
+    for (int a = 0; a < NA; ++a) af[a] = *reinterpret_cast<const double2*>(smA + (wrow + 8 * a) * BK + off);
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const int k = 2 * c + 8 * half + e;
@@ -133,7 +142,7 @@ __device__ __forceinline__ void mma_stage_nc_tma(double (&acc)[FA][FB][2], const
       for (int t = 0; t < FB / 2; ++t)
         bf[t] = *reinterpret_cast<const double2*>(smB + ((wcol >> 4) + t) * 256 + k * BK + ((g ^ (k & 7)) << 1));
 #pragma unroll
-      for (int a = 0; a < FA; ++a)
+      for (int a = 0; a < NA; ++a)
 #pragma unroll
         for (int t = 0; t < FB / 2; ++t) {
           const double av = e ? af[a].y : af[a].x;
