@@ -104,6 +104,39 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
   // j >= i), 136 of the CTA's 256.  The warp roles (wm, wn) are permuted so that every scheduler partition
   // (warp % 4) gets 32-36 of them instead of 10-58: {(0,2),(1,0)}, {(0,3),(1,1)}, {(0,1),(1,2)}, {(0,0),(1,3)}.
   const bool diag = i0 == j0;
+  double* Ws = W + (long long)s * N * ldn;
+  if (!diag && N - j0 <= 96) {
+    // Ragged last tile column with at most 96 valid columns (N = 2400: 96): the 8 warps cover 128 x 96 as 2 x 4 warp
+    // tiles of 64 x 24 instead of leaving the warps of the last 32 columns multiplying padding.
+    constexpr int FB3 = 3;
+    const int wrow3 = (warp / WN) * (8 * FA), wcol3 = (warp % WN) * (8 * FB3);
+    double acc3[FA][FB3][2];
+#pragma unroll
+    for (int a = 0; a < FA; ++a)
+#pragma unroll
+      for (int b = 0; b < FB3; ++b) acc3[a][b][0] = acc3[a][b][1] = 0.0;
+    for (int kt = 0; kt < nk; ++kt) {
+      const int slot = kt % ST;
+      mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
+      const double* sA = tilesm + (size_t)slot * STAGE_D;
+      mma_stage_kc_tma<FA, FB3, true>(acc3, sA, sA + TILE_D, wsm + slot * BK, wrow3, wcol3, pg, c);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+    }
+#pragma unroll
+    for (int a = 0; a < FA; ++a) {
+      const int row = i0 + wrow3 + 8 * a + pg;
+      if (row < N) {
+#pragma unroll
+        for (int b = 0; b < FB3; ++b) {
+          const int col = j0 + wcol3 + 8 * b + c;
+          if (col < N) Ws[(long long)row * ldn + col] = acc3[a][b][0];
+          if (col + 4 < N) Ws[(long long)row * ldn + col + 4] = acc3[a][b][1];
+        }
+      }
+    }
+    return;
+  }
   const int role = diag ? ((warp < 4) ? ((0x0132 >> (4 * warp)) & 15) : warp) : warp;
   const int wrow = (role / WN) * (8 * FA), wcol = (role % WN) * (8 * FB);
   // blocks on or above the diagonal, as row counts for the two column halves of the warp tile (rounded up to a
@@ -138,7 +171,6 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
   }
 
   // epilogue: raw partial sums into slab s.  MMA row g <-> tile row perm8(g); tile col n' <-> perm8(n')
-  double* Ws = W + (long long)s * N * ldn;
 #pragma unroll
   for (int a = 0; a < FA; ++a) {
     const int row = i0 + wrow + 8 * a + pg;
