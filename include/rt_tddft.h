@@ -87,6 +87,9 @@ typedef struct {
    *    [slab_x0, slab_x0 + slab_nx) of the nx*ny*nz grid and `phi` holds only those: [norb][slab_nx*ny*nz].
    *    slab_nx = 0: the whole grid (single GPU; every entry point above).  slab_nx > 0: see rt_slab_* below.   */
   int32_t  slab_x0, slab_nx;
+  /* -- dipole history: > 0 keeps the dipole of the last `history` time levels on the device, appended by the step
+   *    itself (no host synchronisation per step); read with rt_get_dipole_series.  0 = off.                        */
+  int32_t  history;
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
@@ -105,6 +108,11 @@ int rt_get_dipole(rt_handle h, double mu[3]);
 
 /* Density rho(r) at the current time into rho[Ng] (EITHER).  Synchronises the stream. */
 int rt_get_density(rt_handle h, double* rho);
+
+/* Dipole time series mu(t_k), k = first .. first + n - 1 (k = 0 is t = 0), into out[n][4] (HOST): mu_x, mu_y, mu_z and
+ * the charge dVol sum rho.  Needs rt_config.history > 0; only the last `history` levels are kept (RT_EINVAL for
+ * older or future ones).  Synchronises the stream once, however many steps were enqueued. */
+int rt_get_dipole_series(rt_handle h, int64_t first, int32_t n, double* out);
 
 /* ---- diagnostics / test aids ------------------------------------------------------------------ */
 
@@ -195,6 +203,19 @@ int rt_timing_enable(rt_handle h, int32_t enable);
 /* Synchronises; ms[RT_STAGE_COUNT] (HOST) = accumulated device milliseconds per stage since the last call,
  * calls[RT_STAGE_COUNT] (HOST) = number of times each stage ran.  Resets the accumulators. */
 int rt_timing_read(rt_handle h, double ms[RT_STAGE_COUNT], int64_t calls[RT_STAGE_COUNT]);
+
+/* ---- photoabsorption spectrum from delta-kick runs (post-processing kernel, stateless) ------------------
+ * "Photoabsorption spectra are calculated as a sum of Fourier transforms of mu_x(t), mu_y(t) and mu_z(t) obtained from
+ * three independent simulations with the kick ... along x, y, and z".  The paper prints no formula;
+ * DESIGN R16 takes the standard dipole strength function
+ *   S(w) = -(2 w / (3 pi)) sum_q (1/kappa_q) Im  dt sum_n' c_n [mu_q(t_n) - mu_q(0)] exp((i w - gamma)(t_n - t_kick))
+ * with trapezoid weights c_n (1/2 at both ends), t_n = n dt, n = 0..nt-1, kappa_q the delivered impulse (E_kick dt / 2
+ * for the end-point sampled kick of DESIGN R5, with t_kick = dt / 2) and an exponential damping gamma.
+ * mu: [3][nt] (HOST or DEVICE), row q = the q-component of the dipole of the run kicked along q; a row whose
+ * kappa_q == 0 is skipped (and the 1/3 becomes 1/(number of rows used)).  omega: [nw], S: [nw] (HOST or DEVICE).
+ * Runs on `device` / `stream` (cudaStream_t) and synchronises the stream before returning. */
+int rt_spectrum(const double* mu, int32_t nt, double dt, double t_kick, const double kappa[3], double gamma,
+                const double* omega, int32_t nw, double* S, int32_t device, void* stream);
 
 /* ---- calibration instrument (not on the hot path) ----------------------------------------------------
  * Measures the FP64 issue-rate ceilings of `device` with register-resident operands: DMMA.8x8x4 (mma.sync

@@ -365,3 +365,32 @@ class RTOracle:
             e += self.dVol * float(np.sum(exc_density_lda(self.rho) - exc_density_lda(self.rho0) - self.vxc0 * drho))
         e += self.dVol * float(np.sum(field_potential(self.shape, self.h, self.E_next) * drho))
         return e
+
+
+# --------------------------------------------------------------------------------------------------
+# Photoabsorption spectrum of delta-kick runs (DESIGN R16)
+# --------------------------------------------------------------------------------------------------
+
+def dipole_strength(mu: np.ndarray, dt: float, t_kick: float, kappa, gamma: float, omega: np.ndarray) -> np.ndarray:
+    """S(w) = -(2 w / (n_used pi)) sum_q (1/kappa_q) Im dt sum_n c_n [mu_q(t_n) - mu_q(0)] exp((i w - gamma)(t_n - t_kick)).
+
+    "Photoabsorption spectra are calculated as a sum of Fourier transforms of mu_x(t), mu_y(t) and mu_z(t) obtained
+    from three independent simulations with the kick ... along x, y, and z" (L453).  mu[q] is the q-component of the
+    dipole of the run kicked along q with delivered impulse kappa_q (rows with kappa_q = 0 are skipped); trapezoid
+    weights c_n, exponential damping gamma, phases counted from the effective kick time t_kick.  Plain loop over
+    frequencies; no FFT, so omega may be any grid."""
+    mu = np.asarray(mu, dtype=np.float64)
+    omega = np.asarray(omega, dtype=np.float64)
+    nt = mu.shape[1]
+    t = np.arange(nt) * dt - t_kick
+    c = np.ones(nt)
+    c[0] = c[-1] = 0.5
+    used = [q for q in range(3) if kappa[q] != 0.0]
+    S = np.zeros(omega.shape[0])
+    for iw, w in enumerate(omega):
+        acc = 0.0
+        for q in used:
+            ft = dt * np.sum(c * (mu[q] - mu[q, 0]) * np.exp((1j * w - gamma) * t))
+            acc += ft.imag / kappa[q]
+        S[iw] = -(2.0 * w / (len(used) * np.pi)) * acc
+    return S

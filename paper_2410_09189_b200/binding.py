@@ -27,7 +27,7 @@ SYMBOLS = (
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
-    "rt_slab_get_buffers", "rt_slab_phase",
+    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum",
 )
 
 RT_SLAB_INIT, RT_SLAB_PROPAGATE, RT_SLAB_POTENTIAL, RT_SLAB_SHIFT = 0, 1, 2, 3
@@ -51,6 +51,7 @@ class rt_config(C.Structure):
         ("dP_thrs", C.c_double), ("H_thrs", C.c_double),
         ("max_hupdates", C.c_int32),
         ("slab_x0", C.c_int32), ("slab_nx", C.c_int32),
+        ("history", C.c_int32),
     ]
 
 
@@ -81,6 +82,8 @@ def _load():
         "rt_op_propagate": [vp, dp, dp, dp, dp, dp], "rt_op_hartree": [vp, dp, dp, i32], "rt_op_vxc": [vp, dp, dp],
         "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp], "rt_get_convergence": [vp, dp, dp],
         "rt_slab_get_buffers": [vp, C.POINTER(rt_slab_buffers)], "rt_slab_phase": [vp, i32, i32],
+        "rt_get_dipole_series": [vp, C.c_int64, i32, dp],
+        "rt_spectrum": [dp, i32, C.c_double, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
     }
     for name, argtypes in sig.items():
         fn = getattr(lib, name)
@@ -247,6 +250,31 @@ def rt_probe_fp64_peak(device=0):
     return a.value, b.value
 
 
+def rt_get_dipole_series(h, first: int, n: int) -> np.ndarray:
+    """[n][4]: mu_x, mu_y, mu_z, charge of the time levels first .. first + n - 1 (level 0 is t = 0)."""
+    out = np.zeros((int(n), 4))
+    _check(h, _lib.rt_get_dipole_series(h, int(first), int(n), _ptr(out)))
+    return out
+
+
+def rt_spectrum(mu, dt, t_kick, kappa, gamma, omega, device=0, stream=0, out=None):
+    """Dipole strength function S(omega) of delta-kick runs (include/rt_tddft.h rt_spectrum).  mu: [3][nt] numpy array
+    or CUDA tensor; omega: [nw]; returns S as a numpy array unless `out` (numpy / CUDA tensor) is given."""
+    if not hasattr(mu, "is_cuda"):
+        mu = np.ascontiguousarray(mu, dtype=np.float64)
+    nt = int(mu.shape[1])
+    if not hasattr(omega, "is_cuda"):
+        omega = np.ascontiguousarray(omega, dtype=np.float64)
+    nw = int(omega.shape[0])
+    if out is None:
+        out = np.zeros(nw)
+    k = np.ascontiguousarray(kappa, dtype=np.float64)
+    rc = _lib.rt_spectrum(_ptr(mu), nt, float(dt), float(t_kick), _ptr(k), float(gamma), _ptr(omega), nw, _ptr(out),
+                          int(device), int(stream) if stream else None)
+    _check(None, rc)
+    return out
+
+
 def rt_slab_get_buffers(h) -> rt_slab_buffers:
     b = rt_slab_buffers()
     _check(h, _lib.rt_slab_get_buffers(h, C.byref(b)))
@@ -265,11 +293,12 @@ class RTTDDFT:
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
                  nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
                  device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0,
-                 slab=None):
+                 slab=None, history=0):
         """``slab = (x0, nx_local)``: the handle owns those x-planes and ``phi`` is [norb][nx_local*ny*nz]
         (rt_slab_* entry points; see slab.py)."""
         cfg = rt_config()
         cfg.slab_x0, cfg.slab_nx = (int(slab[0]), int(slab[1])) if slab else (0, 0)
+        cfg.history = int(history)
         cfg.propagator = {"taylor": RT_PROP_TAYLOR, "commutator": RT_PROP_COMMUTATOR}[propagator]
         cfg.max_order, cfg.dP_thrs, cfg.H_thrs, cfg.max_hupdates = int(max_order), float(dP_thrs), float(H_thrs), int(max_hupdates)
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)
@@ -303,6 +332,7 @@ class RTTDDFT:
             except ImportError:
                 stream = 0
         cfg.stream = int(stream) if stream else None
+        self._dt = float(dt)
         self.shape, self.norb = tuple(int(s) for s in shape), int(len(eps))
         self.ngrid = self.shape[0] * self.shape[1] * self.shape[2]
         self.handle = rt_create(cfg, phi, eps, occ)
@@ -320,6 +350,12 @@ class RTTDDFT:
         if out is None:
             out = np.empty(self.ngrid)
         return rt_get_density(self.handle, out)
+
+    def dipole_series(self, first=0, n=None):
+        """Dipole history kept on the device (needs history > 0): [n][4] = mu_x, mu_y, mu_z, charge."""
+        if n is None:
+            n = int(round(self.time / self._dt)) + 1 - int(first)
+        return rt_get_dipole_series(self.handle, first, n)
 
     def pmatrix(self):
         re, im = np.empty((self.norb, self.norb)), np.empty((self.norb, self.norb))

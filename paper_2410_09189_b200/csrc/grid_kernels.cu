@@ -106,6 +106,52 @@ void launch_sum_only(const double* v, long long n, double* bsums, double* sums, 
   final_sums_kernel<<<1, 32 * 5, 0, st>>>(bsums, nb, 5, sums);
 }
 
+// ------------------------------------------------------------------------- dipole history and spectrum
+__global__ void record_dipole_kernel(const double* __restrict__ sums, double dvol, double* __restrict__ hist, int cap,
+                                     unsigned long long* __restrict__ count) {
+  if (threadIdx.x == 0) {
+    const unsigned long long k = *count;
+    double* e = hist + (k % (unsigned long long)cap) * 4;
+    e[0] = dvol * sums[1]; e[1] = dvol * sums[2]; e[2] = dvol * sums[3]; e[3] = dvol * sums[0];
+    *count = k + 1;
+  }
+}
+void launch_record_dipole(const double* sums, double dvol, double* hist, int cap, unsigned long long* count,
+                          cudaStream_t st) {
+  record_dipole_kernel<<<1, 32, 0, st>>>(sums, dvol, hist, cap, count);
+}
+
+// Dipole strength function (include/rt_tddft.h rt_spectrum).  One warp per frequency: lanes stride over
+// the time samples, shuffle tree at the end (fixed order).
+__global__ void __launch_bounds__(128)
+spectrum_kernel(const double* __restrict__ mu, int nt, double dt, double t_kick, double k0, double k1, double k2,
+                int nused, double gamma, const double* __restrict__ omega, int nw, double* __restrict__ S) {
+  const int iw = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (iw >= nw) return;
+  const double w = omega[iw];
+  const double kap[3] = {k0, k1, k2};
+  double acc = 0.0;
+  for (int q = 0; q < 3; ++q) {
+    if (kap[q] == 0.0) continue;
+    const double* m = mu + (long long)q * nt;
+    const double m0 = m[0];
+    double im = 0.0;
+    for (int n = lane; n < nt; n += 32) {
+      const double t = (double)n * dt - t_kick;
+      const double cn = (n == 0 || n == nt - 1) ? 0.5 : 1.0;
+      im += cn * (m[n] - m0) * exp(-gamma * t) * sin(w * t);
+    }
+    im = warp_sum(im);
+    acc += im / kap[q];
+  }
+  if (lane == 0) S[iw] = -(2.0 * w / ((double)nused * 3.14159265358979323846)) * dt * acc;
+}
+void launch_spectrum(const double* mu, int nt, double dt, double t_kick, const double* kappa3, int nused, double gamma,
+                     const double* omega, int nw, double* S, cudaStream_t st) {
+  spectrum_kernel<<<(nw + 3) / 4, 128, 0, st>>>(mu, nt, dt, t_kick, kappa3[0], kappa3[1], kappa3[2], nused, gamma, omega,
+                                                 nw, S);
+}
+
 // ---------------------------------------------------------------------------------------------- a8
 // Slater exchange + Perdew-Zunger 1981 correlation, unpolarised (DESIGN R7); branch on rho <= 3/(4 pi).
 __device__ __forceinline__ double vxc_pz81(double rho) {

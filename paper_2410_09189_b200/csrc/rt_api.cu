@@ -31,6 +31,10 @@ struct rt_ctx {
   int x0 = 0;                    // first x-plane of the slab
   bool slab = false;
   int slab_state = 0;            // 0: waiting for RT_SLAB_INIT, 1: ready
+  int hist_cap = 0;              // dipole history (time levels kept on the device); 0 = off
+  double* d_hist = nullptr;      // [hist_cap][4]
+  unsigned long long* d_hist_n = nullptr;   // levels recorded so far (device counter: the step graph increments it)
+  int64_t steps_done = 0;        // time levels after t = 0 enqueued so far
   GridDims gd{};
   double h = 0, dvol = 0, dt = 0, sigma = 0, omega = 0;
   int m = 2, n_vc = 0, nu1 = 2, nu2 = 2, q = 0;           // q: cos/sinc polynomial degree in Y = X^2
@@ -415,9 +419,16 @@ void enqueue_update(rt_ctx* c, int it) {
   enqueue_update_potential(c);
 }
 
+void enqueue_record(rt_ctx* c) {                 // Alg. 1 line 27: the dipole of this time level joins the series
+  if (!c->hist_cap) return;
+  launch_record_dipole(c->d_sums, c->dvol, c->d_hist, c->hist_cap, c->d_hist_n, c->st);
+  c->launches += 1;
+}
+
 void enqueue_shift(rt_ctx* c) {
   launch_copy5(c->N, c->ldn, c->Hm1, c->H0, c->H0, c->H1, c->P0r, c->P1r, c->P0i, c->P1i, c->st);   // line 28
   c->launches += 1;
+  enqueue_record(c);
 }
 
 // One time step with a fixed number of Hamiltonian updates, Algorithm 1 lines 10-28.
@@ -495,6 +506,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     return fail(c, RT_EINVAL, "rt_create: slab [slab_x0, slab_x0 + slab_nx) must lie inside [0, nx)");
   if (cfg->slab_nx > 0 && cfg->H_thrs > 0.0)
     return fail(c, RT_EINVAL, "rt_create: the dynamic H_thrs loop is driven by rt_step and is not available on a slab handle");
+  if (cfg->history < 0) return fail(c, RT_EINVAL, "rt_create: history < 0");
   if (cfg->max_order < 0 || cfg->max_order > MAX_ORDER || cfg->max_hupdates < 0 || !(cfg->dP_thrs >= 0.0) ||
       !(cfg->H_thrs >= 0.0))
     return fail(c, RT_EINVAL, "rt_create: bad max_order / max_hupdates / dP_thrs / H_thrs");
@@ -700,6 +712,12 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   }
   const size_t nn = (size_t)N * ldn;
   ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8);
+  c->hist_cap = cfg->history;
+  if (c->hist_cap) {
+    ALLOC(c->d_hist, (size_t)c->hist_cap * 4);
+    ALLOC(c->d_hist_n, 1);
+    CKC(cudaMemsetAsync(c->d_hist_n, 0, sizeof(unsigned long long), c->st));
+  }
   ALLOC(c->d_bsums, 5 * 1024);
   if (c->prop == RT_PROP_COMMUTATOR || c->dynamic) {
     ALLOC(c->d_cs, 1);
@@ -765,6 +783,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     CKC(cudaMemcpyAsync(c->H1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
     // sums[4] currently holds sum(rho0) (rho0 pointer was NULL): the induced charge at t = 0 is zero
     CKC(cudaMemsetAsync(c->d_sums + 4, 0, 8, c->st));
+    enqueue_record(c);                                             // time level 0
   } else {
     // slab: the local pieces go to the exchange buffers; RT_SLAB_INIT finishes after the caller's all-reduce
     enqueue_density(c, c->P0r, c->rho + c->slab_off, nullptr);
@@ -872,8 +891,26 @@ int rt_step(rt_handle c, int32_t nsteps) {
       CK(cudaGetLastError());
     }
     c->t += c->dt;
+    c->steps_done += 1;
   }
   return RT_OK;
+}
+
+int rt_get_dipole_series(rt_handle c, int64_t first, int32_t n, double* out) {
+  CHECK_HANDLE(c);
+  if (!out || n < 0 || first < 0) return fail(c, RT_EINVAL, "rt_get_dipole_series: bad argument");
+  if (!c->hist_cap) return fail(c, RT_EINVAL, "rt_get_dipole_series: handle created with history = 0");
+  const int64_t have = c->steps_done + 1;                  // levels 0 .. steps_done
+  if (first + n > have || first < have - c->hist_cap)
+    return fail(c, RT_EINVAL, "rt_get_dipole_series: requested levels are not in the history window");
+  CK(cudaSetDevice(c->cfg.device));
+  for (int32_t i = 0; i < n;) {                            // at most two contiguous pieces of the ring
+    const int64_t slot = (first + i) % c->hist_cap;
+    int32_t run = (int32_t)((c->hist_cap - slot < n - i) ? (c->hist_cap - slot) : (n - i));
+    CK(cudaMemcpyAsync(out + (size_t)i * 4, c->d_hist + slot * 4, (size_t)run * 32, cudaMemcpyDeviceToHost, c->st));
+    i += run;
+  }
+  return sync_and_check(c);
 }
 
 int rt_get_convergence(rt_handle c, int32_t n[2], double err[2]) {
@@ -1116,6 +1153,7 @@ int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
       CK(cudaMemcpyAsync(c->H0, c->H1, nn, cudaMemcpyDeviceToDevice, c->st));
       CK(cudaMemcpyAsync(c->Hm1, c->H1, nn, cudaMemcpyDeviceToDevice, c->st));
       CK(cudaMemsetAsync(c->d_sums + 4, 0, 8, c->st));       // induced charge at t = 0
+      enqueue_record(c);                                     // time level 0
       c->slab_state = 1;
       break;
     case RT_SLAB_PROPAGATE:
@@ -1131,11 +1169,44 @@ int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
       if (c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
       enqueue_shift(c);
       c->t += c->dt;
+      c->steps_done += 1;
       break;
     default:
       return fail(c, RT_EINVAL, "rt_slab_phase: unknown phase");
   }
   CK(cudaGetLastError());
+  return RT_OK;
+}
+
+int rt_spectrum(const double* mu, int32_t nt, double dt, double t_kick, const double kappa[3], double gamma,
+                const double* omega, int32_t nw, double* S, int32_t device, void* stream) {
+  rt_ctx* c = nullptr;
+  if (!mu || !kappa || !omega || !S || nt < 2 || nw < 0 || !(dt > 0.0) || !(gamma >= 0.0))
+    return fail(c, RT_EINVAL, "rt_spectrum: bad argument");
+  int nused = 0;
+  for (int q = 0; q < 3; ++q) nused += kappa[q] != 0.0;
+  if (!nused) return fail(c, RT_EINVAL, "rt_spectrum: every kappa is zero");
+  if (nw == 0) return RT_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  cudaError_t e = cudaSetDevice(device);
+  double *d_mu = nullptr, *d_w = nullptr, *d_S = nullptr;
+  auto is_dev = [](const void* p) {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return pa.type == cudaMemoryTypeDevice || pa.type == cudaMemoryTypeManaged;
+  };
+  const bool mu_dev = is_dev(mu), w_dev = is_dev(omega), S_dev = is_dev(S);
+  if (e == cudaSuccess && !mu_dev) { e = cudaMalloc(&d_mu, (size_t)3 * nt * 8); if (e == cudaSuccess) e = cudaMemcpyAsync(d_mu, mu, (size_t)3 * nt * 8, cudaMemcpyHostToDevice, st); }
+  if (e == cudaSuccess && !w_dev) { e = cudaMalloc(&d_w, (size_t)nw * 8); if (e == cudaSuccess) e = cudaMemcpyAsync(d_w, omega, (size_t)nw * 8, cudaMemcpyHostToDevice, st); }
+  if (e == cudaSuccess && !S_dev) e = cudaMalloc(&d_S, (size_t)nw * 8);
+  if (e == cudaSuccess) {
+    launch_spectrum(mu_dev ? mu : d_mu, nt, dt, t_kick, kappa, nused, gamma, w_dev ? omega : d_w, nw, S_dev ? S : d_S, st);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess && !S_dev) e = cudaMemcpyAsync(S, d_S, (size_t)nw * 8, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_mu); cudaFree(d_w); cudaFree(d_S);
+  if (e != cudaSuccess) { cudaGetLastError(); return fail(c, RT_ECUDA, std::string("rt_spectrum: ") + cudaGetErrorString(e)); }
   return RT_OK;
 }
 

@@ -142,6 +142,13 @@ void launch_commutator_check(int N, int ldn, const double* dPr, const double* dP
 // cs->H_bits = max |A - B| over the N x N matrices (line 24)
 void launch_maxabs_diff(int N, int ldn, const double* A, const double* B, ConvState* cs, cudaStream_t st);
 
+// dipole history: hist[(count % cap)][4] = { dvol sums[1..3], dvol sums[0] }; count += 1   (one thread)
+void launch_record_dipole(const double* sums, double dvol, double* hist, int cap, unsigned long long* count,
+                          cudaStream_t st);
+// S[iw] per the formula in include/rt_tddft.h (rt_spectrum); one warp per frequency, fixed summation order
+void launch_spectrum(const double* mu, int nt, double dt, double t_kick, const double* kappa3, int nused, double gamma,
+                     const double* omega, int nw, double* S, cudaStream_t st);
+
 struct MgLevel {
   GridDims gd; double h; long long n;
   double* u; double* tmp; double* f; double* r;     // solution, ping-pong scratch, rhs, residual

@@ -38,6 +38,7 @@ def test_config_struct_layout(built):
     assert binding.rt_config.dP_thrs.offset == 120 and binding.rt_config.H_thrs.offset == 128
     assert binding.rt_config.max_hupdates.offset == 136
     assert binding.rt_config.slab_x0.offset == 140 and binding.rt_config.slab_nx.offset == 144
+    assert binding.rt_config.history.offset == 148
 
 
 def test_no_cpu_fallback(built):

@@ -425,3 +425,65 @@ def test_dynamic_hamiltonian_loop(tiny_inputs):
     assert first == sorted(first) and first[-1] > first[0]
     assert later == sorted(later) and later[-1] > later[0]
     assert all(b <= a for a, b in zip(first, later))
+
+
+# ------------------------------------------------------------------ photoabsorption spectrum (R16)
+def test_dipole_strength_matches_geometric_series():
+    """mu_n = B + A sin(w0 n dt): the damped trapezoid transform is a pair of geometric series with a closed form."""
+    dt, nt, w0, A, B, kappa, gamma = 0.2, 257, 0.37, -3.1e-4, 0.8, 2.5e-4, 0.02
+    n = np.arange(nt)
+    mu = np.zeros((3, nt))
+    mu[1] = B + A * np.sin(w0 * n * dt)
+    omega = np.linspace(0.05, 1.0, 23)
+    S = O.dipole_strength(mu, dt, 0.0, (0.0, kappa, 0.0), gamma, omega)
+
+    def trap_geom(z):                       # sum_{n=0}^{nt-1} c_n z^n with c_0 = c_{nt-1} = 1/2
+        return (1 - z ** nt) / (1 - z) - 0.5 * (1 + z ** (nt - 1))
+
+    for w, s in zip(omega, S):
+        z1, z2 = np.exp((1j * (w + w0) - gamma) * dt), np.exp((1j * (w - w0) - gamma) * dt)
+        ft = A * dt * (trap_geom(z1) - trap_geom(z2)) / 2j
+        assert abs(s - (-(2 * w / np.pi) * ft.imag / kappa)) < 1e-12 * np.max(np.abs(S))
+
+
+def test_dipole_strength_integrates_to_the_oscillator_strength():
+    """Textbook normalisation: dmu(t) = -kappa (f/w0) sin(w0 t)  <=>  S(w) = f delta(w - w0); with damping a Lorentzian
+    f (gamma/pi) / ((w - w0)^2 + gamma^2) whose peak is f/(pi gamma) and whose integral is f."""
+    dt, nt, w0, f, kappa, gamma = 0.05, 40001, 0.5, 1.7, 1e-3, 0.004
+    t = np.arange(nt) * dt
+    mu = np.zeros((3, nt))
+    for q in range(3):
+        mu[q] = 0.3 * q - kappa * (f / w0) * np.sin(w0 * t)
+    omega = np.linspace(0.3, 0.7, 801)
+    S = O.dipole_strength(mu, dt, 0.0, (kappa,) * 3, gamma, omega)
+    assert abs(S[400] - f / (np.pi * gamma)) < 5e-3 * f / (np.pi * gamma)
+    lor = f * (gamma / np.pi) / ((omega - w0) ** 2 + gamma ** 2)
+    assert np.max(np.abs(S - lor)) < 5e-3 * np.max(lor)
+    assert abs(np.sum(0.5 * (S[1:] + S[:-1]) * np.diff(omega)) - f * (2 / np.pi) * np.arctan(0.2 / gamma)) < 5e-3 * f
+
+
+def test_spectrum_of_noninteracting_system_has_the_particle_hole_lines(tiny_inputs):
+    """Interactions off, weak kick along q: S(w) = (1/3) sum_q sum_{i occ, a virt} f_ia^q delta(w - (eps_a - eps_i)) with
+    f_ia^q = 2 occ_i (eps_a - eps_i) |M^q_ai|^2 (first-order response of P0 = diag(occ)).  Pins sign, 1/kappa with the
+    delivered impulse kappa = E dt / 2 and the effective kick time dt/2 of the end-point sampled kick (R5), and the
+    1/3 polarisation average, through the whole oracle step."""
+    w, Phi, eps, occ = tiny_inputs
+    E, nsteps, gamma = 1e-4, 200, 0.15
+    mu = np.zeros((3, nsteps + 1))
+    for q in range(3):
+        o = _make(tiny_inputs, E0=tuple(E * np.eye(3)[q]), hartree=False, xc=False)
+        mu[q, 0] = o.dipole()[q]
+        for n in range(nsteps):
+            o.step(1)
+            mu[q, n + 1] = o.dipole()[q]
+    omega = np.linspace(0.05, 1.1, 85)
+    S = O.dipole_strength(mu, w.dt, 0.5 * w.dt, (0.5 * E * w.dt,) * 3, gamma, omega)
+    ref = np.zeros_like(omega)
+    for q in range(3):
+        M = O.project(Phi, O.field_potential(w.shape, w.h, np.eye(3)[q]), w.dvol)
+        for i in np.nonzero(occ > 0)[0]:
+            for a in np.nonzero(occ == 0)[0]:
+                wn = eps[a] - eps[i]
+                f = 2.0 * occ[i] * wn * M[a, i] ** 2
+                ref += (2 * omega / np.pi) * f * np.imag(1.0 / (wn ** 2 + (gamma - 1j * omega) ** 2)) / 3.0
+    assert np.max(ref) > 0 and np.max(np.abs(S - ref)) < 0.03 * np.max(ref)
