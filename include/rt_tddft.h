@@ -120,6 +120,11 @@ int rt_get_dipole_series(rt_handle h, int64_t first, int32_t n, double* out);
 int rt_get_pmatrix(rt_handle h, double* re, double* im);
 /* H0 (the Hamiltonian at the current time, [norb][norb], EITHER).  Synchronises. */
 int rt_get_hmatrix(rt_handle h, double* H0);
+/* Energy diagnostic (HOST double): E = sum_i eps_i Re P_ii + dVol sum_r [1/2 drho V_H + e_xc(rho) - e_xc(rho0)
+ * - v_xc(rho0) drho + E(t_next).r drho] with the current (fixed-cycle) V_H; its derivative with respect to rho is the dV
+ * of the step, so it is conserved once the field is off ("conservation of energy", Figs. 3-4).
+ * Three small kernels; synchronises. */
+int rt_get_energy(rt_handle h, double* energy);
 /* Warm-start Hartree potential V_H[Ng] (EITHER).  Synchronises. */
 int rt_get_vhartree(rt_handle h, double* vh);
 /* Current time t (HOST). */

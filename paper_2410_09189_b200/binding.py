@@ -27,7 +27,7 @@ SYMBOLS = (
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
-    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum",
+    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum", "rt_get_energy",
 )
 
 RT_SLAB_INIT, RT_SLAB_PROPAGATE, RT_SLAB_POTENTIAL, RT_SLAB_SHIFT = 0, 1, 2, 3
@@ -82,7 +82,7 @@ def _load():
         "rt_op_propagate": [vp, dp, dp, dp, dp, dp], "rt_op_hartree": [vp, dp, dp, i32], "rt_op_vxc": [vp, dp, dp],
         "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp], "rt_get_convergence": [vp, dp, dp],
         "rt_slab_get_buffers": [vp, C.POINTER(rt_slab_buffers)], "rt_slab_phase": [vp, i32, i32],
-        "rt_get_dipole_series": [vp, C.c_int64, i32, dp],
+        "rt_get_dipole_series": [vp, C.c_int64, i32, dp], "rt_get_energy": [vp, C.POINTER(C.c_double)],
         "rt_spectrum": [dp, i32, C.c_double, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
     }
     for name, argtypes in sig.items():
@@ -250,6 +250,12 @@ def rt_probe_fp64_peak(device=0):
     return a.value, b.value
 
 
+def rt_get_energy(h) -> float:
+    e = C.c_double()
+    _check(h, _lib.rt_get_energy(h, C.byref(e)))
+    return e.value
+
+
 def rt_get_dipole_series(h, first: int, n: int) -> np.ndarray:
     """[n][4]: mu_x, mu_y, mu_z, charge of the time levels first .. first + n - 1 (level 0 is t = 0)."""
     out = np.zeros((int(n), 4))
@@ -356,6 +362,9 @@ class RTTDDFT:
         if n is None:
             n = int(round(self.time / self._dt)) + 1 - int(first)
         return rt_get_dipole_series(self.handle, first, n)
+
+    def energy(self):
+        return rt_get_energy(self.handle)
 
     def pmatrix(self):
         re, im = np.empty((self.norb, self.norb)), np.empty((self.norb, self.norb))

@@ -172,6 +172,18 @@ __device__ __forceinline__ double vxc_pz81(double rho) {
   return vx + vc;
 }
 
+// e_xc(rho) = rho (eps_x + eps_c) per unit volume, eps_x = 3/4 v_x (energy diagnostic only)
+__device__ __forceinline__ double exc_pz81(double rho) {
+  if (!(rho >= 1e-30)) return 0.0;
+  const double PI = 3.14159265358979323846;
+  const double ex = -0.75 * cbrt(3.0 * rho / PI);
+  const double rs = cbrt(3.0 / (4.0 * PI * rho));
+  double ec;
+  if (rho <= 3.0 / (4.0 * PI)) ec = -0.1423 / (1.0 + 1.0529 * sqrt(rs) + 0.3334 * rs);
+  else { const double ln = log(rs); ec = 0.0311 * ln + -0.048 + 0.0020 * rs * ln + -0.0116 * rs; }
+  return rho * (ex + ec);
+}
+
 __device__ __forceinline__ double field_at(long long r, GridDims gd, double h, const double* __restrict__ E) {
   const long long nyz = (long long)gd.ny * gd.nz;
   const int ix = (int)(r / nyz);
@@ -202,6 +214,43 @@ __global__ void __launch_bounds__(RB)
 field_kernel(long long Ng, GridDims gd, double h, const double* __restrict__ E, double* __restrict__ w) {
   const long long r = (long long)blockIdx.x * RB + threadIdx.x;
   if (r < Ng) w[r] = field_at(r, gd, h, E);
+}
+
+// Energy diagnostic (conserved after the kick; Figs. 3-4):
+//   E = sum_i eps_i Re P_ii + dVol sum_r [ 1/2 drho V_H + e_xc(rho) - e_xc(rho0) - vxc0 drho + E.r drho ]
+__global__ void __launch_bounds__(RB)
+energy_kernel(long long Ng, GridDims gd, double h, const double* __restrict__ rho, const double* __restrict__ rho0,
+              const double* __restrict__ vxc0, const double* __restrict__ VH, const double* __restrict__ E, int use_h,
+              int use_xc, double* __restrict__ bsums) {
+  __shared__ double sh[RB / 32][5];
+  double v[5] = {0, 0, 0, 0, 0};
+  for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < Ng; r += (long long)gridDim.x * RB) {
+    const double d = rho[r] - rho0[r];
+    double e = field_at(r, gd, h, E) * d;
+    if (use_h) e += 0.5 * d * VH[r];
+    if (use_xc) e += exc_pz81(rho[r]) - exc_pz81(rho0[r]) - vxc0[r] * d;
+    v[0] += e;
+  }
+  block_sum<5>(v, sh);
+  if (threadIdx.x == 0)
+#pragma unroll
+    for (int q = 0; q < 5; ++q) bsums[blockIdx.x * 5 + q] = v[q];
+}
+__global__ void trace_eps_kernel(int N, int ldn, const double* __restrict__ eps, const double* __restrict__ P,
+                                 double* __restrict__ out) {
+  __shared__ double sh[32][5];
+  double v[5] = {0, 0, 0, 0, 0};
+  for (int i = threadIdx.x; i < N; i += blockDim.x) v[0] += eps[i] * P[(long long)i * ldn + i];
+  block_sum<5>(v, sh);
+  if (threadIdx.x == 0) out[5] = v[0];
+}
+void launch_energy(long long Ng, GridDims gd, double h, const double* rho, const double* rho0, const double* vxc0,
+                   const double* VH, const double* E, int use_h, int use_xc, int N, int ldn, const double* eps,
+                   const double* P0r, double* bsums, double* out, cudaStream_t st) {
+  const int nb = reduce_rho_blocks(Ng);
+  energy_kernel<<<nb, RB, 0, st>>>(Ng, gd, h, rho, rho0, vxc0, VH, E, use_h, use_xc, bsums);
+  final_sums_kernel<<<1, 32 * 5, 0, st>>>(bsums, nb, 5, out);          // out[0] = grid part (without dVol)
+  trace_eps_kernel<<<1, 1024, 0, st>>>(N, ldn, eps, P0r, out);          // out[5] = sum_i eps_i P_ii
 }
 
 static inline unsigned nblk(long long n) { return (unsigned)((n + RB - 1) / RB); }

@@ -24,7 +24,7 @@ namespace rt {
 
 namespace {
 
-constexpr int MG_THREADS = 256;          // tile kernels
+constexpr int MG_THREADS = 512;          // tile kernels
 constexpr int CL_THREADS = 1024;         // cluster kernel, per CTA
 constexpr int CL_SIZE = 8;               // CTAs per cluster (portable maximum)
 

@@ -51,7 +51,7 @@ struct rt_ctx {
   std::vector<void*> allocs;
 
   // N-vectors / scalars
-  double *d_eps = nullptr, *d_occ = nullptr, *d_E = nullptr, *d_sums = nullptr, *d_bsums = nullptr;
+  double *d_eps = nullptr, *d_occ = nullptr, *d_E = nullptr, *d_sums = nullptr, *d_bsums = nullptr, *d_energy = nullptr;
   // N x N (ld = ldn)
   double *Hm1 = nullptr, *H0 = nullptr, *H1 = nullptr, *X = nullptr, *Ya = nullptr, *Yb = nullptr, *Yc = nullptr,
          *Cm = nullptr, *Sc = nullptr, *Sm = nullptr, *P0r = nullptr, *P0i = nullptr, *P1r = nullptr, *P1i = nullptr,
@@ -711,7 +711,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     if (e != 0) FAIL_CREATE(RT_ECUDA, std::string("init_tma_kernels: ") + cudaGetErrorString((cudaError_t)e));
   }
   const size_t nn = (size_t)N * ldn;
-  ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8);
+  ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8); ALLOC(c->d_energy, 8);
   c->hist_cap = cfg->history;
   if (c->hist_cap) {
     ALLOC(c->d_hist, (size_t)c->hist_cap * 4);
@@ -963,6 +963,21 @@ int rt_get_density(rt_handle c, double* rho) {
   CK(cudaSetDevice(c->cfg.device));
   CK(cudaMemcpyAsync(rho, c->rho, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
   return sync_and_check(c);
+}
+
+int rt_get_energy(rt_handle c, double* energy) {
+  CHECK_HANDLE(c);
+  if (!energy) return fail(c, RT_EINVAL, "rt_get_energy: NULL");
+  if (c->slab && c->slab_state != 1) return fail(c, RT_ESTATE, "rt_get_energy: RT_SLAB_INIT has not run");
+  CK(cudaSetDevice(c->cfg.device));
+  launch_energy(c->Ng, c->gd, c->h, c->rho, c->rho0, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->N, c->ldn,
+                c->d_eps, c->P0r, c->d_bsums, c->d_energy, c->st);
+  c->launches += 3;
+  double out[8];
+  CK(cudaMemcpyAsync(out, c->d_energy, sizeof out, cudaMemcpyDeviceToHost, c->st));
+  if (int rc = sync_and_check(c)) return rc;
+  *energy = out[5] + c->dvol * out[0];
+  return RT_OK;
 }
 
 int rt_get_vhartree(rt_handle c, double* vh) {

@@ -142,6 +142,10 @@ void launch_commutator_check(int N, int ldn, const double* dPr, const double* dP
 // cs->H_bits = max |A - B| over the N x N matrices (line 24)
 void launch_maxabs_diff(int N, int ldn, const double* A, const double* B, ConvState* cs, cudaStream_t st);
 
+// energy diagnostic: out[0] = sum_r [1/2 drho VH + exc(rho) - exc(rho0) - vxc0 drho + E.r drho], out[5] = sum_i eps_i P_ii
+void launch_energy(long long Ng, GridDims gd, double h, const double* rho, const double* rho0, const double* vxc0,
+                   const double* VH, const double* E, int use_h, int use_xc, int N, int ldn, const double* eps,
+                   const double* P0r, double* bsums, double* out, cudaStream_t st);
 // dipole history: hist[(count % cap)][4] = { dvol sums[1..3], dvol sums[0] }; count += 1   (one thread)
 void launch_record_dipole(const double* sums, double dvol, double* hist, int cap, unsigned long long* count,
                           cudaStream_t st);

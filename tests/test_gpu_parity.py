@@ -307,3 +307,24 @@ def test_zero_steps_and_initial_state(B):
     info = gpu.info()
     assert info["mg_levels"] == 4 and info["coarsest"] == (3, 3, 3) and info["launches_per_step"] > 0
     gpu.close()
+
+
+def test_energy_diagnostic_matches_oracle_and_is_conserved(B):
+    """rt_get_energy against the oracle's energy() along a strong-kick trajectory, then conservation on the GPU over a
+    run far longer than the oracle could follow in a test (Figs. 3-4: "no observable energy drift")."""
+    w = strong_kick(WORKLOADS["tiny"], 0.1)
+    Phi, eps, occ = inputs("tiny")[1:]
+    gpu, cpu = make_pair(B, w, Phi, eps, occ, n_vcycles=6)
+    assert abs(gpu.energy() - cpu.energy()) < 1e-11 * abs(cpu.energy())
+    for _ in range(6):
+        gpu.step(1)
+        cpu.step(1)
+        assert abs(gpu.energy() - cpu.energy()) < 1e-11 * abs(cpu.energy())
+    e1 = gpu.energy()
+    assert abs(e1 - np.sum(eps * occ)) > 1e-6                    # the kick deposited energy (3e-6 Ha)
+    worst = 0.0
+    for _ in range(20):
+        gpu.step(100)
+        worst = max(worst, abs(gpu.energy() - e1))
+    assert worst < 2e-9, worst                                   # 2,000 steps, m = 2, 6 V-cycles per solve
+    gpu.close()
