@@ -100,7 +100,7 @@ project_kernel(const double* __restrict__ phi, const double* __restrict__ w, con
 }
 
 __global__ void project_reduce_kernel(const double* __restrict__ W, const double* __restrict__ eps, double scale,
-                                      double* __restrict__ H, int N, int ldn, int S, int Sd) {
+                                      double* __restrict__ H, int N, int ldn, int S, int Sn, int Sd, int narrow_tile) {
   // one thread per (i, j) with j >= i; fixed summation order over the splits
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int i = blockIdx.y;
@@ -108,7 +108,8 @@ __global__ void project_reduce_kernel(const double* __restrict__ W, const double
   const long long slab = (long long)N * ldn;
   const double* p = W + (long long)i * ldn + j;
   double sum = 0.0;
-  const int ns = (i / TILE == j / TILE) ? Sd : S;        // diagonal tiles have their own split count
+  // diagonal tiles and the tiles of a narrow last column have their own split counts (ProjectPlan)
+  const int ns = (i / TILE == j / TILE) ? Sd : (j / TILE == narrow_tile ? Sn : S);
   for (int s = 0; s < ns; ++s) sum += p[(long long)s * slab];
   double v = scale * sum;
   if (i == j && eps) v += eps[i];
@@ -131,7 +132,7 @@ void launch_project(const ProjectPlan& p, const double* phi, const double* w, co
 void launch_project_reduce(const ProjectPlan& p, const double* W, const double* eps, double scale, double* H,
                            cudaStream_t st) {
   dim3 grid((p.N + 127) / 128, p.N);
-  project_reduce_kernel<<<grid, 128, 0, st>>>(W, eps, scale, H, p.N, p.ldn, p.S, p.Sd);
+  project_reduce_kernel<<<grid, 128, 0, st>>>(W, eps, scale, H, p.N, p.ldn, p.S, p.Sn, p.Sd, p.Tn > 0 ? p.ntile - 1 : -1);
 }
 
 // ======================================================================================================

@@ -610,15 +610,17 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   {
     ProjectPlan& p = c->pp;
     p.N = N; p.Ng = Ng; p.ntile = ntile; p.T = ntile * (ntile + 1) / 2; p.ldn = ldn;
-    p.Toff = ntile * (ntile - 1) / 2;
-    // Split-K factors.  One CTA per SM, CTAs handed out in block order: the plan is the (S, Sd) whose greedy schedule
-    // on `sms` machines finishes first.  Cost model in pipeline stages (16 grid points of one 128 x 128 tile): an
-    // off-diagonal CTA costs kchunk/16, a diagonal one diag_cost * kchunk_d/16 (the TMA kernel issues 160 of the 256
-    // 8 x 8 blocks of a diagonal tile; measured ~0.65), plus a fixed prologue/epilogue per CTA and a term per split for
-    // the second-stage reduction.  (Wave quantisation was 14 % of the first nano profile at S = 2.)
+    // Split-K factors.  One CTA per SM, CTAs handed out in block order: the plan is the (S, Sn, Sd) whose greedy
+    // schedule on `sms` machines finishes first.  Cost model in pipeline stages (16 grid points of one 128 x 128 tile): a
+    // full CTA costs kchunk/16, a narrow one 0.78 and a diagonal one 0.65 of that per stage (TMA kernel; measured), plus
+    // a fixed prologue/epilogue per CTA and a term per split for the second-stage reduction.  (Wave quantisation was
+    // 14 % of the first nano profile at S = 2.)
     const int sms = prop.multiProcessorCount;
     const bool tma_likely = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && get_encode_fn() != nullptr;
-    const double diag_cost = tma_likely ? 0.65 : 1.0;
+    const bool narrow = tma_likely && ntile > 1 && (N - (ntile - 1) * TILE) <= 96;
+    p.Tn = narrow ? ntile - 1 : 0;
+    p.Tfull = ntile * (ntile - 1) / 2 - p.Tn;
+    const double cost_n = 0.78, cost_d = tma_likely ? 0.65 : 1.0;
     // one stage ~ 2.1 us on one SM; the reduction reads one N x ldn slab per split at ~3 TB/s
     const double cta_ovh = 8.0, split_ovh = (double)N * ldn * 8.0 / 3.0e12 / 2.1e-6;
     const long long kmin = 16 * 8;
@@ -627,33 +629,45 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     const double slab_bytes = (double)N * ldn * 8;
     while (smax > 1 && smax * slab_bytes > 2.0e9) --smax;          // workspace cap
     auto chunk_of = [&](long long S_) { long long kc = (Ng + S_ - 1) / S_; return (kc + 15) / 16 * 16; };
-    auto makespan = [&](long long n1, double c1, long long n2, double c2) {
+    auto makespan = [&](const long long (&n)[3], const double (&cst)[3]) {
       std::priority_queue<double, std::vector<double>, std::greater<double>> q;
       for (int i = 0; i < sms; ++i) q.push(0.0);
       double end = 0.0;
-      for (long long j = 0; j < n1 + n2; ++j) {
-        const double t = q.top() + (j < n1 ? c1 : c2);
-        q.pop();
-        q.push(t);
-        if (t > end) end = t;
-      }
+      for (int cls = 0; cls < 3; ++cls)
+        for (long long j = 0; j < n[cls]; ++j) {
+          const double t = q.top() + cst[cls];
+          q.pop();
+          q.push(t);
+          if (t > end) end = t;
+        }
       return end;
     };
     double best = 1e300;
-    p.S = p.Sd = 1;
-    p.kchunk = p.kchunk_d = chunk_of(1);
+    p.S = p.Sn = p.Sd = 1;
+    p.kchunk = p.kchunk_n = p.kchunk_d = chunk_of(1);
     for (long long s = 1; s <= smax; ++s) {
       const long long kc = chunk_of(s);
       const long long S_ = (Ng + kc - 1) / kc;
       if (S_ != s) continue;                                       // same chunk as a smaller s
-      const long long sd0 = (long long)std::llround(diag_cost * (double)s);
-      for (long long sd = sd0 - 1; sd <= sd0 + 1; ++sd) {
-        if (sd < 1 || sd > s) continue;
-        const long long kd = chunk_of(sd);
-        const long long Sd_ = (Ng + kd - 1) / kd;
-        const double obj = makespan(S_ * p.Toff, kc / 16.0 + cta_ovh, Sd_ * ntile, diag_cost * kd / 16.0 + cta_ovh) +
-                           split_ovh * (double)(p.Toff > 0 ? S_ : Sd_);
-        if (obj < best - 1e-9) { best = obj; p.S = (int)S_; p.kchunk = kc; p.Sd = (int)Sd_; p.kchunk_d = kd; }
+      const long long sn0 = p.Tn ? (long long)std::llround(cost_n * (double)s) : 1;
+      const long long sd0 = (long long)std::llround(cost_d * (double)s);
+      for (long long sn = sn0 - 1; sn <= sn0 + 1; ++sn) {
+        if (sn < 1 || sn > s || (!p.Tn && sn != sn0)) continue;
+        const long long kn = chunk_of(sn);
+        const long long Sn_ = (Ng + kn - 1) / kn;
+        for (long long sd = sd0 - 1; sd <= sd0 + 1; ++sd) {
+          if (sd < 1 || sd > s) continue;
+          const long long kd = chunk_of(sd);
+          const long long Sd_ = (Ng + kd - 1) / kd;
+          const long long cnt[3] = {S_ * p.Tfull, Sn_ * p.Tn, Sd_ * ntile};
+          const double cst[3] = {kc / 16.0 + cta_ovh, cost_n * kn / 16.0 + cta_ovh, cost_d * kd / 16.0 + cta_ovh};
+          const long long smost = p.Tfull > 0 ? S_ : (p.Tn > 0 ? Sn_ : Sd_);
+          const double obj = makespan(cnt, cst) + split_ovh * (double)smost;
+          if (obj < best - 1e-9) {
+            best = obj;
+            p.S = (int)S_; p.kchunk = kc; p.Sn = (int)Sn_; p.kchunk_n = kn; p.Sd = (int)Sd_; p.kchunk_d = kd;
+          }
+        }
       }
     }
     DensityPlan& d = c->dp;
@@ -744,8 +758,12 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   }
   {
     std::vector<int2> tiles;
-    for (int ti = 0; ti < ntile; ++ti)                    // off-diagonal tiles first, then the diagonal (ProjectPlan)
-      for (int tj = ti + 1; tj < ntile; ++tj) tiles.push_back(make_int2(ti, tj));
+    // full off-diagonal tiles, then the narrow last column (if any), then the diagonal (ProjectPlan)
+    const int tj_end = c->pp.Tn > 0 ? ntile - 1 : ntile;
+    for (int ti = 0; ti < ntile; ++ti)
+      for (int tj = ti + 1; tj < tj_end; ++tj) tiles.push_back(make_int2(ti, tj));
+    if (c->pp.Tn > 0)
+      for (int ti = 0; ti < ntile - 1; ++ti) tiles.push_back(make_int2(ti, ntile - 1));
     for (int ti = 0; ti < ntile; ++ti) tiles.push_back(make_int2(ti, ti));
     ALLOC(c->d_tiles, tiles.size());
     CKC(cudaMemcpyAsync(c->d_tiles, tiles.data(), tiles.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
