@@ -114,6 +114,17 @@ int rt_get_density(rt_handle h, double* rho);
  * older or future ones).  Synchronises the stream once, however many steps were enqueued. */
 int rt_get_dipole_series(rt_handle h, int64_t first, int32_t n, double* out);
 
+/* ---- checkpoint / resume ---------------------------------------------------------------------------
+ * The propagation state of Algorithm 1 between two steps: t, P0 (re, im), H0, H-1 (line 28), the warm-start V_H, the
+ * field E(t_next), rho and its five sums -- (4 norb^2 + 2 Ng + 16) doubles plus a 64-byte header; Phi, eps, occ and the
+ * configuration are NOT part of it (the caller owns them).  A run restored into a handle created with the same
+ * configuration continues bit-identically.  buf: HOST memory of rt_state_bytes() bytes.  Both calls synchronise.
+ * rt_set_state returns RT_EINVAL when the header does not match the handle (norb, grid, dt) and leaves it untouched.
+ * The dipole history (rt_config.history) restarts at the restored time level. */
+int rt_state_bytes(rt_handle h, int64_t* nbytes);
+int rt_get_state(rt_handle h, void* buf);
+int rt_set_state(rt_handle h, const void* buf);
+
 /* ---- diagnostics / test aids ------------------------------------------------------------------ */
 
 /* P(t) = re + i im, each [norb][norb] (EITHER; either pointer may be NULL).  Synchronises. */

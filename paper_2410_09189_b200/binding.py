@@ -27,7 +27,7 @@ SYMBOLS = (
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
-    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum", "rt_get_energy",
+    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum", "rt_get_energy", "rt_state_bytes", "rt_get_state", "rt_set_state",
 )
 
 RT_SLAB_INIT, RT_SLAB_PROPAGATE, RT_SLAB_POTENTIAL, RT_SLAB_SHIFT = 0, 1, 2, 3
@@ -83,6 +83,7 @@ def _load():
         "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp], "rt_get_convergence": [vp, dp, dp],
         "rt_slab_get_buffers": [vp, C.POINTER(rt_slab_buffers)], "rt_slab_phase": [vp, i32, i32],
         "rt_get_dipole_series": [vp, C.c_int64, i32, dp], "rt_get_energy": [vp, C.POINTER(C.c_double)],
+        "rt_state_bytes": [vp, i64p], "rt_get_state": [vp, vp], "rt_set_state": [vp, vp],
         "rt_spectrum": [dp, i32, C.c_double, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
     }
     for name, argtypes in sig.items():
@@ -250,6 +251,24 @@ def rt_probe_fp64_peak(device=0):
     return a.value, b.value
 
 
+def rt_get_state(h) -> np.ndarray:
+    """Checkpoint of the propagation state as a uint8 array (include/rt_tddft.h rt_get_state)."""
+    n = C.c_int64()
+    _check(h, _lib.rt_state_bytes(h, C.byref(n)))
+    buf = np.zeros(n.value, dtype=np.uint8)
+    _check(h, _lib.rt_get_state(h, buf.ctypes.data))
+    return buf
+
+
+def rt_set_state(h, buf: np.ndarray):
+    buf = np.ascontiguousarray(buf, dtype=np.uint8)
+    n = C.c_int64()
+    _check(h, _lib.rt_state_bytes(h, C.byref(n)))
+    if buf.size != n.value:
+        raise RTError(RT_EINVAL, f"state buffer has {buf.size} bytes, the handle needs {n.value}")
+    _check(h, _lib.rt_set_state(h, buf.ctypes.data))
+
+
 def rt_get_energy(h) -> float:
     e = C.c_double()
     _check(h, _lib.rt_get_energy(h, C.byref(e)))
@@ -362,6 +381,12 @@ class RTTDDFT:
         if n is None:
             n = int(round(self.time / self._dt)) + 1 - int(first)
         return rt_get_dipole_series(self.handle, first, n)
+
+    def get_state(self):
+        return rt_get_state(self.handle)
+
+    def set_state(self, buf):
+        rt_set_state(self.handle, buf)
 
     def energy(self):
         return rt_get_energy(self.handle)

@@ -983,6 +983,74 @@ int rt_get_density(rt_handle c, double* rho) {
   return sync_and_check(c);
 }
 
+// ---- checkpoint / resume ---------------------------------------------------------------------------
+namespace {
+struct StateHeader { uint64_t magic; int32_t norb, nx, ny, nz; double dt, t; int64_t steps; int64_t ndoubles; };
+static_assert(sizeof(StateHeader) <= 64, "header must fit its 64-byte slot");
+constexpr uint64_t STATE_MAGIC = 0x3130455441545352ull;          // "RSTATE01"
+int64_t state_doubles(const rt_ctx* c) { return 4LL * c->N * c->N + 2LL * c->Ng + 16; }
+}  // namespace
+
+int rt_state_bytes(rt_handle c, int64_t* nbytes) {
+  CHECK_HANDLE(c);
+  if (!nbytes) return fail(c, RT_EINVAL, "rt_state_bytes: NULL");
+  *nbytes = 64 + 8 * state_doubles(c);
+  return RT_OK;
+}
+
+int rt_get_state(rt_handle c, void* buf) {
+  CHECK_HANDLE(c);
+  if (!buf) return fail(c, RT_EINVAL, "rt_get_state: NULL");
+  if (c->slab && c->slab_state != 1) return fail(c, RT_ESTATE, "rt_get_state: RT_SLAB_INIT has not run");
+  CK(cudaSetDevice(c->cfg.device));
+  StateHeader hd{STATE_MAGIC, c->N, c->gd.nx, c->gd.ny, c->gd.nz, c->dt, c->t, c->steps_done, state_doubles(c)};
+  memset(buf, 0, 64);
+  memcpy(buf, &hd, sizeof hd);
+  double* p = reinterpret_cast<double*>(static_cast<char*>(buf) + 64);
+  const size_t n2 = (size_t)c->N * c->N;
+  const double* mats[4] = {c->P0r, c->P0i, c->H0, c->Hm1};
+  for (int i = 0; i < 4; ++i)
+    if (int rc = copy_matrix_out(c, mats[i], p + i * n2)) return rc;
+  p += 4 * n2;
+  CK(cudaMemcpyAsync(p, c->lv[0].u, (size_t)c->Ng * 8, cudaMemcpyDeviceToHost, c->st));
+  CK(cudaMemcpyAsync(p + c->Ng, c->rho, (size_t)c->Ng * 8, cudaMemcpyDeviceToHost, c->st));
+  CK(cudaMemcpyAsync(p + 2 * c->Ng, c->d_sums, 8 * 8, cudaMemcpyDeviceToHost, c->st));
+  CK(cudaMemcpyAsync(p + 2 * c->Ng + 8, c->d_E, 8 * 8, cudaMemcpyDeviceToHost, c->st));
+  return sync_and_check(c);
+}
+
+int rt_set_state(rt_handle c, const void* buf) {
+  CHECK_HANDLE(c);
+  if (!buf) return fail(c, RT_EINVAL, "rt_set_state: NULL");
+  if (c->slab && c->slab_state != 1) return fail(c, RT_ESTATE, "rt_set_state: RT_SLAB_INIT has not run");
+  StateHeader hd;
+  memcpy(&hd, buf, sizeof hd);
+  if (hd.magic != STATE_MAGIC || hd.norb != c->N || hd.nx != c->gd.nx || hd.ny != c->gd.ny || hd.nz != c->gd.nz ||
+      hd.dt != c->dt || hd.ndoubles != state_doubles(c))
+    return fail(c, RT_EINVAL, "rt_set_state: the buffer was not written by a handle with this norb / grid / dt");
+  CK(cudaSetDevice(c->cfg.device));
+  const double* p = reinterpret_cast<const double*>(static_cast<const char*>(buf) + 64);
+  const size_t n2 = (size_t)c->N * c->N;
+  double* mats[4] = {c->P0r, c->P0i, c->H0, c->Hm1};
+  for (int i = 0; i < 4; ++i)
+    if (int rc = copy_matrix_in(c, p + i * n2, mats[i])) return rc;
+  p += 4 * n2;
+  CK(cudaMemcpyAsync(c->lv[0].u, p, (size_t)c->Ng * 8, cudaMemcpyHostToDevice, c->st));
+  CK(cudaMemcpyAsync(c->rho, p + c->Ng, (size_t)c->Ng * 8, cudaMemcpyHostToDevice, c->st));
+  CK(cudaMemcpyAsync(c->d_sums, p + 2 * c->Ng, 8 * 8, cudaMemcpyHostToDevice, c->st));
+  CK(cudaMemcpyAsync(c->d_E, p + 2 * c->Ng + 8, 8 * 8, cudaMemcpyHostToDevice, c->st));
+  // H1 is rebuilt from H0 and H-1 by the first update of the next step (line 11); P1 by the propagation
+  c->t = hd.t;
+  c->steps_done = hd.steps;
+  if (c->hist_cap) {                                   // the history restarts at this level
+    const unsigned long long k = (unsigned long long)hd.steps;
+    CK(cudaMemcpyAsync(c->d_hist_n, &k, sizeof k, cudaMemcpyHostToDevice, c->st));
+    if (int rc = sync_and_check(c)) return rc;
+    enqueue_record(c);
+  }
+  return sync_and_check(c);
+}
+
 int rt_get_energy(rt_handle c, double* energy) {
   CHECK_HANDLE(c);
   if (!energy) return fail(c, RT_EINVAL, "rt_get_energy: NULL");

@@ -328,3 +328,32 @@ def test_energy_diagnostic_matches_oracle_and_is_conserved(B):
         worst = max(worst, abs(gpu.energy() - e1))
     assert worst < 2e-9, worst                                   # 2,000 steps, m = 2, 6 V-cycles per solve
     gpu.close()
+
+
+def test_checkpoint_resume_is_bit_identical(B):
+    """rt_get_state / rt_set_state: a run restored into a fresh handle continues exactly like the uninterrupted one."""
+    w = strong_kick(WORKLOADS["ragged"], 0.1)
+    Phi, eps, occ = inputs("ragged")[1:]
+    kw = dict(E0=w.kick, n_hupdates=w.n_hupdates, n_vcycles=w.n_vcycles, history=16)
+    a = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, **kw)
+    a.step(4)
+    state = a.get_state()
+    a.step(5)
+    b = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, **kw)
+    b.set_state(state)
+    assert abs(b.time - 4 * w.dt) < 1e-12
+    assert np.array_equal(b.dipole_series(4, 1)[0], a.dipole_series(4, 1)[0])
+    b.step(5)
+    assert np.array_equal(a.dipole(), b.dipole()) and np.array_equal(a.density(), b.density())
+    assert np.array_equal(a.pmatrix(), b.pmatrix()) and np.array_equal(a.hmatrix(), b.hmatrix())
+    assert np.array_equal(a.vhartree(), b.vhartree()) and a.time == b.time
+    assert np.array_equal(a.dipole_series(5, 5), b.dipole_series(5, 5))
+    # a buffer from a different system is refused and leaves the handle usable
+    w2 = WORKLOADS["tiny"]
+    Phi2, eps2, occ2 = inputs("tiny")[1:]
+    c = B.RTTDDFT(w2.shape, w2.h, Phi2, eps2, occ2, w2.dt)
+    with pytest.raises(B.RTError):
+        B._check(c.handle, B._lib.rt_set_state(c.handle, state.ctypes.data))
+    c.step(1)
+    for s in (a, b, c):
+        s.close()
