@@ -357,3 +357,30 @@ def test_checkpoint_resume_is_bit_identical(B):
     c.step(1)
     for s in (a, b, c):
         s.close()
+
+
+@pytest.mark.parametrize("norb", [130, 200, 225, 300, 384, 400])
+def test_projection_and_density_tile_classes(B, norb):
+    """Orbital counts that exercise every tile class of the a1 plan (full / narrow last column / diagonal; norb = 200 has
+    no full tile at all, 225 has a last column of 97 > 96 columns, 384 no ragged tile) and the masked diagonal blocks of
+    a5, against the oracle's plain contractions."""
+    shape, h = (16, 12, 20), 0.4
+    ng = shape[0] * shape[1] * shape[2]
+    rng = np.random.default_rng(100 + norb)
+    Phi = rng.standard_normal((norb, ng)) / np.sqrt(ng * h ** 3)
+    eps = np.sort(rng.uniform(-1.0, 0.5, norb))
+    occ = np.zeros(norb)
+    occ[: norb // 2] = 2.0
+    gpu = B.RTTDDFT(shape, h, Phi, eps, occ, 0.1)
+    v = rng.standard_normal(ng)
+    H = B.rt_op_project(gpu.handle, v, np.empty((norb, norb)))
+    ref = O.project(Phi, v, h ** 3)
+    assert np.max(np.abs(H - ref)) < 1e-12 * np.max(np.abs(ref))
+    assert np.array_equal(H, H.T)
+    S = rng.standard_normal((norb, norb))
+    S = S + S.T
+    rho = B.rt_op_density(gpu.handle, S, np.empty(ng))
+    rho = rho[0] if isinstance(rho, tuple) else rho
+    ref = O.density(Phi, S)
+    assert np.max(np.abs(rho - ref)) < 1e-12 * np.max(np.abs(ref))
+    gpu.close()
