@@ -158,11 +158,13 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
       if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
     }
   } else {
+    const bool live = i0 + wrow < N && j0 + wcol < N;
     for (int kt = 0; kt < nk; ++kt) {
       const int slot = kt % ST;
       mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
       const double* sA = tilesm + (size_t)slot * STAGE_D;
-      if (dlt >= 8) mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+      if (!live) {}                             // the whole warp tile is padding (N < 128: tiny systems)
+      else if (dlt >= 8) mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
       else if (dlt == 4) mma_stage_kc_tma<FA, FB, true, 6, 8>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
       else if (dlt == 0) mma_stage_kc_tma<FA, FB, true, 2, 4>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
       __syncwarp();
