@@ -4,10 +4,13 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config nano|24k|mid|small|tiny|...] [--impl reference]
 
 A "step" is one pass of the whole hot path (Algorithm 1 lines 10-28: m x [ELDYN, Rho, Vh, XC, Hupdate]) on one
-synthetic system.  Default workload: `nano` (128^3 grid, 2,400 orbitals, Phi = 40 GB
-resident), the largest config whose default run finishes within minutes; `--config 24k` runs the 13,000-orbital
-case.  N > 1 (torchrun): the path does not shard yet ("replicas only"): every rank propagates its own
-system, no data-path collective, value = all ranks' steps / max-over-ranks time, scaling = weak.
+synthetic system.  Default workload: `24k` (104^3 grid, 13,000 orbitals of which 12,000
+are occupied, Phi = 117 GB resident: the configuration north_star's metric is quoted on, shaped like the paper's
+Ag2160 row of Table 1); one step takes ~24 s, so the default `--steps 3 --warmup 3` run ends in
+a few minutes and the driver's `--steps 20 --warmup 5` in ~13.  `--config nano|mid|small|tiny` select the others.
+N > 1 (torchrun): ONE system cut into grid slabs over the ranks (the paper's own decomposition, L420-L424; DESIGN
+section 10): two NCCL all-reduces per Hamiltonian update, scaling = strong, value = the steps of that one system /
+max-over-ranks time.  `--parallel replicas` runs N independent systems instead (weak, no collective).
 
 `--impl reference` times the CPU oracle (oracle/rt_oracle.py, as it stands) on the host cores on a bounded sample
 of the same workload; rank 0 only.
@@ -83,21 +86,28 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ oracle sample
+EIGH_SAMPLE_N = 3000      # largest propagator the bounded oracle sample diagonalises in full (N = 13,000 takes minutes)
+
+
 def oracle_sample(w, slab_pts, phi_slab=None, seed=0):
     """One bounded sample of the oracle's work for workload `w`: returns a function that runs ONE Hamiltonian update
-    of oracle/rt_oracle.py on a grid slab of `slab_pts` points (all N orbitals) plus the full-size N x N propagator and
-    the full-grid Poisson / xc, and the factor by which the slab part must be scaled to the whole grid."""
+    of oracle/rt_oracle.py with (i) the density and the projection on a grid slab of `slab_pts` points (all N orbitals),
+    (ii) the exact-diagonalisation propagator on the leading n_s x n_s block, n_s = min(N, EIGH_SAMPLE_N), (iii) the
+    full-grid Poisson / xc; and the factors that EXTRAPOLATE (i) and (ii) to the whole workload (Ng/slab, (N/n_s)^3)."""
     from oracle import rt_oracle as O
+    from paper_2410_09189_b200.workloads import phi_slab_sample
     N, Ng = w.norb, w.ngrid
     rng = np.random.default_rng(seed)
     if phi_slab is None:
-        phi_slab = rng.standard_normal((N, slab_pts)) / math.sqrt(Ng * w.dvol)
+        phi_slab = phi_slab_sample(w, slab_pts)
+    ns = min(N, EIGH_SAMPLE_N)
     eps = np.sort(rng.uniform(w.eps_range[0], w.eps_range[1], N))
     occ = np.zeros(N)
     occ[: w.nocc] = 2.0
-    A = rng.standard_normal((N, N)) * 1e-4
-    Hbar = np.diag(eps) + 0.5 * (A + A.T)
-    P0 = np.diag(occ).astype(np.complex128)
+    A = rng.standard_normal((ns, ns)) * 1e-4
+    Hbar = np.diag(eps[:ns]) + 0.5 * (A + A.T)
+    P0 = np.diag(occ[:ns]).astype(np.complex128)
+    ReP = np.diag(occ)
     rho_full = np.abs(rng.standard_normal(Ng)) * (occ.sum() / (Ng * w.dvol))
     rho0_full = rho_full * (1 + 1e-6 * rng.standard_normal(Ng))
     vxc0 = O.vxc_lda(rho0_full)
@@ -105,9 +115,10 @@ def oracle_sample(w, slab_pts, phi_slab=None, seed=0):
 
     def parts():
         t0 = time.perf_counter()
-        P1 = O.propagate_eigh(Hbar, P0, w.dt)                       # ELDYN
+        P1 = O.propagate_eigh(Hbar, P0, w.dt)                       # ELDYN on the n_s block
         t1 = time.perf_counter()
-        rho_s = O.density(phi_slab, P1.real)                         # Rho on the slab
+        ReP[:ns, :ns] = P1.real
+        rho_s = O.density(phi_slab, ReP)                             # Rho on the slab
         t2 = time.perf_counter()
         vh = O.hartree_mg(VH, rho_full - rho0_full, w.shape, w.h, w.n_vcycles)     # Vh, full grid
         t3 = time.perf_counter()
@@ -117,13 +128,19 @@ def oracle_sample(w, slab_pts, phi_slab=None, seed=0):
         t5 = time.perf_counter()
         return {"ELDYN": t1 - t0, "Rho": t2 - t1, "Vh": t3 - t2, "XC": t4 - t3, "Hupdate": t5 - t4}, H1
 
-    return parts, Ng / slab_pts
+    return parts, {"grid": Ng / slab_pts, "eldyn": (N / ns) ** 3, "ns": ns}
 
 
 def oracle_step_seconds(w, parts, scale):
     t, _ = parts()
-    per_update = t["ELDYN"] + t["Vh"] + t["XC"] + scale * (t["Rho"] + t["Hupdate"])
+    per_update = scale["eldyn"] * t["ELDYN"] + t["Vh"] + t["XC"] + scale["grid"] * (t["Rho"] + t["Hupdate"])
     return w.n_hupdates * per_update, t
+
+
+def sample_text(w, pts, scale):
+    return (f"EXTRAPOLATED from a bounded sample: per step {w.n_hupdates} Hamiltonian updates, each = eigh propagator on "
+            f"the leading {scale['ns']}^2 block x {scale['eldyn']:.1f} + full-grid Poisson/xc + density & projection on a "
+            f"{pts}-point grid slab (all {w.norb} orbitals) x Ng/slab = {scale['grid']:.1f}")
 
 
 def full_oracle(w):
@@ -135,7 +152,7 @@ def full_oracle(w):
 
 
 def slab_points(w):
-    # ~10-30 s of CPU work: 4 N^2 slab flops per update at ~100 GFLOP/s -> a few seconds
+    # a few seconds of CPU work per sample: 4 N^2 slab flops per update at ~100 GFLOP/s
     pts = int(2.5e11 / (4.0 * w.norb * w.norb))
     pts = max(1024, min(w.ngrid, pts))
     return (pts // 1024) * 1024 if pts >= 1024 else pts
@@ -162,9 +179,7 @@ def run_reference(args, w):
     if big:
         pts = slab_points(w)
         parts, scale = oracle_sample(w, pts, seed=w.seed)
-        sample = (f"per step: {w.n_hupdates} Hamiltonian updates, each = full {w.norb}^2 eigh propagator + full-grid "
-                  f"Poisson/xc + density & projection on a {pts}-point grid slab (all {w.norb} orbitals), slab time "
-                  f"scaled by Ng/slab = {scale:.1f}")
+        sample = sample_text(w, pts, scale) + "; Phi slab = the workload generator's raw seeded draw for those points"
         for i in range(args.warmup + args.steps):
             sec, _ = oracle_step_seconds(w, parts, scale)
             if i >= args.warmup:
@@ -205,16 +220,18 @@ def workload_config(w, args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="nano")
+    ap.add_argument("--config", default="24k")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
-                    help="N > 1: replicas = one independent system per rank (weak scaling, no data-path collective; "
-                         "default); slabs = ONE system cut into grid slabs over the ranks (strong scaling, two NCCL "
-                         "all-reduces per Hamiltonian update; paper_2410_09189_b200/slab.py)")
+    ap.add_argument("--parallel", default=None, choices=["replicas", "slabs"],
+                    help="slabs (default for N > 1) = ONE system cut into grid slabs over the ranks (strong scaling, "
+                         "NCCL all-reduces per Hamiltonian update; paper_2410_09189_b200/slab.py); replicas = one "
+                         "independent system per rank (weak scaling, no data-path collective)")
     args = ap.parse_args()
+    if args.parallel is None:
+        args.parallel = "slabs" if args.gpus > 1 or int(os.environ.get("WORLD_SIZE", "1")) > 1 else "replicas"
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
 
     from paper_2410_09189_b200.workloads import WORKLOADS, make_inputs_device, make_inputs_numpy
@@ -339,8 +356,11 @@ def main():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
+        # a step of the two largest configs takes seconds: a quarter of the K steps (at least 3) is enough for the wall
+        # clock, and keeps the driver's --steps 20 run of the 24k config inside its time limit
+        e2e_steps = args.steps if ms_total / args.steps < 1000.0 else max(3, args.steps // 4)
         t0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(e2e_steps):
             E = w.E_of_t((step_no[0] + 1) * w.dt)
             e_host[0], e_host[1], e_host[2] = E
             B._check(sim.handle, B._lib.rt_set_field(sim.handle, e_host.data_ptr()))
@@ -349,7 +369,7 @@ def main():
             mu = sim.dipole()
             B.rt_get_density(sim.handle, rho_host)
         torch.cuda.synchronize()
-        e2e_sec = time.perf_counter() - t0
+        e2e_sec = (time.perf_counter() - t0) * args.steps / e2e_steps      # scaled to K steps for the max over ranks
         charge = B.rt_get_charge(sim.handle)
 
     ms_total, e2e_ms = replicas.max_over_ranks([ms_total, e2e_sec * 1e3], device=f"cuda:{local}")
@@ -373,7 +393,8 @@ def main():
            "ELDYN": ("tensor", ((info["exp_order"] // 2 + 1) + 12.0) * N ** 3,
                      "a3+a4 gemm_abt_tma_kernel: (q+1) symmetric-output series GEMMs (N^3 each) + U P U^dagger "
                      "(2 full dual GEMMs 8N^3 + Hermitian output 4N^3)"),
-           "Vh": ("hbm", 167.0 * w.ngrid * 8 / 7 * w.n_vcycles, "a7 V-cycles: 167 B/pt/cycle unfused x 8/7"),
+           "Vh": ("hbm", 57.0 * w.ngrid * w.n_vcycles, "a7 V-cycles: 57 B/pt/cycle (SURVEY 8d fused-ideal, coarse levels "
+                  "included); L2-resident and launch-latency-bound in practice"),
            "XC": ("hbm", 32.0 * w.ngrid, "a8 delta_v_kernel: 32 B/pt")}
     shares = {k: (stage_ms[k] / max(1, stage_calls[k])) for k in stage_ms}
     tot_stage = sum(stage_ms.values())
@@ -419,10 +440,8 @@ def main():
             parts, scale = oracle_sample(w, pts, phi_slab=slab, seed=w.seed)
             sec, t = oracle_step_seconds(w, parts, scale)
             cpu = {"value": 1.0 / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-                   "sample": (f"one Hamiltonian update of oracle/rt_oracle.py: full {N}^2 eigh propagator + full-grid "
-                              f"Poisson/xc + density & projection on the first {pts} grid points of the same Phi, slab "
-                              f"time x {scale:.1f}, x m = {w.n_hupdates}; measured parts (s): "
-                              + ", ".join(f"{k}={v:.2f}" for k, v in t.items()))}
+                   "sample": (sample_text(w, pts, scale) + "; Phi slab = the first grid points of the SAME Phi; "
+                              "measured parts (s): " + ", ".join(f"{k}={v:.2f}" for k, v in t.items()))}
         else:
             o = full_oracle(w)
             n = 0
@@ -440,7 +459,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if slabs else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(w, args), "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 24, "d2h_bytes_per_step": 24 + 8 * w.ngrid,
-                    "ms_per_step": e2e_ms / args.steps},
+                    "ms_per_step": e2e_ms / args.steps, "steps_timed": e2e_steps},
             "gpu_launches": int(launches), "roofline": roof, "per_kernel": per_kernel, "cpu_baseline": cpu,
             "fp64_peaks_tflops": {"dmma": peak_dmma, "dfma": peak_dfma}, "lib": info,
             "checks": {"ortho_err": ortho_err, "charge": float(charge[0]), "n_electrons": 2.0 * w.nocc,

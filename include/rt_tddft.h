@@ -42,6 +42,7 @@ extern "C" {
 #define RT_ENOMEM  -2   /* not enough device memory for the workspaces */
 #define RT_ECUDA   -3   /* CUDA runtime error (message in rt_last_error) */
 #define RT_ESTATE  -4   /* handle poisoned by an earlier error, or NULL */
+#define RT_ENUMERIC -5  /* non-finite value on the device, or a dynamic loop of Alg. 1 ran out of iterations */
 
 /* rt_config.flags */
 #define RT_PHI_DEVICE  1u   /* `phi` is a DEVICE pointer that the library BORROWS (never copies, never writes)
@@ -97,7 +98,10 @@ typedef struct {
  * eps, occ: [norb] HOST, copied; occ in [0,2].  *out receives the handle (owned by the caller -> rt_destroy). */
 int rt_create(const rt_config* cfg, const double* phi, const double* eps, const double* occ, rt_handle* out);
 
-/* Field E(t_{n+1}) used by the following step(s): HOST double[3]; sticky; default (0,0,0). */
+/* Field E(t_{n+1}) used by the following step(s): HOST double[3]; sticky; default (0,0,0).  The three values are read
+ * before the call returns (they travel to the device as kernel arguments), so the buffer may be reused at once.
+ * RT_EINVAL when |E| is so large that the series order fixed at rt_create (DESIGN R8: spectral bound with E0 and a
+ * 0.5 Ha margin) would leave a truncation term above 1e-15 -- create the handle with that E0 or an explicit order. */
 int rt_set_field(rt_handle h, const double E[3]);
 
 /* Enqueue nsteps >= 0 time steps on the stream.  Does not synchronise the host. */
@@ -111,7 +115,8 @@ int rt_get_density(rt_handle h, double* rho);
 
 /* Dipole time series mu(t_k), k = first .. first + n - 1 (k = 0 is t = 0), into out[n][4] (HOST): mu_x, mu_y, mu_z and
  * the charge dVol sum rho.  Needs rt_config.history > 0; only the last `history` levels are kept (RT_EINVAL for
- * older or future ones).  Synchronises the stream once, however many steps were enqueued. */
+ * older or future ones, and for levels before the one restored by rt_set_state).  Synchronises the stream once,
+ * however many steps were enqueued. */
 int rt_get_dipole_series(rt_handle h, int64_t first, int32_t n, double* out);
 
 /* ---- checkpoint / resume ---------------------------------------------------------------------------
@@ -151,7 +156,9 @@ int rt_get_info(rt_handle h, int32_t info[8]);
 int rt_get_launch_count(rt_handle h, int64_t* n);
 /* What the loops of Alg. 1 did in the most recent step.  HOST: n[0] = Hamiltonian updates (n_hupdates unless
  * H_thrs > 0), n[1] = orders summed by the commutator series in the last update (0 with RT_PROP_TAYLOR);
- * err[0] = last max|H1 - H1_old| (0 unless H_thrs > 0), err[1] = last max|dP^(k)|.  Synchronises. */
+ * err[0] = last max|H1 - H1_old| (0 unless H_thrs > 0), err[1] = last max|dP^(k)|.  Synchronises.  Returns
+ * RT_ENUMERIC (outputs filled) when the last commutator series went non-finite or used max_order terms without
+ * reaching dP_thrs; with H_thrs > 0 rt_step itself returns RT_ENUMERIC in those cases. */
 int rt_get_convergence(rt_handle h, int32_t n[2], double err[2]);
 /* Text of the last error on this handle (or of the last failed rt_create when h == NULL).  Never NULL. */
 const char* rt_last_error(rt_handle h);
@@ -232,6 +239,11 @@ int rt_timing_read(rt_handle h, double ms[RT_STAGE_COUNT], int64_t calls[RT_STAG
  * Runs on `device` / `stream` (cudaStream_t) and synchronises the stream before returning. */
 int rt_spectrum(const double* mu, int32_t nt, double dt, double t_kick, const double kappa[3], double gamma,
                 const double* omega, int32_t nw, double* S, int32_t device, void* stream);
+
+/* Same, for the end-point sampled kick of this library (DESIGN R5): E_kick[3] (HOST) is the rt_config.E0 of the three
+ * runs (component q = field of the run kicked along q); kappa_q = E_q dt / 2 and t_kick = dt / 2 are formed here. */
+int rt_spectrum_kick(const double* mu, int32_t nt, double dt, const double E_kick[3], double gamma, const double* omega,
+                     int32_t nw, double* S, int32_t device, void* stream);
 
 /* ---- calibration instrument (not on the hot path) ----------------------------------------------------
  * Measures the FP64 issue-rate ceilings of `device` with register-resident operands: DMMA.8x8x4 (mma.sync

@@ -15,7 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librt_tddft.so")
 
-RT_OK, RT_EINVAL, RT_ENOMEM, RT_ECUDA, RT_ESTATE = 0, -1, -2, -3, -4
+RT_OK, RT_EINVAL, RT_ENOMEM, RT_ECUDA, RT_ESTATE, RT_ENUMERIC = 0, -1, -2, -3, -4, -5
 RT_PHI_DEVICE, RT_NO_HARTREE, RT_NO_XC, RT_NO_GRAPH, RT_NO_TMA = 1, 2, 4, 8, 16
 RT_PROP_TAYLOR, RT_PROP_COMMUTATOR = 0, 1
 RT_STAGE_NAMES = ("Hupdate", "Rho", "Vh", "ELDYN", "XC")      # Table 1 of the paper, L543-L547
@@ -27,7 +27,7 @@ SYMBOLS = (
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
-    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum", "rt_get_energy", "rt_state_bytes", "rt_get_state", "rt_set_state",
+    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum", "rt_spectrum_kick", "rt_get_energy", "rt_state_bytes", "rt_get_state", "rt_set_state",
 )
 
 RT_SLAB_INIT, RT_SLAB_PROPAGATE, RT_SLAB_POTENTIAL, RT_SLAB_SHIFT = 0, 1, 2, 3
@@ -85,6 +85,7 @@ def _load():
         "rt_get_dipole_series": [vp, C.c_int64, i32, dp], "rt_get_energy": [vp, C.POINTER(C.c_double)],
         "rt_state_bytes": [vp, i64p], "rt_get_state": [vp, vp], "rt_set_state": [vp, vp],
         "rt_spectrum": [dp, i32, C.c_double, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
+        "rt_spectrum_kick": [dp, i32, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
     }
     for name, argtypes in sig.items():
         fn = getattr(lib, name)
@@ -296,6 +297,23 @@ def rt_spectrum(mu, dt, t_kick, kappa, gamma, omega, device=0, stream=0, out=Non
     k = np.ascontiguousarray(kappa, dtype=np.float64)
     rc = _lib.rt_spectrum(_ptr(mu), nt, float(dt), float(t_kick), _ptr(k), float(gamma), _ptr(omega), nw, _ptr(out),
                           int(device), int(stream) if stream else None)
+    _check(None, rc)
+    return out
+
+
+def rt_spectrum_kick(mu, dt, E_kick, gamma, omega, device=0, stream=0, out=None):
+    """rt_spectrum for the end-point sampled kick of this library: E_kick[q] = field of the run kicked along q; the
+    delivered impulse and the effective kick time are formed inside the library (include/rt_tddft.h)."""
+    if not hasattr(mu, "is_cuda"):
+        mu = np.ascontiguousarray(mu, dtype=np.float64)
+    if not hasattr(omega, "is_cuda"):
+        omega = np.ascontiguousarray(omega, dtype=np.float64)
+    nt, nw = int(mu.shape[1]), int(omega.shape[0])
+    if out is None:
+        out = np.zeros(nw)
+    e = np.ascontiguousarray(E_kick, dtype=np.float64)
+    rc = _lib.rt_spectrum_kick(_ptr(mu), nt, float(dt), _ptr(e), float(gamma), _ptr(omega), nw, _ptr(out), int(device),
+                               int(stream) if stream else None)
     _check(None, rc)
     return out
 

@@ -262,6 +262,13 @@ void launch_delta_v(long long Ng, GridDims gd, double h, const double* rho, cons
 void launch_vxc(long long Ng, const double* rho, double* vxc, cudaStream_t st) {
   vxc_kernel<<<nblk(Ng), RB, 0, st>>>(Ng, rho, vxc);
 }
+// E(t_{n+1}) passed BY VALUE (a kernel argument is captured at launch: the caller's buffer can be reused at once)
+__global__ void set_field_kernel(double* __restrict__ dE, double ex, double ey, double ez) {
+  if (threadIdx.x == 0) { dE[0] = ex; dE[1] = ey; dE[2] = ez; }
+}
+void launch_set_field(double* dE, double ex, double ey, double ez, cudaStream_t st) {
+  set_field_kernel<<<1, 32, 0, st>>>(dE, ex, ey, ez);
+}
 void launch_field(long long Ng, GridDims gd, double h, const double* E, double* w, cudaStream_t st) {
   field_kernel<<<nblk(Ng), RB, 0, st>>>(Ng, gd, h, E, w);
 }
@@ -312,11 +319,13 @@ void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, d
   series_init_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, Y, C, c1, S, s1);
 }
 
-__global__ void copy4_kernel(long long n, double* __restrict__ d0, const double* __restrict__ s0, double* __restrict__ d1,
-                             const double* __restrict__ s1, double* __restrict__ d2, const double* __restrict__ s2,
-                             double* __restrict__ d3, const double* __restrict__ s3) {
+// Line 28 shifts H-1 <- H0 and H0 <- H1 in ONE launch, so H0 is both a source and a destination: no __restrict__
+// here, and every element is read into registers before any store.
+__global__ void copy4_kernel(long long n, double* d0, const double* s0, double* d1, const double* s1, double* d2,
+                             const double* s2, double* d3, const double* s3) {
   for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += (long long)gridDim.x * blockDim.x) {
-    d0[r] = s0[r]; d1[r] = s1[r]; d2[r] = s2[r]; d3[r] = s3[r];
+    const double a = s0[r], b = s1[r], c = s2[r], d = s3[r];
+    d0[r] = a; d1[r] = b; d2[r] = c; d3[r] = d;
   }
 }
 void launch_copy5(int N, int ldn, double* d0, const double* s0, double* d1, const double* s1, double* d2,
@@ -328,17 +337,22 @@ void launch_copy5(int N, int ldn, double* d0, const double* s0, double* d1, cons
 }
 
 // ---------------------------------------------------------------- dynamic-loop error norms (Alg. 1 lines 22, 24)
+// max that does not drop NaN/Inf: a non-finite operand turns the result into +inf, so a blown-up series or Hamiltonian
+// can never read as "converged" (fmax alone discards NaN)
+__device__ __forceinline__ double max_nf(double m, double x) {
+  return (x != x || m != m) ? __longlong_as_double(0x7ff0000000000000LL) : (x > m ? x : m);
+}
 __device__ __forceinline__ double block_max(double m) {
   __shared__ double shm[32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  for (int o = 16; o > 0; o >>= 1) m = max_nf(m, __shfl_xor_sync(0xffffffffu, m, o));
   if (lane == 0) shm[warp] = m;
   __syncthreads();
   if (warp == 0) {
     m = lane < (int)(blockDim.x >> 5) ? shm[lane] : 0.0;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    for (int o = 16; o > 0; o >>= 1) m = max_nf(m, __shfl_xor_sync(0xffffffffu, m, o));
   }
   return m;      // valid in thread 0
 }
@@ -350,7 +364,7 @@ commutator_check_kernel(long long n, const double* __restrict__ a, const double*
   if (*reinterpret_cast<volatile int*>(&cs->done)) return;
   double m = 0.0;
   for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < n; r += (long long)gridDim.x * RB)
-    m = fmax(m, fmax(fabs(a[r]), fabs(b[r])));
+    m = max_nf(max_nf(m, fabs(a[r])), fabs(b[r]));
   m = block_max(m);
   if (threadIdx.x == 0) {
     atomicMax(&cs->dP_bits[k], (unsigned long long)__double_as_longlong(m));
@@ -377,7 +391,7 @@ __global__ void __launch_bounds__(RB)
 maxabs_diff_kernel(long long n, const double* __restrict__ a, const double* __restrict__ b, ConvState* __restrict__ cs) {
   double m = 0.0;
   for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < n; r += (long long)gridDim.x * RB)
-    m = fmax(m, fabs(a[r] - b[r]));
+    m = max_nf(m, fabs(a[r] - b[r]));
   m = block_max(m);
   if (threadIdx.x == 0) atomicMax(&cs->H_bits, (unsigned long long)__double_as_longlong(m));
 }

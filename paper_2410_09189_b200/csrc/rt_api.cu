@@ -35,6 +35,10 @@ struct rt_ctx {
   double* d_hist = nullptr;      // [hist_cap][4]
   unsigned long long* d_hist_n = nullptr;   // levels recorded so far (device counter: the step graph increments it)
   int64_t steps_done = 0;        // time levels after t = 0 enqueued so far
+  int64_t hist_first = 0;        // oldest level the history can hold (0, or the level restored by rt_set_state)
+  double theta0 = 0;             // dt * (spectral half-width + 0.5 Ha margin): the series orders were sized with this
+  double half_len[3] = {0, 0, 0}; // largest |x_q| on the grid
+  double* op_T[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // rt_op_propagate scratch (lazily allocated once)
   GridDims gd{};
   double h = 0, dvol = 0, dt = 0, sigma = 0, omega = 0;
   int m = 2, n_vc = 0, nu1 = 2, nu2 = 2, q = 0;           // q: cos/sinc polynomial degree in Y = X^2
@@ -565,6 +569,8 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     double vmax = 0.5;
     for (int d = 0; d < 3; ++d) vmax += std::fabs(cfg->E0[d]) * half[d];
     const double theta = c->dt * (0.5 * (emax - emin) + vmax);
+    c->theta0 = c->dt * (0.5 * (emax - emin) + 0.5);
+    for (int d = 0; d < 3; ++d) c->half_len[d] = half[d];
     int q;
     if (cfg->exp_order > 0) q = (cfg->exp_order > 1) ? cfg->exp_order / 2 : 1;   // degree 2q+1 >= K
     else {
@@ -729,6 +735,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   c->hist_cap = cfg->history;
   if (c->hist_cap) {
     ALLOC(c->d_hist, (size_t)c->hist_cap * 4);
+    CKC(cudaMemsetAsync(c->d_hist, 0, (size_t)c->hist_cap * 32, c->st));
     ALLOC(c->d_hist_n, 1);
     CKC(cudaMemsetAsync(c->d_hist_n, 0, sizeof(unsigned long long), c->st));
   }
@@ -862,8 +869,30 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
 int rt_set_field(rt_handle c, const double E[3]) {
   CHECK_HANDLE(c);
   if (!E) return fail(c, RT_EINVAL, "rt_set_field: NULL");
+  const double e0 = E[0], e1 = E[1], e2 = E[2];                 // read now: the value travels as a kernel argument
+  if (!(e0 == e0 && e1 == e1 && e2 == e2)) return fail(c, RT_EINVAL, "rt_set_field: NaN");
+  // The Taylor degree q / the commutator kmax were fixed at rt_create from the spectral bound with E0 (DESIGN R8):
+  // refuse a field that takes the truncation term of that fixed order above 1e-15 (design bound 1e-17).
+  {
+    const double theta = c->theta0 + c->dt * (std::fabs(e0) * c->half_len[0] + std::fabs(e1) * c->half_len[1] +
+                                               std::fabs(e2) * c->half_len[2]);
+    bool ok = true;
+    if (c->prop == RT_PROP_TAYLOR && c->cfg.exp_order == 0) {
+      double term = 1.0;
+      for (int k = 1; k <= 2 * c->q + 2; ++k) term *= theta / k;
+      ok = term <= 1e-15;
+    } else if (c->prop == RT_PROP_COMMUTATOR && c->cfg.max_order == 0) {
+      double term = 2.0;
+      for (int k = 1; k <= c->kmax; ++k) term *= 2.0 * theta / k;
+      ok = term <= c->dP_thrs;
+    }
+    if (!ok) return fail(c, RT_EINVAL, "rt_set_field: |E| exceeds the bound the series order was sized for at rt_create "
+                                       "(create the handle with E0 of that magnitude or with an explicit exp_order / max_order)");
+  }
   CK(cudaSetDevice(c->cfg.device));
-  CK(cudaMemcpyAsync(c->d_E, E, 3 * sizeof(double), cudaMemcpyHostToDevice, c->st));
+  launch_set_field(c->d_E, e0, e1, e2, c->st);
+  c->launches += 1;
+  CK(cudaGetLastError());
   return RT_OK;
 }
 
@@ -894,6 +923,14 @@ int rt_step(rt_handle c, int32_t nsteps) {
         c->last_orders = hs.k_used;
         memcpy(&c->last_dP_err, &hs.dP_bits[hs.k_used], 8);
         ++it;
+        if (!std::isfinite(herr) || !std::isfinite(c->last_dP_err)) {
+          c->last_hupdates = it; c->last_H_err = herr;
+          return fail(c, RT_ENUMERIC, "rt_step: non-finite H1 or dP (time step too large for the series, or bad input)");
+        }
+        if (c->prop == RT_PROP_COMMUTATOR && !hs.done) {
+          c->last_hupdates = it; c->last_H_err = herr;
+          return fail(c, RT_ENUMERIC, "rt_step: the commutator series did not reach dP_thrs within max_order terms");
+        }
       }
       enqueue_shift(c);
       CK(cudaGetLastError());
@@ -919,7 +956,7 @@ int rt_get_dipole_series(rt_handle c, int64_t first, int32_t n, double* out) {
   if (!out || n < 0 || first < 0) return fail(c, RT_EINVAL, "rt_get_dipole_series: bad argument");
   if (!c->hist_cap) return fail(c, RT_EINVAL, "rt_get_dipole_series: handle created with history = 0");
   const int64_t have = c->steps_done + 1;                  // levels 0 .. steps_done
-  if (first + n > have || first < have - c->hist_cap)
+  if (first + n > have || first < have - c->hist_cap || first < c->hist_first)
     return fail(c, RT_EINVAL, "rt_get_dipole_series: requested levels are not in the history window");
   CK(cudaSetDevice(c->cfg.device));
   for (int32_t i = 0; i < n;) {                            // at most two contiguous pieces of the ring
@@ -947,6 +984,8 @@ int rt_get_convergence(rt_handle c, int32_t n[2], double err[2]) {
       if (int rc = sync_and_check(c)) return rc;
       n[1] = hs.k_used;
       memcpy(&err[1], &hs.dP_bits[hs.k_used], 8);
+      if (c->steps_done > 0 && (!std::isfinite(err[1]) || !hs.done))
+        return fail(c, RT_ENUMERIC, "rt_get_convergence: the last commutator series is non-finite or stopped at max_order above dP_thrs");
     }
   }
   return RT_OK;
@@ -1042,6 +1081,7 @@ int rt_set_state(rt_handle c, const void* buf) {
   // H1 is rebuilt from H0 and H-1 by the first update of the next step (line 11); P1 by the propagation
   c->t = hd.t;
   c->steps_done = hd.steps;
+  c->hist_first = hd.steps;
   if (c->hist_cap) {                                   // the history restarts at this level
     const unsigned long long k = (unsigned long long)hd.steps;
     CK(cudaMemcpyAsync(c->d_hist_n, &k, sizeof k, cudaMemcpyHostToDevice, c->st));
@@ -1158,34 +1198,27 @@ int rt_op_propagate(rt_handle c, const double* Hbar, const double* P0re, const d
   if (c->slab) return fail(c, RT_ESTATE, "rt_op_propagate: not available on a slab handle");
   if (!Hbar || !P0re || !P0im || !P1re || !P1im) return fail(c, RT_EINVAL, "rt_op_propagate: NULL");
   CK(cudaSetDevice(c->cfg.device));
-  // scratch: H1 <- Hbar (as both H0 and H1 of launch_hbar), P1r/P1i <- P0 ; outputs in Hm1-free buffers
-  // The propagation state uses Hm1/H0/H1/P0/P1, so stage everything in W (>= 1 slab) plus X..Sm scratch.
-  // W holds S >= 1 slabs of N*ldn; we need 5 matrices -> use Hm1-independent temporaries allocated lazily.
   const size_t nn = (size_t)c->N * c->ldn;
-  double* T[5];
-  for (int i = 0; i < 5; ++i) {
-    void* p = nullptr;
-    CK(cudaMalloc(&p, nn * 8));
-    T[i] = (double*)p;
+  // The propagation state owns Hm1/H0/H1/P0/P1 and the series owns X..Sm: the call needs five more N x N matrices.
+  // They are allocated once per handle, on first use, and freed by rt_destroy.
+  if (!c->op_T[0]) {
+    double* T5 = nullptr;
+    if (int rc = dev_alloc(c, &T5, 5 * nn)) return rc;
+    for (int i = 0; i < 5; ++i) c->op_T[i] = T5 + i * nn;
   }
-  int rc = RT_OK;
-  do {
-    if ((rc = copy_matrix_in(c, Hbar, T[0]))) break;
-    if ((rc = copy_matrix_in(c, P0re, T[1]))) break;
-    if ((rc = copy_matrix_in(c, P0im, T[2]))) break;
-    stage_begin(c, RT_STAGE_ELDYN);
-    launch_hbar(c->N, c->ldn, T[0], T[0], T[0], c->X, c->dt, c->sigma, 0, c->st);   // X = dt (Hbar - sigma I)
-    c->launches += 1;
-    if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);
-    enqueue_propagate(c, T[1], T[2], T[3], T[4]);
-    stage_end(c);
-    if ((rc = copy_matrix_out(c, T[3], P1re))) break;
-    if ((rc = copy_matrix_out(c, T[4], P1im))) break;
-    rc = sync_and_check(c);
-  } while (0);
-  cudaStreamSynchronize(c->st);
-  for (int i = 0; i < 5; ++i) cudaFree(T[i]);
-  return rc;
+  double** T = c->op_T;
+  if (int rc = copy_matrix_in(c, Hbar, T[0])) return rc;
+  if (int rc = copy_matrix_in(c, P0re, T[1])) return rc;
+  if (int rc = copy_matrix_in(c, P0im, T[2])) return rc;
+  stage_begin(c, RT_STAGE_ELDYN);
+  launch_hbar(c->N, c->ldn, T[0], T[0], T[0], c->X, c->dt, c->sigma, 0, c->st);   // X = dt (Hbar - sigma I)
+  c->launches += 1;
+  if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);
+  enqueue_propagate(c, T[1], T[2], T[3], T[4]);
+  stage_end(c);
+  if (int rc = copy_matrix_out(c, T[3], P1re)) return rc;
+  if (int rc = copy_matrix_out(c, T[4], P1im)) return rc;
+  return sync_and_check(c);
 }
 
 int rt_op_hartree(rt_handle c, double* vh, const double* drho, int32_t n_vc) {
@@ -1309,6 +1342,14 @@ int rt_spectrum(const double* mu, int32_t nt, double dt, double t_kick, const do
   cudaFree(d_mu); cudaFree(d_w); cudaFree(d_S);
   if (e != cudaSuccess) { cudaGetLastError(); return fail(c, RT_ECUDA, std::string("rt_spectrum: ") + cudaGetErrorString(e)); }
   return RT_OK;
+}
+
+int rt_spectrum_kick(const double* mu, int32_t nt, double dt, const double E_kick[3], double gamma, const double* omega,
+                     int32_t nw, double* S, int32_t device, void* stream) {
+  if (!E_kick) return fail(nullptr, RT_EINVAL, "rt_spectrum_kick: NULL");
+  // end-point sampled kick (DESIGN R5): the trapezoid of Alg. 1 line 14 delivers E dt / 2 at the effective time dt / 2
+  const double kappa[3] = {0.5 * E_kick[0] * dt, 0.5 * E_kick[1] * dt, 0.5 * E_kick[2] * dt};
+  return rt_spectrum(mu, nt, dt, 0.5 * dt, kappa, gamma, omega, nw, S, device, stream);
 }
 
 int rt_timing_enable(rt_handle c, int32_t enable) {

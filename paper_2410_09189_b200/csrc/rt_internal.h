@@ -128,6 +128,7 @@ void launch_delta_v(long long Ng, GridDims gd, double h, const double* rho, cons
                     const double* E, int use_h, int use_xc, double* w, cudaStream_t st);
 void launch_vxc(long long Ng, const double* rho, double* vxc, cudaStream_t st);
 void launch_field(long long Ng, GridDims gd, double h, const double* E, double* w, cudaStream_t st);
+void launch_set_field(double* dE, double ex, double ey, double ez, cudaStream_t st);   // dE[0..2] = E, by value
 // f = 4 pi (rho - rho0 - sums[4]/Ng)      (rho0 may be nullptr: f = 4 pi (rho - sums[4]/Ng))
 void launch_poisson_rhs(long long Ng, const double* rho, const double* rho0, const double* sums, double* f,
                         cudaStream_t st);

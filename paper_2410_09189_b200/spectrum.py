@@ -51,15 +51,17 @@ class KickTriple:
             mu[ax] = sim.dipole_series(0, self.nsteps + 1)[:, ax]
         return mu
 
-    def kappa(self):
-        k = [0.0, 0.0, 0.0]
+    def kick_field(self):
+        """E_kick[q] = field strength of the run kicked along q (0 for axes that were not run)."""
+        e = [0.0, 0.0, 0.0]
         for ax in self.axes:
-            k[ax] = 0.5 * self.kick * self.dt
-        return k
+            e[ax] = self.kick
+        return e
 
     def spectrum(self, omega, gamma):
-        """Dipole strength function S(omega) with exponential damping gamma (a.u.)."""
-        return B.rt_spectrum(self.dipoles(), self.dt, 0.5 * self.dt, self.kappa(), gamma, omega, device=self.device)
+        """Dipole strength function S(omega) with exponential damping gamma (a.u.); the delivered impulse and the
+        effective kick time of the end-point sampled kick are formed inside the library (rt_spectrum_kick)."""
+        return B.rt_spectrum_kick(self.dipoles(), self.dt, self.kick_field(), gamma, omega, device=self.device)
 
     def synchronize(self):
         for st in self.streams:

@@ -119,6 +119,14 @@ def make_inputs_numpy(w: Workload):
     return Phi, eps, occ
 
 
+def phi_slab_sample(w: Workload, npts: int) -> np.ndarray:
+    """[N][npts] slab of orbital values for the bounded CPU-baseline sample of the configs whose Phi only exists on the
+    device: the generator's raw seeded draw N(0, 1/(Ng dV)) for those points, before orthonormalisation (which changes
+    it by O(sqrt(N/Ng)); the oracle's run time does not depend on the values)."""
+    rng = np.random.default_rng(w.seed)
+    return rng.standard_normal((w.norb, int(npts))) / math.sqrt(w.ngrid * w.dvol)
+
+
 def make_inputs_device(w: Workload, device="cuda", tile: int = 16384, passes: int = 2):
     """Large configs: Phi generated and orthonormalised in place on the device (no second copy).
 

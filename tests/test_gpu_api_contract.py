@@ -1,0 +1,151 @@
+"""Boundary behaviour of the C ABI on a GPU (include/rt_tddft.h): error paths and the contracts the round-1 review
+found unenforced.  No oracle arithmetic is needed except where a result is compared."""
+import numpy as np
+import pytest
+
+from oracle import rt_oracle as O
+from paper_2410_09189_b200.workloads import WORKLOADS, make_inputs_numpy, strong_kick
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2410_09189_b200.build import build
+    build()
+    from paper_2410_09189_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    w = strong_kick(WORKLOADS["tiny"], 0.1)
+    return (w,) + make_inputs_numpy(w)
+
+
+def test_history_restarts_at_the_restored_level(B, tiny):
+    """rt_set_state: the dipole history restarts at the restored time level -- older levels were never recorded in
+    this handle and must be refused, not returned as zeros or garbage."""
+    w, Phi, eps, occ = tiny
+    kw = dict(E0=w.kick, n_vcycles=w.n_vcycles, history=16)
+    a = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, **kw)
+    a.step(4)
+    state = a.get_state()
+    b = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, **kw)
+    assert np.all(b.dipole_series(0, 1)[0, :3] == b.dipole())
+    b.set_state(state)
+    for first, n in ((0, 5), (3, 2), (0, 1)):
+        with pytest.raises(B.RTError) as ei:
+            b.dipole_series(first, n)
+        assert ei.value.code == B.RT_EINVAL
+    assert np.array_equal(b.dipole_series(4, 1), a.dipole_series(4, 1))
+    b.step(3)
+    a.step(3)
+    assert np.array_equal(b.dipole_series(4, 4), a.dipole_series(4, 4))
+    with pytest.raises(B.RTError):
+        b.dipole_series(3, 3)
+    a.close()
+    b.close()
+
+
+def test_set_field_reads_its_argument_before_returning(B, tiny):
+    """rt_set_field from page-locked host memory that is overwritten right after the call (no synchronisation in
+    between): the step must see the value that was in the buffer AT the call."""
+    import torch
+    w, Phi, eps, occ = tiny
+    Es = [(0.0, 0.0, 0.02), (0.01, -0.02, 0.0), (0.0, 0.03, 0.01), (0.0, 0.0, 0.0)]
+    gpu = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, E0=(0, 0, 0), n_vcycles=w.n_vcycles, history=8)
+    cpu = O.RTOracle(w.shape, w.h, Phi, eps, occ, dt=w.dt, E0=(0, 0, 0), n_vcycles=w.n_vcycles)
+    e_host = torch.zeros(3, dtype=torch.float64).pin_memory()
+    mus = [cpu.dipole()]
+    for E in Es:
+        e_host[0], e_host[1], e_host[2] = E
+        B._check(gpu.handle, B._lib.rt_set_field(gpu.handle, e_host.data_ptr()))
+        e_host.fill_(123.0)                       # poison: a late asynchronous read would pick this up
+        gpu.step(1)
+        cpu.set_field(E)
+        cpu.step(1)
+        mus.append(cpu.dipole())
+    got = gpu.dipole_series(0, len(Es) + 1)[:, :3]
+    assert np.max(np.abs(got - np.array(mus))) < 1e-9 * np.max(np.abs(mus))
+    gpu.close()
+
+
+def test_set_field_beyond_the_series_bound_is_refused(B, tiny):
+    """The Taylor degree is fixed at rt_create from the spectral bound with E0 (DESIGN R8): a later field far outside
+    that bound must not silently run with a truncated series."""
+    w, Phi, eps, occ = tiny
+    gpu = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, E0=(0, 0, 0))
+    gpu.set_field((0.0, 0.05, 0.0))               # well inside the 0.5 Ha margin
+    with pytest.raises(B.RTError) as ei:
+        gpu.set_field((50.0, 0.0, 0.0))
+    assert ei.value.code == B.RT_EINVAL
+    with pytest.raises(B.RTError):
+        gpu.set_field((float("nan"), 0.0, 0.0))
+    gpu.step(1)                                    # the handle stays usable, the accepted field is still in force
+    gpu.close()
+    # an explicit order is the caller's responsibility: accepted
+    g2 = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, E0=(0, 0, 0), exp_order=31)
+    g2.set_field((5.0, 0.0, 0.0))
+    g2.close()
+    # commutator mode has the same guard on kmax
+    g3 = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, E0=(0, 0, 0), propagator="commutator")
+    with pytest.raises(B.RTError):
+        g3.set_field((50.0, 0.0, 0.0))
+    g3.close()
+
+
+def test_non_finite_values_are_reported_not_declared_converged(B, tiny):
+    """A NaN in the state (bad input) must not read as `converged`: fmax-style reductions drop NaN, the library's do
+    not.  Dynamic H loop: rt_step returns RT_ENUMERIC; fixed-count commutator mode: rt_get_convergence does."""
+    w, Phi, eps, occ = tiny
+    bad = eps.copy()
+    bad[3] = float("inf")                          # H0 = diag(eps) + ... is then non-finite
+    g = B.RTTDDFT(w.shape, w.h, Phi, np.where(np.isfinite(bad), bad, 1e300), occ, w.dt, E0=w.kick,
+                  propagator="commutator", H_thrs=1e-7, max_order=20)
+    with pytest.raises(B.RTError) as ei:
+        g.step(1)
+    assert ei.value.code == B.RT_ENUMERIC
+    g.close()
+    # a series cut off far above dP_thrs is reported too
+    g = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, E0=w.kick, propagator="commutator", max_order=2, dP_thrs=1e-14)
+    g.step(1)
+    with pytest.raises(B.RTError) as ei:
+        g.convergence()
+    assert ei.value.code == B.RT_ENUMERIC
+    g.close()
+    g = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, E0=w.kick, propagator="commutator")
+    g.step(1)
+    c = g.convergence()
+    assert 3 < c["orders"] < 40 and c["dP_err"] <= 1e-10
+    g.close()
+
+
+def test_op_propagate_reuses_its_scratch(B, tiny):
+    """rt_op_propagate allocates its five N x N scratch matrices once per handle (round 1: cudaMalloc/cudaFree per call)."""
+    import torch
+    w, Phi, eps, occ = tiny
+    g = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt)
+    N = w.norb
+    H = np.diag(eps)
+    P0 = np.diag(occ).astype(complex)
+    out = [np.empty((N, N)), np.empty((N, N))]
+    B.rt_op_propagate(g.handle, H, np.ascontiguousarray(P0.real), np.ascontiguousarray(P0.imag), *out)
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(20):
+        B.rt_op_propagate(g.handle, H, np.ascontiguousarray(P0.real), np.ascontiguousarray(P0.imag), *out)
+    assert torch.cuda.mem_get_info()[0] == free0
+    assert np.max(np.abs(out[0] - np.diag(occ))) < 1e-14 and np.max(np.abs(out[1])) < 1e-14
+    g.close()
+
+
+def test_spectrum_kick_forms_the_impulse_inside_the_library(B):
+    rng = np.random.default_rng(5)
+    mu = rng.standard_normal((3, 300)) * 1e-3
+    omega = np.linspace(0.1, 1.0, 17)
+    dt, E = 0.2, (1e-3, 0.0, 2e-3)
+    S = B.rt_spectrum_kick(mu, dt, E, 0.02, omega)
+    ref = O.dipole_strength(mu, dt, 0.5 * dt, tuple(0.5 * e * dt for e in E), 0.02, omega)
+    assert np.max(np.abs(S - ref)) < 1e-12 * np.max(np.abs(ref))

@@ -144,6 +144,9 @@ def test_spectral_solve_inverts_stencil_and_plane_wave():
         u = O.spectral_solve(f, 0.8)
         assert np.allclose(O.apply_A(u, 0.8), f, rtol=0, atol=1e-12)
         assert abs(u.mean()) < 1e-14
+        # a right-hand side with a mean: the constant mode is projected out (zero-mean subspace, DESIGN R6)
+        u2 = O.spectral_solve(f + 0.7, 0.8)
+        assert abs(u2.mean()) < 1e-14 and np.allclose(u2, u, rtol=0, atol=1e-12)
     # closed form: f = cos(2 pi i/n) is an eigenvector with eigenvalue (2 - 2cos(2 pi/n))/h^2
     n, h = 12, 0.5
     f = np.cos(2 * np.pi * np.arange(n) / n)[:, None, None] * np.ones((n, n, n))
@@ -487,3 +490,113 @@ def test_spectrum_of_noninteracting_system_has_the_particle_hole_lines(tiny_inpu
                 f = 2.0 * occ[i] * wn * M[a, i] ** 2
                 ref += (2 * omega / np.pi) * f * np.imag(1.0 / (wn ** 2 + (gamma - 1j * omega) ** 2)) / 3.0
     assert np.max(ref) > 0 and np.max(np.abs(S - ref)) < 0.03 * np.max(ref)
+
+
+# ------------------------------------------------------------------ time-dependent field path (Alg. 1 lines 11, 14)
+def _dipole_matrices_plain(w, Phi):
+    """M_q = dV sum_r phi_i(r) x_q(r) phi_j(r) written out here with np.indices (not through oracle.project /
+    field_potential), centred sawtooth x(i) = (i - (n-1)/2) h (DESIGN R4)."""
+    idx = np.indices(w.shape).reshape(3, -1).astype(np.float64)
+    M = []
+    for q in range(3):
+        xq = (idx[q] - 0.5 * (w.shape[q] - 1)) * w.h
+        M.append(w.dvol * (Phi * xq[None, :]) @ Phi.T)
+    return M
+
+
+def test_line11_extrapolation_is_exact_for_a_field_linear_in_time(tiny_inputs):
+    """Alg. 1 line 11 H1 = 2 H0 - H-1.  Interactions off, ONE Hamiltonian update per step (so the
+    corrector never repairs the predictor) and a field linear in time, E(t_k) = a t_k, driven through set_field: then
+    H(t_k) = diag eps + E(t_k).M and from the second step on 2 H(t_n) - H(t_{n-1}) IS H(t_{n+1}), so
+        P(t_{n+1}) = exp(-i dt (H(t_n) + H(t_{n+1}))/2) P(t_n) exp(+...)            (Eq. 12, Eq. 15)
+    with scipy's Pade expm.  The first step has H-1 = H0 (line 8, L357), i.e. Hbar = H(0).  A predictor H1 = H0, a
+    wrong sign / factor in line 11, or a shift (line 28) that mixes up H-1 and H0 is off by O(a dt) = 1e-3."""
+    w, Phi, eps, occ = tiny_inputs
+    a = np.array([0.02, -0.01, 0.015])
+    M = _dipole_matrices_plain(w, Phi)
+
+    def H(t):
+        return np.diag(eps) + sum(a[q] * t * M[q] for q in range(3))
+
+    o = _make(tiny_inputs, E0=(0, 0, 0), n_hupdates=1, hartree=False, xc=False)
+    P = np.diag(occ).astype(complex)
+    worst = 0.0
+    for n in range(8):
+        t0, t1 = n * w.dt, (n + 1) * w.dt
+        o.set_field(a * t1)
+        o.step(1)
+        Hbar = H(0.0) if n == 0 else 0.5 * (H(t0) + H(t1))
+        U = scipy.linalg.expm(-1j * w.dt * Hbar)
+        P = U @ P @ U.conj().T
+        worst = max(worst, np.max(np.abs(o.P0 - P)))
+        assert np.allclose(o.H0, H(t1), rtol=0, atol=1e-13)            # line 25 with E(t_{n+1}); line 28 H0 <- H1
+        assert np.allclose(o.Hm1, H(t0), rtol=0, atol=1e-13)           # line 28 H-1 <- H0
+        mu_ref = np.array([np.sum(P.real * M[q].T) for q in range(3)])
+        assert np.max(np.abs(o.dipole() - mu_ref)) < 1e-12            # line 27: mu = tr(P M)
+    assert worst < 5e-13
+    # the predictor matters: the same trajectory with Hbar = H(t_n) is far outside the tolerance
+    Pw = np.diag(occ).astype(complex)
+    for n in range(8):
+        U = scipy.linalg.expm(-1j * w.dt * H(n * w.dt))
+        Pw = U @ Pw @ U.conj().T
+    assert np.max(np.abs(Pw - P)) > 1e-5
+
+
+def test_set_field_is_the_end_point_value_of_the_trapezoid(tiny_inputs):
+    """Alg. 1 line 14 (L373): Omega = -i dt/2 (H0 + H1 + V_{j-1} + V_j).  Interactions off, m = 2: the first update
+    rebuilds H1 = diag eps + E_next.M exactly (whatever the predictor was), so the second one propagates with
+    Hbar = (H(t_n) + H(t_{n+1}))/2 where E(t_{n+1}) is the value handed to set_field BEFORE the step (DESIGN R5) and
+    E(t_0) = E0.  Arbitrary (non-smooth) field sequence along all three axes.  Catches: a dropped E.x term in delta_v,
+    set_field taken as E(t_n) or as a mid-point value, a field that is not sticky, a missing factor 1/2."""
+    w, Phi, eps, occ = tiny_inputs
+    rng = np.random.default_rng(11)
+    Es = rng.uniform(-0.03, 0.03, size=(7, 3))
+    Es[3] = Es[2]                      # one step without a new set_field call: the value is sticky
+    M = _dipole_matrices_plain(w, Phi)
+
+    def H(E):
+        return np.diag(eps) + sum(E[q] * M[q] for q in range(3))
+
+    o = _make(tiny_inputs, E0=tuple(Es[0]), n_hupdates=2, hartree=False, xc=False)
+    assert np.allclose(o.H0, H(Es[0]), rtol=0, atol=1e-13)              # Alg. 1 lines 7-8: H0 includes V(t_0)
+    P = np.diag(occ).astype(complex)
+    for n in range(6):
+        if n != 2:
+            o.set_field(Es[n + 1])
+        o.step(1)
+        U = scipy.linalg.expm(-1j * w.dt * 0.5 * (H(Es[n]) + H(Es[n + 1])))
+        P = U @ P @ U.conj().T
+        assert np.max(np.abs(o.P0 - P)) < 5e-13, n
+        assert np.allclose(o.H0, H(Es[n + 1]), rtol=0, atol=1e-13)
+    # sensitivity: end-point value replaced by the previous one changes P by O(|dE| dt)
+    U = scipy.linalg.expm(-1j * w.dt * H(Es[5]))
+    assert np.max(np.abs(U @ P @ U.conj().T - scipy.linalg.expm(-1j * w.dt * 0.5 * (H(Es[5]) + H(Es[6]))) @ P @
+                         scipy.linalg.expm(+1j * w.dt * 0.5 * (H(Es[5]) + H(Es[6]))))) > 1e-6
+
+
+def test_field_energy_term_and_work_done_by_a_laser(tiny_inputs):
+    """With the full interacting step and a smooth pulse, dE/dt = dVol sum_r (dE_field/dt . r) drho  (the energy
+    diagnostic includes E.r drho, so only the explicit time dependence does work): over the pulse the oracle's
+    energy() must change by the trapezoid of that power; after the pulse it is conserved.  Pins the sign and the end-point
+    timing of the E(t_{n+1}).x term of delta_v inside the INTERACTING step (a field applied one step late or with the
+    wrong sign breaks the balance at first order)."""
+    w, Phi, eps, occ = tiny_inputs
+    dt, nst = 0.05, 60
+    o = _make(tiny_inputs, E0=(0, 0, 0), dt=dt, n_hupdates=3, n_vcycles=8)
+
+    def E(t):
+        return np.array([0.0, 0.0, 0.05 * math.sin(math.pi * t / 2.0) ** 2 if t < 2.0 else 0.0])
+
+    es, mus = [o.energy()], [o.dipole() - O.dipole(o.rho0, w.shape, w.h)]
+    for n in range(nst):
+        o.set_field(E((n + 1) * dt))
+        o.step(1)
+        es.append(o.energy())
+        mus.append(o.dipole() - O.dipole(o.rho0, w.shape, w.h))
+    es, mus = np.array(es), np.array(mus)
+    # work = int dE/dt . dmu dt (trapezoid in dE): sum_n (E_{n+1} - E_n) . (dmu_n + dmu_{n+1})/2
+    work = sum(np.dot(E((n + 1) * dt) - E(n * dt), 0.5 * (mus[n] + mus[n + 1])) for n in range(40))
+    gained = es[40] - es[0]
+    assert gained > 1e-5                                                # the pulse deposited energy (7.5e-5 Ha)
+    assert abs(gained - work) < 1e-11                                   # discrete energy balance of the midpoint rule
+    assert np.max(np.abs(es[41:] - es[41])) < 1e-11                     # field off: conserved
