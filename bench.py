@@ -212,6 +212,8 @@ def workload_config(w, args):
             "l2": "inputs larger than L2 (Phi streamed twice per Hamiltonian update)" if w.norb * w.ngrid * 8 > 2.5e8
             else "L2 flushed between timed steps is not possible inside a CUDA graph: working set fits L2 (stated)",
             "parallelism": (f"grid slabs over {args.gpus} rank(s), 2 all-reduces per Hamiltonian update"
+                            + (", N x N propagator sharded by row blocks (3 all-gathers per update)"
+                               if args.gpus > 1 and w.norb >= 2048 else "")
                             if getattr(args, "parallel", "replicas") == "slabs" else
                             "replicas only" if args.gpus > 1 else "single GPU")}
 
@@ -292,9 +294,11 @@ def main():
     E0 = w.kick if not w.laser else w.E_of_t(0.0)
     with torch.cuda.stream(stream):
         if slabs:
+            # past the crossover ("once N exceeds a few thousands") the N x N propagator is sharded too
+            shard = dict(prop_shard=(rank, world)) if world > 1 and w.norb >= 2048 else {}
             backend = S.CudaSlabBackend(w.shape, w.h, phi, eps, occ, w.dt, slab, device=local,
                                         stream=stream.cuda_stream, E0=E0, n_hupdates=w.n_hupdates,
-                                        n_vcycles=w.n_vcycles)
+                                        n_vcycles=w.n_vcycles, **shard)
             stepper = S.SlabStepper(backend, comm, n_hupdates=w.n_hupdates)
             sim = backend.sim                   # the rt_handle owner: getters, timing and launch counts
             sim.step = stepper.step             # rt_step is not available on a slab handle

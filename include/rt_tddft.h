@@ -91,6 +91,11 @@ typedef struct {
   /* -- dipole history: > 0 keeps the dipole of the last `history` time levels on the device, appended by the step
    *    itself (no host synchronisation per step); read with rt_get_dipole_series.  0 = off.                        */
   int32_t  history;
+  /* -- row-sharded N x N propagator on slab handles (the replicated N^3 work is replaced by a
+   *    multi-GPU product "once N exceeds a few thousands"): rank prop_shard of prop_shards owns a block of whole
+   *    128-row tiles of every N x N product of a2-a4; the caller all-gathers the blocks at three points of a
+   *    Hamiltonian update (rt_slab_get_shard, RT_SLAB_PROP_A..D).  0 or 1 = replicated propagator.  Taylor mode only. */
+  int32_t  prop_shards, prop_shard;
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
@@ -195,23 +200,47 @@ int rt_op_vxc(rt_handle h, const double* rho, double* vxc);
  * RT_ESTATE.  Sequence (every rank, same order):
  *   rt_create                      -> local rho0 slab in xchg_rho, partial H(t=0) in xchg_H
  *   [all-reduce xchg_rho, xchg_H]     rt_slab_phase(h, RT_SLAB_INIT, 0)
- *   per time step, for it = 0 .. m-1:
+ *   per time step, it = 0, 1, ... :
  *     rt_slab_phase(h, RT_SLAB_PROPAGATE, it)  (a2-a5, a6 partial)   [all-reduce xchg_rho]
  *     rt_slab_phase(h, RT_SLAB_POTENTIAL, it)  (a7, a8, a1 partial)  [all-reduce xchg_H]
+ *     rt_slab_phase(h, RT_SLAB_CHECK, it)      (Alg. 1 lines 12-13, 24: one more update?)  rt_slab_more_updates
  *   rt_slab_phase(h, RT_SLAB_SHIFT, 0)         (Alg. 1 line 28)
- * Phases enqueue on the handle's stream and do not synchronise; the collectives must run on the same stream (or be
- * ordered after it). */
+ * With rt_config.prop_shards > 1 RT_SLAB_PROPAGATE is replaced by four phases with all-gathers of row blocks between
+ * them (buffers from rt_slab_get_shard; every rank's block is block_count doubles at offset prop_shard * block_count):
+ *     RT_SLAB_PROP_A (a2, Y = X^2 rows)                    [all-gather Y]
+ *     RT_SLAB_PROP_B (a3 series, first half of a4, rows)   [all-gather C, S]
+ *     RT_SLAB_PROP_C (second half of a4, rows)             [all-gather P1re, P1im]
+ *     RT_SLAB_PROP_D (P1 made exactly Hermitian, a5, a6 partial)   [all-reduce xchg_rho]
+ * Phases enqueue on the handle's stream and do not synchronise (RT_SLAB_CHECK does when H_thrs > 0: it reads the 8-byte
+ * error norm); the collectives must run on the same stream (or be ordered after it).  Each phase is captured into a
+ * CUDA graph on first use and replayed afterwards (unless RT_NO_GRAPH). */
 #define RT_SLAB_INIT      0
 #define RT_SLAB_PROPAGATE 1
 #define RT_SLAB_POTENTIAL 2
 #define RT_SLAB_SHIFT     3
+#define RT_SLAB_PROP_A    4
+#define RT_SLAB_PROP_B    5
+#define RT_SLAB_PROP_C    6
+#define RT_SLAB_PROP_D    7
+#define RT_SLAB_CHECK     8
 typedef struct {
   double* xchg_rho;  int64_t xchg_rho_count;   /* DEVICE, Ng + 8 doubles                          */
   double* xchg_H;    int64_t xchg_H_count;     /* DEVICE, norb * ldn doubles (ldn = norb rounded up to 8) */
   int64_t slab_offset, slab_count;             /* this rank's range of grid points inside xchg_rho */
 } rt_slab_buffers;
+typedef struct {
+  double *Y, *C, *S, *P1re, *P1im;             /* DEVICE, total_count doubles each: [prop_shards * rows_per_rank][ldn]   */
+  int64_t block_count;                         /* doubles per rank block (rows_per_rank * ldn)                          */
+  int64_t total_count;                         /* >= prop_shards * block_count                                           */
+  int32_t prop_shards, prop_shard;
+} rt_shard_buffers;
 int rt_slab_get_buffers(rt_handle h, rt_slab_buffers* out);
+int rt_slab_get_shard(rt_handle h, rt_shard_buffers* out);
 int rt_slab_phase(rt_handle h, int32_t phase, int32_t it);
+/* After RT_SLAB_CHECK(it) (or RT_SLAB_POTENTIAL(it) on a fixed-count handle): *more (HOST) = 1 if Algorithm 1 wants
+ * another Hamiltonian update in this time step (fixed count: it + 1 < n_hupdates; H_thrs > 0: max|H1 - H1_old| >
+ * H_thrs and it + 1 < max_hupdates), else 0.  Identical on every rank. */
+int rt_slab_more_updates(rt_handle h, int32_t* more);
 
 /* ---- per-stage timing (CUDA events on the launching stream) ------------------------------------
  * Stage ids follow Table 1 (L543-L547) plus the rest of the step. */

@@ -27,10 +27,11 @@ SYMBOLS = (
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
-    "rt_slab_get_buffers", "rt_slab_phase", "rt_get_dipole_series", "rt_spectrum", "rt_spectrum_kick", "rt_get_energy", "rt_state_bytes", "rt_get_state", "rt_set_state",
+    "rt_slab_get_buffers", "rt_slab_phase", "rt_slab_get_shard", "rt_slab_more_updates", "rt_get_dipole_series", "rt_spectrum", "rt_spectrum_kick", "rt_get_energy", "rt_state_bytes", "rt_get_state", "rt_set_state",
 )
 
 RT_SLAB_INIT, RT_SLAB_PROPAGATE, RT_SLAB_POTENTIAL, RT_SLAB_SHIFT = 0, 1, 2, 3
+RT_SLAB_PROP_A, RT_SLAB_PROP_B, RT_SLAB_PROP_C, RT_SLAB_PROP_D, RT_SLAB_CHECK = 4, 5, 6, 7, 8
 
 
 class rt_config(C.Structure):
@@ -52,12 +53,19 @@ class rt_config(C.Structure):
         ("max_hupdates", C.c_int32),
         ("slab_x0", C.c_int32), ("slab_nx", C.c_int32),
         ("history", C.c_int32),
+        ("prop_shards", C.c_int32), ("prop_shard", C.c_int32),
     ]
 
 
 class rt_slab_buffers(C.Structure):
     _fields_ = [("xchg_rho", C.c_void_p), ("xchg_rho_count", C.c_int64), ("xchg_H", C.c_void_p),
                 ("xchg_H_count", C.c_int64), ("slab_offset", C.c_int64), ("slab_count", C.c_int64)]
+
+
+class rt_shard_buffers(C.Structure):
+    _fields_ = [("Y", C.c_void_p), ("C", C.c_void_p), ("S", C.c_void_p), ("P1re", C.c_void_p), ("P1im", C.c_void_p),
+                ("block_count", C.c_int64), ("total_count", C.c_int64), ("prop_shards", C.c_int32),
+                ("prop_shard", C.c_int32)]
 
 
 class RTError(RuntimeError):
@@ -82,6 +90,7 @@ def _load():
         "rt_op_propagate": [vp, dp, dp, dp, dp, dp], "rt_op_hartree": [vp, dp, dp, i32], "rt_op_vxc": [vp, dp, dp],
         "rt_timing_enable": [vp, i32], "rt_timing_read": [vp, dp, dp], "rt_get_convergence": [vp, dp, dp],
         "rt_slab_get_buffers": [vp, C.POINTER(rt_slab_buffers)], "rt_slab_phase": [vp, i32, i32],
+        "rt_slab_get_shard": [vp, C.POINTER(rt_shard_buffers)], "rt_slab_more_updates": [vp, C.POINTER(C.c_int32)],
         "rt_get_dipole_series": [vp, C.c_int64, i32, dp], "rt_get_energy": [vp, C.POINTER(C.c_double)],
         "rt_state_bytes": [vp, i64p], "rt_get_state": [vp, vp], "rt_set_state": [vp, vp],
         "rt_spectrum": [dp, i32, C.c_double, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
@@ -328,6 +337,18 @@ def rt_slab_phase(h, phase: int, it: int = 0):
     _check(h, _lib.rt_slab_phase(h, int(phase), int(it)))
 
 
+def rt_slab_get_shard(h) -> rt_shard_buffers:
+    b = rt_shard_buffers()
+    _check(h, _lib.rt_slab_get_shard(h, C.byref(b)))
+    return b
+
+
+def rt_slab_more_updates(h) -> bool:
+    m = C.c_int32(0)
+    _check(h, _lib.rt_slab_more_updates(h, C.byref(m)))
+    return bool(m.value)
+
+
 # ---- convenience wrapper (the call a user makes) -------------------------------------------------------
 
 class RTTDDFT:
@@ -336,12 +357,13 @@ class RTTDDFT:
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
                  nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
                  device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0,
-                 slab=None, history=0):
+                 slab=None, history=0, prop_shard=None):
         """``slab = (x0, nx_local)``: the handle owns those x-planes and ``phi`` is [norb][nx_local*ny*nz]
-        (rt_slab_* entry points; see slab.py)."""
+        (rt_slab_* entry points; see slab.py).  ``prop_shard = (rank, nranks)``: row-sharded N x N propagator."""
         cfg = rt_config()
         cfg.slab_x0, cfg.slab_nx = (int(slab[0]), int(slab[1])) if slab else (0, 0)
         cfg.history = int(history)
+        cfg.prop_shards, cfg.prop_shard = (int(prop_shard[1]), int(prop_shard[0])) if prop_shard else (0, 0)
         cfg.propagator = {"taylor": RT_PROP_TAYLOR, "commutator": RT_PROP_COMMUTATOR}[propagator]
         cfg.max_order, cfg.dP_thrs, cfg.H_thrs, cfg.max_hupdates = int(max_order), float(dP_thrs), float(H_thrs), int(max_hupdates)
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)

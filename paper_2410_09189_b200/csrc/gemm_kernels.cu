@@ -311,7 +311,7 @@ gemm_abt_kernel(GemmArgs ga) {
   const int g = lane >> 2, c = lane & 3;
   const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
   const int N = ga.N, ldn = ga.ldn;
-  const int i0 = blockIdx.y * BM, j0 = blockIdx.x * BN;
+  const int i0 = ga.row_beg + blockIdx.y * BM, j0 = blockIdx.x * BN;
   const int nk1 = (N + BK - 1) / BK;
   const int nk = ga.A1 ? 2 * nk1 : nk1;
 
@@ -395,7 +395,9 @@ static void launch_gemm_variant(const GemmArgs& g, cudaStream_t st) {
     cudaFuncSetAttribute(gemm_abt_kernel<FA_, FB_, WM_, WN_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr = true;
   }
-  gemm_abt_kernel<FA_, FB_, WM_, WN_><<<dim3((g.N + bn - 1) / bn, (g.N + bm - 1) / bm), 32 * WM_ * WN_, smem, st>>>(g);
+  const int rows = g.row_end - g.row_beg;
+  if (rows <= 0) return;
+  gemm_abt_kernel<FA_, FB_, WM_, WN_><<<dim3((g.N + bn - 1) / bn, (rows + bm - 1) / bm), 32 * WM_ * WN_, smem, st>>>(g);
 }
 
 void launch_gemm_abt(const GemmArgs& g, cudaStream_t st) {

@@ -375,16 +375,32 @@ void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUte
 }
 
 // ======================================================================================================
-// a3/a4 N x N GEMM
+// a3/a4 N x N GEMM (stream-K)
 // ======================================================================================================
+// The work of one launch is the list of (tile, pipeline stage) units, ntiles x nk of them, in tile-list order.  It is cut
+// into G = min(#SMs, ...) contiguous RANGES of (almost) equal length and every CTA processes one range, so all SMs
+// finish together whatever ntiles is (round 1: one CTA per 128 x 128 tile -- N = 2400 gave 190 upper tiles on 148 SMs,
+// two waves at 64 % fill, ELDYN at 0.58 of the DMMA roof).  A tile that straddles ranges is finished by the CTA that
+// holds its FIRST stages (the "head", at the end of that CTA's range); the CTAs holding later stages (the "tails", at
+// the very start of their ranges) park their partial accumulators in a workspace slot and raise a flag.  The head adds
+// the slots in range order, so the summation order -- and therefore every bit of the result -- is fixed by (N, G)
+// alone.  Deadlock freedom does not depend on all CTAs being co-resident (three delta-kick handles share the GPU on
+// three streams): ranges are handed out through a ticket counter in reverse order, so a head only ever waits for CTAs
+// that took their ticket BEFORE it, i.e. that are already running or done.
 struct GemmTmaArgs {
   int N, ldn, nterms;
-  int sym;                 // +1: D is symmetric, -1: antisymmetric -> only tiles ti <= tj are computed and mirrored
-  const int2* tiles;       // upper-triangular tile list (sym != 0)
+  int sym;                 // +1: D is symmetric, -1: antisymmetric -> the tile list holds ti <= tj only and the mirror
+                           //  image is written too; 0: plain tile list
+  const int2* tiles;       // tile list (ti, tj)
+  int ntiles;
   double alpha0, alpha1;
   double* D; double* Z1; double beta1; double* Z2; double beta2;
   const int* skip;         // non-zero -> no-op (orders past convergence of the commutator series)
+  double* ws;              // [G][TILE*TILE] partial accumulators of the tail items, indexed by range
+  int* sync;               // [0] = ticket counter, [1] = finished-CTA counter, [2 + p] = flag of range p (0 = empty)
 };
+
+__device__ __forceinline__ long long range_begin(long long total, int G, int j) { return total * j / G; }
 
 __global__ void __launch_bounds__(NTHREADS, 1)
 gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmB0,
@@ -395,100 +411,186 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
   Bars* bars = reinterpret_cast<Bars*>(wsm + ST * BK);
+  int* sh_ticket = reinterpret_cast<int*>(bars + 1);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  init_bars(bars);
+  const int G = gridDim.x;
+  if (threadIdx.x == 0) *sh_ticket = atomicAdd(&ga.sync[0], 1);
+  init_bars(bars);                                  // ends with __syncthreads
+  const int range = G - 1 - *sh_ticket;             // later tickets take earlier ranges (see above)
   const int N = ga.N, ldn = ga.ldn;
-  int i0, j0;
-  if (ga.sym) { const int2 tt = ga.tiles[blockIdx.x]; i0 = tt.x * TILE; j0 = tt.y * TILE; }
-  else { i0 = blockIdx.y * TILE; j0 = blockIdx.x * TILE; }
   const int nk1 = (N + BK - 1) / BK;
   const int nk = ga.nterms * nk1;
+  const long long total = (long long)ga.ntiles * nk;
+  const long long u0 = range_begin(total, G, range), u1 = range_begin(total, G, range + 1);
 
   if (warp >= NCONS) {
     regs_producer();
     if (warp == NCONS && lane == 0) {
       tma_prefetch_desc(&tmA0);
       tma_prefetch_desc(&tmB0);
-      for (int kt = 0; kt < nk; ++kt) {
-        const int slot = kt % ST;
-        if (kt >= ST) mbar_wait(smem_u32(&bars->empty[slot]), ((kt / ST) - 1) & 1);
-        const uint32_t full = smem_u32(&bars->full[slot]);
-        mbar_expect_tx(full, 2 * TILE_BYTES);
-        const bool second = kt >= nk1;
-        const int k0 = (second ? kt - nk1 : kt) * BK;
-        double* sA = tilesm + (size_t)slot * STAGE_D;
-        tma_load_2d(sA, second ? &tmA1 : &tmA0, k0, i0, full);
-        tma_load_2d(sA + TILE_D, second ? &tmB1 : &tmB0, k0, j0, full);
+      long long it = 0;
+      for (long long u = u0; u < u1;) {
+        const int t = (int)(u / nk), kt0 = (int)(u - (long long)t * nk);
+        const int kt1 = (int)((u1 - u < nk - kt0) ? (kt0 + (u1 - u)) : nk);
+        const int2 tt = ga.tiles[t];
+        const int i0 = tt.x * TILE, j0 = tt.y * TILE;
+        for (int kt = kt0; kt < kt1; ++kt, ++it) {
+          const int slot = (int)(it % ST);
+          if (it >= ST) mbar_wait(smem_u32(&bars->empty[slot]), (uint32_t)((it / ST) - 1) & 1);
+          const uint32_t full = smem_u32(&bars->full[slot]);
+          mbar_expect_tx(full, 2 * TILE_BYTES);
+          const bool second = kt >= nk1;
+          const int k0 = (second ? kt - nk1 : kt) * BK;
+          double* sA = tilesm + (size_t)slot * STAGE_D;
+          tma_load_2d(sA, second ? &tmA1 : &tmA0, k0, i0, full);
+          tma_load_2d(sA + TILE_D, second ? &tmB1 : &tmB0, k0, j0, full);
+        }
+        u += kt1 - kt0;
       }
     }
-    return;
-  }
-
-  regs_consumer();
-  const int g = lane >> 2, c = lane & 3, pg = perm8(g);
-  const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
-  double acc[FA][FB][2];
-#pragma unroll
-  for (int a = 0; a < FA; ++a)
-#pragma unroll
-    for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
-  const double ratio = ga.nterms == 2 ? ga.alpha1 / ga.alpha0 : 1.0;
-
-  for (int kt = 0; kt < nk; ++kt) {
-    const int slot = kt % ST;
-    mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
-    if (kt == nk1 && ratio != 1.0) {            // fold alpha1/alpha0 (+-1 in this library: exact) into the accumulators
-      const double inv = 1.0 / ratio;
+  } else {
+    regs_consumer();
+    const int g = lane >> 2, c = lane & 3, pg = perm8(g);
+    const int wrow = (warp / WN) * (8 * FA), wcol = (warp % WN) * (8 * FB);
+    const int ctid = threadIdx.x;                      // 0 .. 255
+    const double ratio = ga.nterms == 2 ? ga.alpha1 / ga.alpha0 : 1.0;
+    const double inv = 1.0 / ratio;                     // +-1 in this library: exact
+    const double fin = (ga.nterms == 2 && ratio != 1.0) ? ga.alpha0 * ratio : ga.alpha0;
+    const double msign = (double)ga.sym;
+    long long it = 0;
+    for (long long u = u0; u < u1;) {
+      const int t = (int)(u / nk), kt0 = (int)(u - (long long)t * nk);
+      const int kt1 = (int)((u1 - u < nk - kt0) ? (kt0 + (u1 - u)) : nk);
+      const int2 tt = ga.tiles[t];
+      const int i0 = tt.x * TILE, j0 = tt.y * TILE;
+      double acc[FA][FB][2];
 #pragma unroll
       for (int a = 0; a < FA; ++a)
 #pragma unroll
-        for (int b = 0; b < FB; ++b) { acc[a][b][0] *= inv; acc[a][b][1] *= inv; }
-    }
-    const double* sA = tilesm + (size_t)slot * STAGE_D;
-    mma_stage_kc_tma<FA, FB, false>(acc, sA, sA + TILE_D, nullptr, wrow, wcol, pg, c);
-    __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
-  }
-  const double fin = (ga.nterms == 2 && ratio != 1.0) ? ga.alpha0 * ratio : ga.alpha0;
-  const bool diag = ga.sym && i0 == j0;
-  const double msign = (double)ga.sym;
+        for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
 
+      for (int kt = kt0; kt < kt1; ++kt, ++it) {
+        const int slot = (int)(it % ST);
+        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        if (kt == nk1 && ratio != 1.0) {            // fold alpha1/alpha0 into the first term's sum
 #pragma unroll
-  for (int a = 0; a < FA; ++a) {
-    const int row = i0 + wrow + 8 * a + pg;
-    if (row < N) {
+          for (int a = 0; a < FA; ++a)
 #pragma unroll
-      for (int b = 0; b < FB; ++b) {
+            for (int b = 0; b < FB; ++b) { acc[a][b][0] *= inv; acc[a][b][1] *= inv; }
+        }
+        const double* sA = tilesm + (size_t)slot * STAGE_D;
+        mma_stage_kc_tma<FA, FB, false>(acc, sA, sA + TILE_D, nullptr, wrow, wcol, pg, c);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+      }
+      if (ga.nterms == 2 && ratio != 1.0 && kt1 <= nk1) {      // the item never reached the second term
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          const int col = j0 + wcol + 8 * b + c + 4 * e;
-          if (col < N && (!diag || col >= row)) {
-            const long long o = (long long)row * ldn + col;
-            double d = fin * acc[a][b][e];
-            if (ga.sym < 0 && row == col) d = 0.0;
-            if (ga.D) ga.D[o] = d;
-            if (ga.Z1) ga.Z1[o] += ga.beta1 * d;
-            if (ga.Z2) ga.Z2[o] += ga.beta2 * d;
-            if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
-              const long long om = (long long)col * ldn + row;
-              const double dm = msign * d;
-              if (ga.D) ga.D[om] = dm;
-              if (ga.Z1) ga.Z1[om] += ga.beta1 * dm;
-              if (ga.Z2) ga.Z2[om] += ga.beta2 * dm;
+        for (int a = 0; a < FA; ++a)
+#pragma unroll
+          for (int b = 0; b < FB; ++b) { acc[a][b][0] *= inv; acc[a][b][1] *= inv; }
+      }
+      u += kt1 - kt0;
+
+      if (kt0 > 0) {
+        // ---- tail of a tile whose head lives in an earlier range: park the partial sums, raise the flag ----
+        double* slotp = ga.ws + (size_t)range * (TILE * TILE);
+#pragma unroll
+        for (int a = 0; a < FA; ++a)
+#pragma unroll
+          for (int b = 0; b < FB; ++b)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) slotp[((a * FB + b) * 2 + e) * (32 * NCONS) + ctid] = acc[a][b][e];
+        __threadfence();
+        consumer_sync(32 * NCONS);
+        if (ctid == 0) {
+          __threadfence();
+          atomicExch(&ga.sync[2 + range], 1);
+        }
+        continue;
+      }
+      if (kt1 < nk) {
+        // ---- head of a tile that continues in the following ranges: add their partial sums in range order ----
+        const long long tile_end = (long long)(t + 1) * nk;
+        for (int p = range + 1; p < G && range_begin(total, G, p) < tile_end; ++p) {
+          if (ctid == 0) {
+            const long long t0 = clock64();
+            while (atomicAdd(&ga.sync[2 + p], 0) == 0) {
+              if (clock64() - t0 > 20000000000LL) __trap();
+            }
+            __threadfence();
+          }
+          consumer_sync(32 * NCONS);
+          const double* slotp = ga.ws + (size_t)p * (TILE * TILE);
+#pragma unroll
+          for (int a = 0; a < FA; ++a)
+#pragma unroll
+            for (int b = 0; b < FB; ++b)
+#pragma unroll
+              for (int e = 0; e < 2; ++e) acc[a][b][e] += __ldcg(slotp + ((a * FB + b) * 2 + e) * (32 * NCONS) + ctid);
+          consumer_sync(32 * NCONS);
+          if (ctid == 0) atomicExch(&ga.sync[2 + p], 0);            // self-cleaning: the next launch finds every flag at 0
+        }
+      }
+
+      // ---- epilogue of a complete tile ----
+      const bool diag = ga.sym && i0 == j0;
+#pragma unroll
+      for (int a = 0; a < FA; ++a) {
+        const int row = i0 + wrow + 8 * a + pg;
+        if (row < N) {
+#pragma unroll
+          for (int b = 0; b < FB; ++b) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const int col = j0 + wcol + 8 * b + c + 4 * e;
+              if (col < N && (!diag || col >= row)) {
+                const long long o = (long long)row * ldn + col;
+                double d = fin * acc[a][b][e];
+                if (ga.sym < 0 && row == col) d = 0.0;
+                if (ga.D) ga.D[o] = d;
+                if (ga.Z1) ga.Z1[o] += ga.beta1 * d;
+                if (ga.Z2) ga.Z2[o] += ga.beta2 * d;
+                if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
+                  const long long om = (long long)col * ldn + row;
+                  const double dm = msign * d;
+                  if (ga.D) ga.D[om] = dm;
+                  if (ga.Z1) ga.Z1[om] += ga.beta1 * dm;
+                  if (ga.Z2) ga.Z2[om] += ga.beta2 * dm;
+                }
+              }
             }
           }
         }
       }
     }
   }
+  // the last CTA to finish rewinds the two counters for the next launch
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (atomicAdd(&ga.sync[1], 1) == G - 1) {
+      atomicExch(&ga.sync[0], 0);
+      atomicExch(&ga.sync[1], 0);
+    }
+  }
 }
 
+int gemm_tma_grid(int ntiles, int N, int nterms, int sms) {
+  const long long total = (long long)ntiles * nterms * ((N + BK - 1) / BK);
+  long long g = total / 8;                      // at least 8 stages per range
+  if (g > sms) g = sms;
+  return (int)(g < 1 ? 1 : g);
+}
+size_t gemm_tma_ws_doubles(int sms) { return (size_t)sms * TILE * TILE; }
+size_t gemm_tma_sync_ints(int sms) { return (size_t)sms + 2; }
+
 void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
-                         const CUtensorMap& tmB1, int sym, const int2* tiles, cudaStream_t st) {
-  GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, sym, tiles, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2, g.skip};
-  const int nt = (g.N + TILE - 1) / TILE;
-  if (sym) gemm_abt_tma_kernel<<<nt * (nt + 1) / 2, NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
-  else gemm_abt_tma_kernel<<<dim3(nt, nt), NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
+                         const CUtensorMap& tmB1, int sym, const int2* tiles, int ntiles, double* ws, int* sync, int sms,
+                         cudaStream_t st) {
+  if (ntiles <= 0) return;
+  GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, sym, tiles, ntiles, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2,
+                g.skip, ws, sync};
+  const int grid = gemm_tma_grid(ntiles, g.N, a.nterms, sms);
+  gemm_abt_tma_kernel<<<grid, NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
 }
 
 int init_tma_kernels() {

@@ -405,6 +405,20 @@ __global__ void set_diag_kernel(int N, int ldn, double* __restrict__ M, const do
   if (j >= ldn) return;
   M[(long long)i * ldn + j] = (i == j) ? d[i] : 0.0;
 }
+__global__ void hermitize_kernel(int N, int ldn, double* Re, double* Im) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;      // (i, j), j > i is the source
+  if (j >= N) return;
+  if (j > i) {
+    Re[(long long)j * ldn + i] = Re[(long long)i * ldn + j];
+    Im[(long long)j * ldn + i] = -Im[(long long)i * ldn + j];
+  } else if (j == i) {
+    Im[(long long)i * ldn + i] = 0.0;
+  }
+}
+void launch_hermitize(int N, int ldn, double* Re, double* Im, cudaStream_t st) {
+  hermitize_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, Re, Im);
+}
+
 void launch_set_diag(int N, int ldn, double* M, const double* diag, cudaStream_t st) {
   set_diag_kernel<<<dim3((ldn + 127) / 128, N), 128, 0, st>>>(N, ldn, M, diag);
 }

@@ -60,7 +60,18 @@ struct rt_ctx {
   double *Hm1 = nullptr, *H0 = nullptr, *H1 = nullptr, *X = nullptr, *Ya = nullptr, *Yb = nullptr, *Yc = nullptr,
          *Cm = nullptr, *Sc = nullptr, *Sm = nullptr, *P0r = nullptr, *P0i = nullptr, *P1r = nullptr, *P1i = nullptr,
          *W = nullptr;
-  int2* d_tiles = nullptr;
+  int2* d_tiles = nullptr;        // upper tiles (ti <= tj), class-ordered for the projection; also the sym GEMMs' list
+  int2* d_tiles_full = nullptr;   // all ntile x ntile tiles, row-major (plain GEMMs; a row block is a contiguous piece)
+  int ntile = 0;
+  double* gemm_ws = nullptr;      // stream-K fix-up workspace and flags of the TMA N x N GEMM (gemm_tma.cu)
+  int* gemm_sync = nullptr;
+  // row-sharded propagator: rank `shard` of `nshard` owns the rows [row_beg, row_end) of every N x N product
+  int nshard = 1, shard = 0, shard_rows = 0, row_beg = 0, row_end = 0;
+  size_t nn_alloc = 0;            // doubles per N x N buffer (rows padded to nshard * shard_rows for the all-gathers)
+  int slab_more = 0;              // decision of the last RT_SLAB_CHECK: another Hamiltonian update is needed
+  std::map<int, cudaGraphExec_t> phase_exec;      // slab phases captured as CUDA graphs, key = 2 * phase + (it == 0)
+  std::map<int, int64_t> phase_launches;
+  std::vector<cudaGraph_t> phase_graphs;
   DensSeg* d_segs = nullptr;
   std::vector<DensSeg> segs;
   ProjectPlan pp{};
@@ -267,15 +278,25 @@ void stage_end(rt_ctx* c) {
 }
 
 // ---- the stages ------------------------------------------------------------------------------------
+// sym = +1 / -1: D is known to be (anti)symmetric: upper tiles + mirror image.  rows = true: this launch computes only
+// the row block [row_beg, row_end) that this rank owns (row-sharded propagator; nshard = 1: the whole matrix) -- as a
+// plain product, because the mirror image of a row block belongs to other ranks.
 void enqueue_gemm(rt_ctx* c, int sym, const double* A0, const double* B0, double a0, const double* A1,
                   const double* B1, double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr,
-                  double b2 = 0, const int* skip = nullptr) {
-  GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2, skip};
+                  double b2 = 0, const int* skip = nullptr, bool rows = false) {
+  const bool shard = rows && c->nshard > 1;
+  GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2, skip, shard ? c->row_beg : 0,
+             shard ? c->row_end : c->N};
+  if (g.row_end <= g.row_beg) return;                       // this rank owns no rows (more ranks than tile rows)
   if (c->use_tma && c->N > GEMM_SMALL_N) {
     const CUtensorMap& mA0 = nn_map(c, A0);
     const CUtensorMap& mB0 = nn_map(c, B0);
-    launch_gemm_abt_tma(g, mA0, mB0, A1 ? nn_map(c, A1) : mA0, B1 ? nn_map(c, B1) : mB0, sym, c->d_tiles,
-                        c->st);
+    const int2* tiles = c->d_tiles;
+    int ntiles = c->pp.T;
+    if (shard) { sym = 0; tiles = c->d_tiles_full + (size_t)(c->row_beg / TILE) * c->ntile; ntiles = ((c->row_end - c->row_beg + TILE - 1) / TILE) * c->ntile; }
+    else if (!sym) { tiles = c->d_tiles_full; ntiles = c->ntile * c->ntile; }
+    launch_gemm_abt_tma(g, mA0, mB0, A1 ? nn_map(c, A1) : mA0, B1 ? nn_map(c, B1) : mB0, sym, tiles, ntiles, c->gemm_ws,
+                        c->gemm_sync, c->sms, c->st);
   } else {
     launch_gemm_abt(g, c->st);
   }
@@ -308,6 +329,48 @@ void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, doub
   enqueue_gemm(c, 0, c->Cm, Ai, -1.0, c->Sm, Ar, -1.0, c->Yc);
   enqueue_gemm(c, 1, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, Or);      // P1 Hermitian: Re symmetric,
   enqueue_gemm(c, -1, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, Oi);      // Im antisymmetric
+}
+
+// ---- the same propagation with the N^3 work sharded over ranks by row blocks ("once N exceeds a few
+// thousands" the multi-GPU product wins over the replicated one).  D = A B^T needs only the rows of A that the rank
+// owns and all of B, so a chain prev -> prev * Y stays local; three points need a matrix complete on every rank, and
+// the caller all-gathers the row blocks there (rt_slab_get_shard):
+//   A: Y = X X^T                                                        -> gather Y
+//   B: powers of Y, C = cos X, Sc = sinc-series, S = Sc X, Yr, Yi        -> gather C, S   (right factors of the last two)
+//   C: P1r = Yr C - Yi S, P1i = Yr S + Yi C                              -> gather P1r, P1i
+//   D: P1 made exactly Hermitian from its upper triangle (both triangles were computed separately), then the density
+// Every element is computed by exactly one rank, so all ranks hold bit-identical matrices after each gather.
+void enqueue_shard_A(rt_ctx* c, int it) {
+  stage_begin(c, RT_STAGE_ELDYN);
+  if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);
+  launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st);       // lines 11, 14 (replicated)
+  c->launches += 1;
+  enqueue_gemm(c, 0, c->X, c->X, 1.0, nullptr, nullptr, 0, c->Ya, nullptr, 0, nullptr, 0, nullptr, true);
+  stage_end(c);
+}
+void enqueue_shard_B(rt_ctx* c) {
+  stage_begin(c, RT_STAGE_ELDYN);
+  launch_series_init(c->N, c->ldn, c->Ya, c->Cm, -0.5, c->Sc, -1.0 / 6.0, c->st);    // elementwise on the whole matrix
+  c->launches += 1;
+  double ck = -0.5, sk = -1.0 / 6.0;
+  const double* prev = c->Ya;
+  for (int k = 2; k <= c->q; ++k) {
+    ck = -ck / ((2.0 * k - 1.0) * (2.0 * k));
+    sk = -sk / ((2.0 * k) * (2.0 * k + 1.0));
+    double* cur = (k < c->q) ? ((k & 1) ? c->Yc : c->Yb) : nullptr;
+    enqueue_gemm(c, 0, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk, nullptr, true);
+    prev = cur;
+  }
+  enqueue_gemm(c, 0, c->Sc, c->X, 1.0, nullptr, nullptr, 0, c->Sm, nullptr, 0, nullptr, 0, nullptr, true);   // S = Sc X (commute)
+  enqueue_gemm(c, 0, c->Cm, c->P0r, 1.0, c->Sm, c->P0i, -1.0, c->Yb, nullptr, 0, nullptr, 0, nullptr, true);
+  enqueue_gemm(c, 0, c->Cm, c->P0i, -1.0, c->Sm, c->P0r, -1.0, c->Yc, nullptr, 0, nullptr, 0, nullptr, true);
+  stage_end(c);
+}
+void enqueue_shard_C(rt_ctx* c) {
+  stage_begin(c, RT_STAGE_ELDYN);
+  enqueue_gemm(c, 0, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, c->P1r, nullptr, 0, nullptr, 0, nullptr, true);
+  enqueue_gemm(c, 0, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, c->P1i, nullptr, 0, nullptr, 0, nullptr, true);
+  stage_end(c);
 }
 
 // The paper's propagator (Eq. 39, Alg. 1 lines 15-23 L375-L392) with S = 1 and Hbar real symmetric (L433):
@@ -377,6 +440,13 @@ void enqueue_project_dv(rt_ctx* c, double* H) {
   enqueue_project(c, c->op_u, c->x0 == 0 ? c->d_eps : nullptr, H);
 }
 
+void enqueue_density_stage(rt_ctx* c) {
+  stage_begin(c, RT_STAGE_RHO);
+  if (c->slab) cudaMemsetAsync(c->rho, 0, (size_t)(c->Ng + 8) * 8, c->st);                     // other ranks' slabs
+  enqueue_density(c, c->P1r, c->rho + c->slab_off, c->rho0 + c->slab_off);                     // Eq. 27 + line 27
+  stage_end(c);
+}
+
 // First half of a Hamiltonian update, Algorithm 1 lines 14-23 + Eq. 27 (`it` = 0 also extrapolates H1, line 11):
 // mean Hamiltonian, propagation, density of this handle's grid points (+ partial dipole / charge sums).
 void enqueue_update_propagate(rt_ctx* c, int it) {
@@ -386,11 +456,7 @@ void enqueue_update_propagate(rt_ctx* c, int it) {
   c->launches += 1;
   enqueue_propagate(c, c->P0r, c->P0i, c->P1r, c->P1i);                                        // Eq. 15 / Eq. 39
   stage_end(c);
-
-  stage_begin(c, RT_STAGE_RHO);
-  if (c->slab) cudaMemsetAsync(c->rho, 0, (size_t)(c->Ng + 8) * 8, c->st);                     // other ranks' slabs
-  enqueue_density(c, c->P1r, c->rho + c->slab_off, c->rho0 + c->slab_off);                     // Eq. 27 + line 27
-  stage_end(c);
+  enqueue_density_stage(c);
 }
 
 // Second half, lines 24-25: potential update on the whole grid from the (complete) density, then the projection
@@ -411,7 +477,7 @@ void enqueue_update_potential(rt_ctx* c) {
   if (c->dynamic)                                                                              // H1_old <- H1
     cudaMemcpyAsync(c->Ya, c->H1, (size_t)c->N * c->ldn * 8, cudaMemcpyDeviceToDevice, c->st);
   enqueue_project_dv(c, c->H1);                                                                // line 25
-  if (c->dynamic) {
+  if (c->dynamic && !c->slab) {               // a slab holds a partial sum here: RT_SLAB_CHECK measures after the all-reduce
     launch_maxabs_diff(c->N, c->ldn, c->H1, c->Ya, c->d_cs, c->st);                            // line 24
     c->launches += 1;
   }
@@ -487,6 +553,8 @@ int rt_destroy(rt_handle c) {
     if (c->gexec_upd[i]) cudaGraphExecDestroy(c->gexec_upd[i]);
     if (c->graph_upd[i]) cudaGraphDestroy(c->graph_upd[i]);
   }
+  for (auto& kv : c->phase_exec) cudaGraphExecDestroy(kv.second);
+  for (auto g : c->phase_graphs) cudaGraphDestroy(g);
   for (auto& ep : c->ev_used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
   for (auto& ep : c->ev_free) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
   for (void* p : c->allocs) cudaFree(p);
@@ -508,8 +576,12 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     return fail(c, RT_EINVAL, "rt_create: unknown propagator");
   if (cfg->slab_nx < 0 || cfg->slab_x0 < 0 || (cfg->slab_nx > 0 && cfg->slab_x0 + cfg->slab_nx > cfg->nx))
     return fail(c, RT_EINVAL, "rt_create: slab [slab_x0, slab_x0 + slab_nx) must lie inside [0, nx)");
-  if (cfg->slab_nx > 0 && cfg->H_thrs > 0.0)
-    return fail(c, RT_EINVAL, "rt_create: the dynamic H_thrs loop is driven by rt_step and is not available on a slab handle");
+  if (cfg->prop_shards < 0 || (cfg->prop_shards > 1 && (cfg->prop_shard < 0 || cfg->prop_shard >= cfg->prop_shards)))
+    return fail(c, RT_EINVAL, "rt_create: prop_shard must lie in [0, prop_shards)");
+  if (cfg->prop_shards > 1 && cfg->slab_nx == 0)
+    return fail(c, RT_EINVAL, "rt_create: the row-sharded propagator is part of the slab protocol (set slab_nx)");
+  if (cfg->prop_shards > 1 && cfg->propagator != RT_PROP_TAYLOR)
+    return fail(c, RT_EINVAL, "rt_create: the row-sharded propagator implements the Taylor mode only");
   if (cfg->history < 0) return fail(c, RT_EINVAL, "rt_create: history < 0");
   if (cfg->max_order < 0 || cfg->max_order > MAX_ORDER || cfg->max_hupdates < 0 || !(cfg->dP_thrs >= 0.0) ||
       !(cfg->H_thrs >= 0.0))
@@ -531,6 +603,13 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   c->cfg = *cfg;
   c->N = cfg->norb;
   c->ldn = roundup(c->N, 8);
+  c->ntile = (c->N + TILE - 1) / TILE;
+  c->nshard = cfg->prop_shards > 1 ? cfg->prop_shards : 1;
+  c->shard = c->nshard > 1 ? cfg->prop_shard : 0;
+  c->shard_rows = ((c->ntile + c->nshard - 1) / c->nshard) * TILE;       // whole tile rows per rank
+  c->row_beg = std::min(c->N, c->shard * c->shard_rows);
+  c->row_end = std::min(c->N, (c->shard + 1) * c->shard_rows);
+  c->nn_alloc = (size_t)std::max(c->N, c->nshard * c->shard_rows) * c->ldn;
   c->gd = GridDims{cfg->nx, cfg->ny, cfg->nz};
   c->Ng = (long long)cfg->nx * cfg->ny * cfg->nz;
   c->Ngl = c->Ng;
@@ -693,7 +772,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   {
     size_t freeb = 0, totalb = 0;
     CKC(cudaMemGetInfo(&freeb, &totalb));
-    double need = 15.0 * N * (double)ldn * 8 + (double)c->pp.S * N * ldn * 8 + (double)c->dp.ntypes * Ng * 8 + 12.0 * NgF * 8;
+    double need = 15.0 * (double)c->nn_alloc * 8 + (double)c->pp.S * N * ldn * 8 + (double)c->dp.ntypes * Ng * 8 + 12.0 * NgF * 8;
     if (!(cfg->flags & RT_PHI_DEVICE)) need += (double)N * Ng * 8;
     if (need > (double)freeb) {
       char buf[256];
@@ -730,7 +809,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     const int e = init_tma_kernels();
     if (e != 0) FAIL_CREATE(RT_ECUDA, std::string("init_tma_kernels: ") + cudaGetErrorString((cudaError_t)e));
   }
-  const size_t nn = (size_t)N * ldn;
+  const size_t nn = c->nn_alloc;        // N x ldn, rows padded so that every rank's row block has the same size
   ALLOC(c->d_eps, N); ALLOC(c->d_occ, N); ALLOC(c->d_E, 8); ALLOC(c->d_energy, 8);
   c->hist_cap = cfg->history;
   if (c->hist_cap) {
@@ -747,7 +826,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   double** mats[] = {&c->Hm1, &c->H0, &c->H1, &c->X, &c->Ya, &c->Yb, &c->Yc, &c->Cm, &c->Sc, &c->Sm,
                      &c->P0r, &c->P0i, &c->P1r, &c->P1i};
   for (double** mp : mats) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
-  ALLOC(c->W, (size_t)c->pp.S * nn);
+  ALLOC(c->W, (size_t)c->pp.S * N * ldn);
   // rho and the five sums share one allocation: it is the first exchange buffer of the slab mode
   ALLOC(c->rho, NgF + 8); ALLOC(c->rho0, NgF); ALLOC(c->vxc0, NgF);
   c->d_sums = c->rho + NgF;
@@ -774,6 +853,16 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     for (int ti = 0; ti < ntile; ++ti) tiles.push_back(make_int2(ti, ti));
     ALLOC(c->d_tiles, tiles.size());
     CKC(cudaMemcpyAsync(c->d_tiles, tiles.data(), tiles.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
+    std::vector<int2> full;
+    for (int ti = 0; ti < ntile; ++ti)
+      for (int tj = 0; tj < ntile; ++tj) full.push_back(make_int2(ti, tj));
+    ALLOC(c->d_tiles_full, full.size());
+    CKC(cudaMemcpyAsync(c->d_tiles_full, full.data(), full.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
+    if (c->use_tma && N > GEMM_SMALL_N) {
+      ALLOC(c->gemm_ws, gemm_tma_ws_doubles(c->sms));
+      ALLOC(c->gemm_sync, gemm_tma_sync_ints(c->sms));
+      CKC(cudaMemsetAsync(c->gemm_sync, 0, gemm_tma_sync_ints(c->sms) * sizeof(int), c->st));
+    }
     CKC(cudaStreamSynchronize(c->st));
   }
   {
@@ -1273,11 +1362,53 @@ int rt_slab_get_buffers(rt_handle c, rt_slab_buffers* out) {
   return RT_OK;
 }
 
+int rt_slab_get_shard(rt_handle c, rt_shard_buffers* out) {
+  CHECK_HANDLE(c);
+  if (!out) return fail(c, RT_EINVAL, "rt_slab_get_shard: NULL");
+  if (!c->slab) return fail(c, RT_ESTATE, "rt_slab_get_shard: handle was created without a slab");
+  out->Y = c->Ya; out->C = c->Cm; out->S = c->Sm; out->P1re = c->P1r; out->P1im = c->P1i;
+  out->block_count = (int64_t)c->shard_rows * c->ldn;
+  out->total_count = (int64_t)c->nn_alloc;
+  out->prop_shards = c->nshard;
+  out->prop_shard = c->shard;
+  return RT_OK;
+}
+
+int rt_slab_more_updates(rt_handle c, int32_t* more) {
+  CHECK_HANDLE(c);
+  if (!more) return fail(c, RT_EINVAL, "rt_slab_more_updates: NULL");
+  if (!c->slab) return fail(c, RT_ESTATE, "rt_slab_more_updates: handle was created without a slab");
+  *more = c->slab_more;
+  return RT_OK;
+}
+
+namespace {
+// one phase of the slab protocol, enqueued on c->st (directly, or while that stream is capturing)
+void enqueue_slab_phase(rt_ctx* c, int phase, int it) {
+  switch (phase) {
+    case RT_SLAB_PROPAGATE: enqueue_update_propagate(c, it); break;
+    case RT_SLAB_PROP_A: enqueue_shard_A(c, it); break;
+    case RT_SLAB_PROP_B: enqueue_shard_B(c); break;
+    case RT_SLAB_PROP_C: enqueue_shard_C(c); break;
+    case RT_SLAB_PROP_D:
+      launch_hermitize(c->N, c->ldn, c->P1r, c->P1i, c->st);
+      c->launches += 1;
+      enqueue_density_stage(c);
+      break;
+    case RT_SLAB_POTENTIAL: enqueue_update_potential(c); break;
+    case RT_SLAB_SHIFT: enqueue_shift(c); break;
+    default: break;
+  }
+}
+}  // namespace
+
 int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
   CHECK_HANDLE(c);
   if (!c->slab) return fail(c, RT_ESTATE, "rt_slab_phase: handle was created without a slab");
   CK(cudaSetDevice(c->cfg.device));
   const size_t nn = (size_t)c->N * c->ldn * 8;
+  if (phase != RT_SLAB_INIT && c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
+  if (it < 0) return fail(c, RT_EINVAL, "rt_slab_phase: it < 0");
   switch (phase) {
     case RT_SLAB_INIT:            // xchg_rho holds rho0 of the whole grid, xchg_H holds H(t = 0)  (Alg. 1 lines 7-8)
       if (c->slab_state != 0) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT already done");
@@ -1291,20 +1422,67 @@ int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
       c->slab_state = 1;
       break;
     case RT_SLAB_PROPAGATE:
-      if (c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
-      if (it < 0) return fail(c, RT_EINVAL, "rt_slab_phase: it < 0");
-      enqueue_update_propagate(c, it);
-      break;
+      if (c->nshard > 1) return fail(c, RT_ESTATE, "rt_slab_phase: a handle with prop_shards > 1 propagates with RT_SLAB_PROP_A..D");
+      goto enqueue;
+    case RT_SLAB_PROP_A: case RT_SLAB_PROP_B: case RT_SLAB_PROP_C: case RT_SLAB_PROP_D:
+      if (c->nshard <= 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_PROP_A..D need prop_shards > 1");
+      goto enqueue;
     case RT_SLAB_POTENTIAL:
-      if (c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
-      enqueue_update_potential(c);
-      break;
     case RT_SLAB_SHIFT:
-      if (c->slab_state != 1) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT has not run");
-      enqueue_shift(c);
-      c->t += c->dt;
-      c->steps_done += 1;
+    enqueue: {
+      // The phases are fixed launch sequences: each (phase, first-update?) pair is captured once into a CUDA graph on a
+      // private stream and replayed afterwards (one launch instead of ~50 at the small configs).
+      const int key = 2 * phase + (it == 0 ? 1 : 0);
+      if (c->use_graph && !c->timing) {
+        auto ex = c->phase_exec.find(key);
+        if (ex == c->phase_exec.end()) {
+          cudaStream_t user = c->st, cap = nullptr;
+          CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+          c->st = cap;
+          const int64_t before = c->launches;
+          cudaGraph_t g = nullptr;
+          cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+          if (e == cudaSuccess) {
+            enqueue_slab_phase(c, phase, it);
+            e = cudaStreamEndCapture(cap, &g);
+          }
+          c->phase_launches[key] = c->launches - before;
+          c->launches = before;
+          c->st = user;
+          cudaStreamDestroy(cap);
+          cudaGraphExec_t gx = nullptr;
+          if (e == cudaSuccess) e = cudaGraphInstantiate(&gx, g, 0);
+          if (e != cudaSuccess) { cudaGetLastError(); return fail(c, RT_ECUDA, std::string("slab phase capture: ") + cudaGetErrorString(e)); }
+          c->phase_graphs.push_back(g);
+          ex = c->phase_exec.emplace(key, gx).first;
+        }
+        CK(cudaGraphLaunch(ex->second, c->st));
+        c->launches += c->phase_launches[key];
+      } else {
+        enqueue_slab_phase(c, phase, it);
+      }
+      if (phase == RT_SLAB_SHIFT) { c->t += c->dt; c->steps_done += 1; }
+      if (phase == RT_SLAB_POTENTIAL && !c->dynamic) { c->slab_more = (it + 1 < c->m) ? 1 : 0; c->last_hupdates = it + 1; }
       break;
+    }
+    case RT_SLAB_CHECK: {
+      // Alg. 1 lines 12-13 / 24 on a sharded system: xchg_H now holds the complete H1 (after the caller's all-reduce)
+      // and Ya the previous one; the norm is a max over replicated, bit-identical matrices, so every rank takes the
+      // same decision without another collective.  Fixed-count handles just count.
+      if (!c->dynamic) { c->slab_more = (it + 1 < c->m) ? 1 : 0; break; }
+      launch_maxabs_diff(c->N, c->ldn, c->H1, c->Ya, c->d_cs, c->st);
+      c->launches += 1;
+      ConvState hs;
+      CK(cudaMemcpyAsync(&hs, c->d_cs, sizeof hs, cudaMemcpyDeviceToHost, c->st));
+      if (int rc = sync_and_check(c)) return rc;
+      double herr;
+      memcpy(&herr, &hs.H_bits, 8);
+      c->last_H_err = herr;
+      c->last_hupdates = it + 1;
+      if (!std::isfinite(herr)) return fail(c, RT_ENUMERIC, "rt_slab_phase: non-finite H1");
+      c->slab_more = (herr > c->H_thrs && it + 1 < c->max_hup) ? 1 : 0;
+      break;
+    }
     default:
       return fail(c, RT_EINVAL, "rt_slab_phase: unknown phase");
   }

@@ -83,6 +83,9 @@ struct GemmArgs {
   double* Z1; double beta1;                             // may be nullptr
   double* Z2; double beta2;
   const int* skip;                                      // device flag (may be nullptr): non-zero -> the launch is a no-op
+  int row_beg, row_end;                                 // rows of D computed by this launch (multiples of TILE; row_end
+                                                        // clipped to N); 0, N = the whole matrix.  A row block is what
+                                                        // one rank of the sharded propagator owns
 };
 // N <= GEMM_SMALL_N32: 32 x 32 CTA tiles; N <= GEMM_SMALL_N: 64 x 64; above: 128 x 128 (rt_api.cu sends N > GEMM_SMALL_N
 // to the TMA-fed kernel when TMA is available)
@@ -102,8 +105,14 @@ void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUte
                         const double* phi, const DensSeg* segs, double* rho_part, int sms, cudaStream_t st);
 // sym = +1 / -1: the product is known to be symmetric / antisymmetric (polynomials of the symmetric X commute; P1 is
 // Hermitian): only the upper tiles (list `tiles`, ti <= tj) are computed and the mirror image is written too
+// `tiles` / `ntiles`: the 128 x 128 output tiles of this launch (sym != 0: upper tiles only).  Stream-K: the (tile, stage)
+// units are cut into one contiguous range per CTA; ws / sync are the fix-up workspace and flags (gemm_tma_ws_doubles,
+// gemm_tma_sync_ints; sync must be zero before the first launch and is left zero by every launch).
 void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUtensorMap& tmB0, const CUtensorMap& tmA1,
-                         const CUtensorMap& tmB1, int sym, const int2* tiles, cudaStream_t st);
+                         const CUtensorMap& tmB1, int sym, const int2* tiles, int ntiles, double* ws, int* sync, int sms,
+                         cudaStream_t st);
+size_t gemm_tma_ws_doubles(int sms);
+size_t gemm_tma_sync_ints(int sms);
 
 // ---- elementwise N x N (a2 and series glue) -------------------------------------------------------------
 // first != 0: H1 = 2 H0 - Hm1 first.  X = dt * ((H0 + H1)/2 - sigma I)
@@ -115,6 +124,9 @@ void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, d
 void launch_copy5(int N, int ldn, double* d0, const double* s0, double* d1, const double* s1, double* d2,
                   const double* s2, double* d3, const double* s3, cudaStream_t st);
 void launch_set_diag(int N, int ldn, double* M, const double* diag, cudaStream_t st);   // M = diag(d)
+// Re[j][i] = Re[i][j], Im[j][i] = -Im[i][j] for j > i, Im[i][i] = 0: makes P exactly Hermitian from its upper triangle
+// (the row-sharded propagator computes both triangles separately)
+void launch_hermitize(int N, int ldn, double* Re, double* Im, cudaStream_t st);
 
 // ---- grid kernels (a6, a7, a8) ---------------------------------------------------------------------------
 // rho[r] = sum_p rho_part[p][r]; block partial sums of {rho, x rho, y rho, z rho, rho - rho0} -> bsums[nb][5]

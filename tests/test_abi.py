@@ -31,7 +31,8 @@ def test_header_symbols_exported(built):
 def test_config_struct_layout(built):
     from paper_2410_09189_b200 import binding
     # values printed by a C program (sizeof / offsetof on include/rt_tddft.h, x86-64 SysV ABI)
-    assert ctypes.sizeof(binding.rt_config) == 152 and ctypes.sizeof(binding.rt_slab_buffers) == 48
+    assert ctypes.sizeof(binding.rt_config) == 160 and ctypes.sizeof(binding.rt_slab_buffers) == 48
+    assert ctypes.sizeof(binding.rt_shard_buffers) == 64 and binding.rt_shard_buffers.block_count.offset == 40
     assert binding.rt_config.dt.offset == 32 and binding.rt_config.E0.offset == 72
     assert binding.rt_config.flags.offset == 96 and binding.rt_config.stream.offset == 104
     assert binding.rt_config.propagator.offset == 112 and binding.rt_config.max_order.offset == 116
@@ -39,6 +40,7 @@ def test_config_struct_layout(built):
     assert binding.rt_config.max_hupdates.offset == 136
     assert binding.rt_config.slab_x0.offset == 140 and binding.rt_config.slab_nx.offset == 144
     assert binding.rt_config.history.offset == 148
+    assert binding.rt_config.prop_shards.offset == 152 and binding.rt_config.prop_shard.offset == 156
 
 
 def test_no_cpu_fallback(built):
