@@ -53,8 +53,13 @@ extern "C" {
 #define RT_NO_TMA     16u   /* use the cp.async versions of the DMMA kernels even where TMA applies (the
                                library falls back to them by itself when Ng is odd or phi is not 16-byte aligned) */
 
+#define RT_NONORTHOGONAL 32u /* Phi is a NON-orthonormal basis of real functions: S = dVol Phi Phi^T != 1 and P is propagated
+                               with Eq. 33-38.  Needs rt_create_general and RT_PROP_COMMUTATOR      */
+
 /* rt_config.propagator */
 #define RT_PROP_TAYLOR      0   /* U = exp(-i Hbar dt) by a fixed-degree Taylor polynomial, then P1 = U P0 U^dagger      */
+#define RT_XC_LDA_PZ81 0
+#define RT_XC_PBE      1
 #define RT_PROP_COMMUTATOR  1   /* the paper's own series applied to P: dP^(k) = (-i dt/k)[Hbar, dP^(k-1)],
                                    P1 = P0 + sum_k dP^(k) until max|dP^(k)| <= dP_thrs (Eq. 39, Alg. 1 lines
                                    15-23 L375-L392; real/imaginary split of Eq. 40)                          */
@@ -96,12 +101,25 @@ typedef struct {
    *    128-row tiles of every N x N product of a2-a4; the caller all-gathers the blocks at three points of a
    *    Hamiltonian update (rt_slab_get_shard, RT_SLAB_PROP_A..D).  0 or 1 = replicated propagator.  Taylor mode only. */
   int32_t  prop_shards, prop_shard;
+  /* -- closer-to-paper physics; all zero = the north_star step ------------------------------- */
+  int32_t  magnus_order;    /* 0 or 1: Omega = Omega_1 (Eq. 12, "mid-point"); 2: + Omega_2 = dt^2/12 [H0, H1] (Eq. 13,
+                               L125), fourth order in dt.  Needs RT_PROP_COMMUTATOR (the series takes any Omega)     */
+  int32_t  xc_functional;   /* RT_XC_LDA_PZ81 (0, north_star) or RT_XC_PBE (the functional the paper ran, L453)       */
+  int32_t  poisson_order;   /* 0 or 2: 7-point Laplacian in the Hartree solve; 4: fourth-order 13-point stencil
+                               (Eq. 2 with n = 2, L58-L60) as the operator whose solution V_H converges to            */
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
  * H0 = H-1 = diag(eps) + Proj(E0.r).   phi: [norb][Ng] HOST (copied) or DEVICE (borrowed, RT_PHI_DEVICE);
  * eps, occ: [norb] HOST, copied; occ in [0,2].  *out receives the handle (owned by the caller -> rt_destroy). */
 int rt_create(const rt_config* cfg, const double* phi, const double* eps, const double* occ, rt_handle* out);
+
+/* The same with the ground state given as MATRICES in the basis Phi (all HOST, row-major [norb][norb], copied):
+ * Hks = <phi_i|H_KS|phi_j>, P0re/P0im = the density matrix at t = 0 (P0im may be NULL = 0; tr(P0 S) = N_e), eps[norb] =
+ * the Kohn-Sham eigenvalues (only their range is used: spectral shift and the bound that sizes the series).  With
+ * RT_NONORTHOGONAL the library forms S = dVol Phi Phi^T and S^-1 itself.  H0 = H-1 = Hks + Proj(E0.r). */
+int rt_create_general(const rt_config* cfg, const double* phi, const double* eps, const double* Hks, const double* P0re,
+                      const double* P0im, rt_handle* out);
 
 /* Field E(t_{n+1}) used by the following step(s): HOST double[3]; sticky; default (0,0,0).  The three values are read
  * before the call returns (they travel to the device as kernel arguments), so the buffer may be reused at once.
@@ -148,6 +166,9 @@ int rt_get_hmatrix(rt_handle h, double* H0);
 int rt_get_energy(rt_handle h, double* energy);
 /* Warm-start Hartree potential V_H[Ng] (EITHER).  Synchronises. */
 int rt_get_vhartree(rt_handle h, double* vh);
+/* Overlap matrix S = dVol Phi Phi^T and its inverse as the library computed them (RT_NONORTHOGONAL handles; each
+ * [norb][norb], EITHER, either may be NULL).  Synchronises. */
+int rt_get_overlap(rt_handle h, double* S, double* Sinv);
 /* Current time t (HOST). */
 int rt_get_time(rt_handle h, double* t);
 /* Integrals of the current density, HOST double[2]: { dVol sum rho , dVol sum (rho - rho0) }.  Synchronises. */

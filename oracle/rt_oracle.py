@@ -261,6 +261,57 @@ def propagate_commutator(Hbar: np.ndarray, P0: np.ndarray, dt: float, dP_thrs: f
 
 
 # --------------------------------------------------------------------------------------------------
+# Closer-to-paper propagation: second Magnus term (Eq. 13) and a non-orthogonal basis (Eq. 33-38)
+# --------------------------------------------------------------------------------------------------
+
+def magnus_omega(H0: np.ndarray, H1: np.ndarray, dt: float, order: int = 1, Sinv=None) -> np.ndarray:
+    """Omega of U = exp(Omega) for a Hamiltonian that changes linearly from H0 (at t) to H1 (at t + dt), hbar = 1:
+    Omega_1 = -i dt (H0 + H1)/2 (Eq. 12); order 2 adds Omega_2 = (dt^2/12)[H0, H1] (Eq. 13).
+    With an overlap matrix S != 1 every H is replaced by S^-1 H (Eq. 36: Omega_1 = -i dt S^-1 Hbar)."""
+    if Sinv is not None:
+        H0, H1 = Sinv @ H0, Sinv @ H1
+    Om = (-1j * dt) * 0.5 * (H0 + H1)
+    if order >= 2:
+        Om = Om + (dt * dt / 12.0) * (H0 @ H1 - H1 @ H0)
+    return Om
+
+
+def propagate_omega_series(Om: np.ndarray, P0: np.ndarray, dP_thrs: float = 1e-14, kmax: int = 200):
+    """The paper's series for a general Omega, Eq. 21-23 (L191-L209) / Eq. 37-38 (L289-L304):
+    dP^(k) = (1/k){Omega, dP^(k-1)} = (1/k)(Omega dP^(k-1) + dP^(k-1) Omega^dagger), P1 = P0 + sum_k dP^(k),
+    until max|dP^(k)| <= dP_thrs.  Returns (P1, k).  Reduces to propagate_commutator for Omega = -i dt Hbar."""
+    P1 = P0.astype(np.complex128).copy()
+    dP = P0.astype(np.complex128).copy()
+    k = 0
+    err = 2.0 * dP_thrs
+    while err > dP_thrs and k < kmax:
+        k += 1
+        dP = (Om @ dP + dP @ Om.conj().T) / k
+        P1 = P1 + dP
+        err = np.max(np.abs(dP))
+    return P1, k
+
+
+def propagate_exact_general(H0: np.ndarray, H1: np.ndarray, P0: np.ndarray, dt: float, order: int = 1, S=None):
+    """P1 = exp(Omega) P0 exp(Omega)^dagger with the exponential by exact diagonalisation (L129, L147).  For S != 1 the
+    problem is first taken to an orthogonal basis with the Cholesky factor S = L L^T (L271 / Appendix A):
+    H_o = L^-1 H L^-T, P_o = L^T P L; after the propagation P = L^-T P_o L^-1.  Omega_o = magnus_omega(H0_o, H1_o) is
+    anti-Hermitian, so i Omega_o is Hermitian and eigh applies."""
+    if S is not None:
+        L = np.linalg.cholesky(S)
+        Li = np.linalg.inv(L)
+        H0, H1 = Li @ H0 @ Li.T, Li @ H1 @ Li.T
+        P0 = L.T @ P0 @ L
+    Om = magnus_omega(H0, H1, dt, order)
+    w, W = np.linalg.eigh(1j * Om)                       # Omega = -i (i Omega), i Omega Hermitian
+    U = (W * np.exp(-1j * w)[None, :]) @ W.conj().T
+    P1 = U @ P0 @ U.conj().T
+    if S is not None:
+        P1 = Li.T @ P1 @ Li
+    return P1
+
+
+# --------------------------------------------------------------------------------------------------
 # The time stepper
 # --------------------------------------------------------------------------------------------------
 
@@ -274,12 +325,17 @@ class RTOracle:
 
     def __init__(self, shape, h, Phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2,
                  nu_pre=2, nu_post=2, omega=6.0 / 7.0, hartree=True, xc=True,
-                 propagator="eigh", dP_thrs=1e-10, max_order=200, H_thrs=0.0, max_hupdates=20):
+                 propagator="eigh", dP_thrs=1e-10, max_order=200, H_thrs=0.0, max_hupdates=20,
+                 magnus=1, Hks=None, P0=None, nonorthogonal=False):
         """propagator = "eigh": exact spectral exponential (north_star).  propagator = "commutator": the
         paper's own series applied to P (Eq. 39, Alg. 1 lines 15-23) until max|dP^(k)| <= dP_thrs
         (Alg. 1 line 5: 1e-10).  H_thrs > 0 turns the fixed count of Hamiltonian updates into the paper's
         dynamic loop (Alg. 1 lines 12-13, 24-26; L483): repeat while max|H1 - H1_old| > H_thrs, at most
-        max_hupdates times.  ``last_hupdates``, ``last_H_err``, ``last_orders`` report what the last step did."""
+        max_hupdates times.  ``last_hupdates``, ``last_H_err``, ``last_orders`` report what the last step did.
+        magnus = 2 adds the second Magnus term Omega_2 = dt^2/12 [H0, H1] (Eq. 13).  nonorthogonal = True: Phi is
+        any basis of real functions, S = dVol Phi Phi^T != 1 and P is propagated with Eq. 33-38 (L262-L304); the
+        ground state then enters as a Hamiltonian matrix ``Hks`` [N][N] (instead of eps) and a density matrix ``P0``
+        [N][N] with tr(P0 S) = N_e (instead of occ).  Both options route the propagation through magnus_omega."""
         assert propagator in ("eigh", "commutator")
         self.propagator, self.dP_thrs, self.max_order = propagator, float(dP_thrs), int(max_order)
         self.H_thrs, self.max_hupdates = float(H_thrs), int(max_hupdates)
@@ -297,13 +353,17 @@ class RTOracle:
         self.nu1, self.nu2, self.omega = int(nu_pre), int(nu_post), float(omega)
         self.hartree, self.xc = bool(hartree), bool(xc)
         self.t = 0.0
-        self.P0 = np.diag(self.occ).astype(np.complex128)
-        self.rho0 = density(self.Phi, np.diag(self.occ))
+        self.magnus, self.nonorth = int(magnus), bool(nonorthogonal)
+        self.Hks = np.diag(self.eps) if Hks is None else np.asarray(Hks, dtype=np.float64).copy()
+        self.P0 = (np.diag(self.occ) if P0 is None else np.asarray(P0)).astype(np.complex128)
+        self.S = project(self.Phi, np.ones(self.Ng), self.dVol) if self.nonorth else None      # overlap, Eq. 30
+        self.Sinv = np.linalg.inv(self.S) if self.nonorth else None
+        self.rho0 = density(self.Phi, self.P0.real)
         self.rho = self.rho0.copy()
         self.vxc0 = vxc_lda(self.rho0) if self.xc else np.zeros(self.Ng)
         self.VH = np.zeros(self.Ng)
         self.E_next = np.zeros(3)
-        self.H0 = np.diag(self.eps) + project(self.Phi, field_potential(self.shape, self.h, np.asarray(E0, float)), self.dVol)
+        self.H0 = self.Hks + project(self.Phi, field_potential(self.shape, self.h, np.asarray(E0, float)), self.dVol)
         self.Hm1 = self.H0.copy()
 
     def set_field(self, E):
@@ -320,7 +380,14 @@ class RTOracle:
             dv = dv + vxc_lda(rho) - self.vxc0
         return dv
 
-    def _propagate(self, Hbar):
+    def _propagate(self, Hbar, H1=None):
+        if self.magnus >= 2 or self.nonorth:              # general Omega (Eq. 13 / Eq. 36)
+            if self.propagator == "eigh":
+                return propagate_exact_general(self.H0, H1, self.P0, self.dt, self.magnus, self.S)
+            Om = magnus_omega(self.H0, H1, self.dt, self.magnus, self.Sinv)
+            P1, k = propagate_omega_series(Om, self.P0, self.dP_thrs, self.max_order)      # Eq. 37-38
+            self.last_orders.append(k)
+            return P1
         if self.propagator == "eigh":
             return propagate_eigh(Hbar, self.P0, self.dt)                  # Eq. 15
         P1, k = propagate_commutator(Hbar, self.P0, self.dt, self.dP_thrs, self.max_order)   # lines 15-23
@@ -335,10 +402,10 @@ class RTOracle:
             H_err = 2.0 * self.H_thrs                                      # line 12
             while (it < self.m) if self.H_thrs <= 0.0 else (H_err > self.H_thrs and it < self.max_hupdates):
                 Hbar = 0.5 * (self.H0 + H1)                                # line 14 / Eq. 12
-                P1 = self._propagate(Hbar)
+                P1 = self._propagate(Hbar, H1)
                 rho = density(self.Phi, P1.real)                           # Eq. 27
                 H1_old = H1
-                H1 = np.diag(self.eps) + project(self.Phi, self.delta_v(rho), self.dVol)   # line 25
+                H1 = self.Hks + project(self.Phi, self.delta_v(rho), self.dVol)            # line 25
                 H_err = float(np.max(np.abs(H1 - H1_old)))                 # line 24 (after the update, DESIGN R2)
                 self.last_H_errs.append(H_err)
                 it += 1
@@ -358,7 +425,7 @@ class RTOracle:
         (+ dVol sum E.x drho while a field is on).  Its functional derivative w.r.t. rho is delta_v, so it
         is conserved by the exact dynamics when E = 0 (test aid; uses the current, unconverged V_H)."""
         drho = self.rho - self.rho0
-        e = float(np.sum(self.eps * np.real(np.diag(self.P0))))
+        e = float(np.sum(self.Hks * self.P0.real))        # tr(H_KS P); = sum_i eps_i Re P_ii in the KS basis
         if self.hartree:
             e += 0.5 * self.dVol * float(np.sum(drho * self.VH))
         if self.xc:

@@ -16,14 +16,15 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librt_tddft.so")
 
 RT_OK, RT_EINVAL, RT_ENOMEM, RT_ECUDA, RT_ESTATE, RT_ENUMERIC = 0, -1, -2, -3, -4, -5
-RT_PHI_DEVICE, RT_NO_HARTREE, RT_NO_XC, RT_NO_GRAPH, RT_NO_TMA = 1, 2, 4, 8, 16
+RT_PHI_DEVICE, RT_NO_HARTREE, RT_NO_XC, RT_NO_GRAPH, RT_NO_TMA, RT_NONORTHOGONAL = 1, 2, 4, 8, 16, 32
+RT_XC_LDA_PZ81, RT_XC_PBE = 0, 1
 RT_PROP_TAYLOR, RT_PROP_COMMUTATOR = 0, 1
 RT_STAGE_NAMES = ("Hupdate", "Rho", "Vh", "ELDYN", "XC")      # Table 1 of the paper, L543-L547
 RT_STAGE_COUNT = 5
 
 # every symbol include/rt_tddft.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
-    "rt_create", "rt_set_field", "rt_step", "rt_get_dipole", "rt_get_density", "rt_get_pmatrix", "rt_get_hmatrix",
+    "rt_create", "rt_create_general", "rt_get_overlap", "rt_set_field", "rt_step", "rt_get_dipole", "rt_get_density", "rt_get_pmatrix", "rt_get_hmatrix",
     "rt_get_vhartree", "rt_get_time", "rt_get_charge", "rt_get_info", "rt_get_launch_count", "rt_last_error",
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
@@ -54,6 +55,7 @@ class rt_config(C.Structure):
         ("slab_x0", C.c_int32), ("slab_nx", C.c_int32),
         ("history", C.c_int32),
         ("prop_shards", C.c_int32), ("prop_shard", C.c_int32),
+        ("magnus_order", C.c_int32), ("xc_functional", C.c_int32), ("poisson_order", C.c_int32),
     ]
 
 
@@ -83,6 +85,7 @@ def _load():
     vp, dp, i32, i64p = C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int64)
     sig = {
         "rt_create": [C.POINTER(rt_config), dp, dp, dp, C.POINTER(vp)],
+        "rt_create_general": [C.POINTER(rt_config), dp, dp, dp, dp, dp, C.POINTER(vp)], "rt_get_overlap": [vp, dp, dp],
         "rt_set_field": [vp, dp], "rt_step": [vp, i32], "rt_get_dipole": [vp, dp], "rt_get_density": [vp, dp],
         "rt_get_pmatrix": [vp, dp, dp], "rt_get_hmatrix": [vp, dp], "rt_get_vhartree": [vp, dp],
         "rt_get_time": [vp, dp], "rt_get_charge": [vp, dp], "rt_get_info": [vp, dp], "rt_get_launch_count": [vp, i64p],
@@ -141,6 +144,22 @@ def rt_create(cfg: rt_config, phi, eps, occ) -> int:
     rc = _lib.rt_create(C.byref(cfg), _ptr(phi), _ptr(eps), _ptr(occ), C.byref(h))
     _check(None, rc)
     return h.value
+
+
+def rt_create_general(cfg: rt_config, phi, eps, Hks, P0re, P0im=None) -> int:
+    h = C.c_void_p()
+    eps = np.ascontiguousarray(eps, dtype=np.float64)
+    Hks = np.ascontiguousarray(Hks, dtype=np.float64)
+    P0re = np.ascontiguousarray(P0re, dtype=np.float64)
+    P0im = None if P0im is None else np.ascontiguousarray(P0im, dtype=np.float64)
+    rc = _lib.rt_create_general(C.byref(cfg), _ptr(phi), _ptr(eps), _ptr(Hks), _ptr(P0re), _ptr(P0im), C.byref(h))
+    _check(None, rc)
+    return h.value
+
+
+def rt_get_overlap(h, S, Sinv):
+    _check(h, _lib.rt_get_overlap(h, _ptr(S), _ptr(Sinv)))
+    return S, Sinv
 
 
 def rt_set_field(h, E):
@@ -357,13 +376,19 @@ class RTTDDFT:
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
                  nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
                  device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0,
-                 slab=None, history=0, prop_shard=None):
+                 slab=None, history=0, prop_shard=None, magnus=1, xc_functional="lda", poisson_order=2, Hks=None,
+                 P0=None, nonorthogonal=False):
         """``slab = (x0, nx_local)``: the handle owns those x-planes and ``phi`` is [norb][nx_local*ny*nz]
-        (rt_slab_* entry points; see slab.py).  ``prop_shard = (rank, nranks)``: row-sharded N x N propagator."""
+        (rt_slab_* entry points; see slab.py).  ``prop_shard = (rank, nranks)``: row-sharded N x N propagator.
+        ``Hks`` / ``P0`` ([norb][norb] host arrays; P0 may be complex): the ground state as matrices (rt_create_general);
+        ``nonorthogonal``: phi is a non-orthonormal basis.  ``magnus`` = 2: second Magnus term.  ``occ`` may then be None."""
         cfg = rt_config()
         cfg.slab_x0, cfg.slab_nx = (int(slab[0]), int(slab[1])) if slab else (0, 0)
         cfg.history = int(history)
         cfg.prop_shards, cfg.prop_shard = (int(prop_shard[1]), int(prop_shard[0])) if prop_shard else (0, 0)
+        cfg.magnus_order = int(magnus)
+        cfg.xc_functional = {"lda": RT_XC_LDA_PZ81, "pbe": RT_XC_PBE}[xc_functional]
+        cfg.poisson_order = int(poisson_order)
         cfg.propagator = {"taylor": RT_PROP_TAYLOR, "commutator": RT_PROP_COMMUTATOR}[propagator]
         cfg.max_order, cfg.dP_thrs, cfg.H_thrs, cfg.max_hupdates = int(max_order), float(dP_thrs), float(H_thrs), int(max_hupdates)
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)
@@ -389,6 +414,8 @@ class RTTDDFT:
             flags |= RT_NO_GRAPH
         if not tma:
             flags |= RT_NO_TMA
+        if nonorthogonal:
+            flags |= RT_NONORTHOGONAL
         cfg.flags, cfg.device = flags, int(device)
         if stream is None:
             try:
@@ -400,7 +427,11 @@ class RTTDDFT:
         self._dt = float(dt)
         self.shape, self.norb = tuple(int(s) for s in shape), int(len(eps))
         self.ngrid = self.shape[0] * self.shape[1] * self.shape[2]
-        self.handle = rt_create(cfg, phi, eps, occ)
+        if Hks is not None or P0 is not None:
+            P0 = np.asarray(P0)
+            self.handle = rt_create_general(cfg, phi, eps, Hks, P0.real, P0.imag if np.iscomplexobj(P0) else None)
+        else:
+            self.handle = rt_create(cfg, phi, eps, occ)
 
     def set_field(self, E):
         rt_set_field(self.handle, E)
@@ -438,6 +469,10 @@ class RTTDDFT:
 
     def hmatrix(self):
         return rt_get_hmatrix(self.handle, np.empty((self.norb, self.norb)))
+
+    def overlap(self):
+        S, Si = np.empty((self.norb, self.norb)), np.empty((self.norb, self.norb))
+        return rt_get_overlap(self.handle, S, Si)
 
     def vhartree(self):
         return rt_get_vhartree(self.handle, np.empty(self.ngrid))

@@ -100,7 +100,8 @@ project_kernel(const double* __restrict__ phi, const double* __restrict__ w, con
 }
 
 __global__ void project_reduce_kernel(const double* __restrict__ W, const double* __restrict__ eps, double scale,
-                                      double* __restrict__ H, int N, int ldn, int S, int Sn, int Sd, int narrow_tile) {
+                                      double* __restrict__ H, int N, int ldn, int S, int Sn, int Sd, int narrow_tile,
+                                      const double* __restrict__ Hadd) {
   // one thread per (i, j) with j >= i; fixed summation order over the splits
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int i = blockIdx.y;
@@ -113,6 +114,7 @@ __global__ void project_reduce_kernel(const double* __restrict__ W, const double
   for (int s = 0; s < ns; ++s) sum += p[(long long)s * slab];
   double v = scale * sum;
   if (i == j && eps) v += eps[i];
+  if (Hadd) v += Hadd[(long long)i * ldn + j];
   H[(long long)i * ldn + j] = v;
   H[(long long)j * ldn + i] = v;
 }
@@ -130,9 +132,10 @@ void launch_project(const ProjectPlan& p, const double* phi, const double* w, co
 }
 
 void launch_project_reduce(const ProjectPlan& p, const double* W, const double* eps, double scale, double* H,
-                           cudaStream_t st) {
+                           cudaStream_t st, const double* Hadd) {
   dim3 grid((p.N + 127) / 128, p.N);
-  project_reduce_kernel<<<grid, 128, 0, st>>>(W, eps, scale, H, p.N, p.ldn, p.S, p.Sn, p.Sd, p.Tn > 0 ? p.ntile - 1 : -1);
+  project_reduce_kernel<<<grid, 128, 0, st>>>(W, eps, scale, H, p.N, p.ldn, p.S, p.Sn, p.Sd, p.Tn > 0 ? p.ntile - 1 : -1,
+                                              Hadd);
 }
 
 // ======================================================================================================

@@ -289,8 +289,10 @@ void launch_poisson_rhs(long long Ng, const double* rho, const double* rho0, con
 }
 
 // ---------------------------------------------------------------------------------------------- a2 and glue
+// S == nullptr: orthonormal basis, X = dt (Hbar - sigma I); else X = dt (Hbar - sigma S)  (then S^-1 X = dt (S^-1 Hbar - sigma I))
 __global__ void hbar_kernel(int N, int ldn, const double* __restrict__ Hm1, const double* __restrict__ H0,
-                            double* __restrict__ H1, double* __restrict__ X, double dt, double sigma, int first) {
+                            double* __restrict__ H1, double* __restrict__ X, double dt, double sigma, int first,
+                            const double* __restrict__ S) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
   if (j >= N) return;
   const long long o = (long long)i * ldn + j;
@@ -298,12 +300,79 @@ __global__ void hbar_kernel(int N, int ldn, const double* __restrict__ Hm1, cons
   double h1;
   if (first) { h1 = 2.0 * h0 - Hm1[o]; H1[o] = h1; } else { h1 = H1[o]; }
   double x = 0.5 * (h0 + h1);
-  if (i == j) x -= sigma;
+  if (S) x -= sigma * S[o];
+  else if (i == j) x -= sigma;
   X[o] = dt * x;
 }
 void launch_hbar(int N, int ldn, const double* Hm1, const double* H0, double* H1, double* X, double dt, double sigma,
-                 int first, cudaStream_t st) {
-  hbar_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, Hm1, H0, H1, X, dt, sigma, first);
+                 int first, cudaStream_t st, const double* S) {
+  hbar_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, Hm1, H0, H1, X, dt, sigma, first, S);
+}
+
+// ---- the paper's "one multiply + transpose" form of a commutator step (DGEAM) -------------
+// R, I: real and imaginary part of M = Omega dP (full N x N products).  dP' = (M + M^dagger)/k:
+//   Sn = (R + R^T)/k (symmetric), An = (I - I^T)/k (antisymmetric);  P1r += Sn, P1i += An.
+// 32 x 32 tiles through shared memory so that both the (i, j) and the (j, i) accesses are coalesced; only tiles
+// bj >= bi are visited and both images are written, so the outputs are exactly (anti)symmetric.
+__global__ void __launch_bounds__(256)
+transpose_add_kernel(int N, int ldn, const double* __restrict__ R, const double* __restrict__ I, double inv_k,
+                     double* __restrict__ Sn, double* __restrict__ An, double* __restrict__ P1r,
+                     double* __restrict__ P1i, const int* __restrict__ skip) {
+  if (skip && *skip) return;
+  const int bi = blockIdx.y, bj = blockIdx.x;
+  if (bj < bi) return;
+  __shared__ double tR[32][33], tI[32][33];
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;      // 32 x 8
+  for (int r = ty; r < 32; r += 8) {                            // tile (bj, bi), read row-wise
+    const int row = bj * 32 + r, col = bi * 32 + tx;
+    const bool ok = row < N && col < N;
+    tR[r][tx] = ok ? R[(long long)row * ldn + col] : 0.0;
+    tI[r][tx] = ok ? I[(long long)row * ldn + col] : 0.0;
+  }
+  __syncthreads();
+  double sv[4], av[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {                                 // tile (bi, bj): element (row, col) needs (col, row)
+    const int r = ty + 8 * q;
+    const int row = bi * 32 + r, col = bj * 32 + tx;
+    sv[q] = av[q] = 0.0;
+    if (row < N && col < N) {
+      const long long o = (long long)row * ldn + col;
+      sv[q] = (R[o] + tR[tx][r]) * inv_k;
+      av[q] = (row == col) ? 0.0 : (I[o] - tI[tx][r]) * inv_k;
+      if (bj > bi || col >= row) { Sn[o] = sv[q]; An[o] = av[q]; P1r[o] += sv[q]; P1i[o] += av[q]; }
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int q = 0; q < 4; ++q) { tR[ty + 8 * q][tx] = sv[q]; tI[ty + 8 * q][tx] = av[q]; }
+  __syncthreads();
+  for (int r = ty; r < 32; r += 8) {                            // mirror image into tile (bj, bi), written row-wise
+    const int row = bj * 32 + r, col = bi * 32 + tx;            // = transpose of element (col, row) of tile (bi, bj)
+    if (row < N && col < N && (bj > bi || col < row)) {
+      const long long o = (long long)row * ldn + col;
+      const double s = tR[tx][r], a = -tI[tx][r];
+      Sn[o] = s; An[o] = a; P1r[o] += s; P1i[o] += a;
+    }
+  }
+}
+void launch_transpose_add(int N, int ldn, const double* R, const double* I, double inv_k, double* Sn, double* An,
+                          double* P1r, double* P1i, const int* skip, cudaStream_t st) {
+  const int nb = (N + 31) / 32;
+  transpose_add_kernel<<<dim3(nb, nb), 256, 0, st>>>(N, ldn, R, I, inv_k, Sn, An, P1r, P1i, skip);
+}
+
+// out = a X + b Y (whole N x ldn buffers; padding stays zero)
+__global__ void axpby_kernel(long long n, double a, const double* __restrict__ X, double b, const double* __restrict__ Y,
+                             double* __restrict__ out) {
+  for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += (long long)gridDim.x * blockDim.x)
+    out[r] = a * X[r] + b * Y[r];
+}
+void launch_axpby(int N, int ldn, double a, const double* X, double b, const double* Y, double* out, cudaStream_t st) {
+  const long long n = (long long)N * ldn;
+  long long nb = (n + 255) / 256;
+  if (nb > 148 * 16) nb = 148 * 16;
+  axpby_kernel<<<(unsigned)nb, 256, 0, st>>>(n, a, X, b, Y, out);
 }
 
 __global__ void series_init_kernel(int N, int ldn, const double* __restrict__ Y, double* __restrict__ C, double c1,
@@ -398,6 +467,36 @@ maxabs_diff_kernel(long long n, const double* __restrict__ a, const double* __re
 void launch_maxabs_diff(int N, int ldn, const double* A, const double* B, ConvState* cs, cudaStream_t st) {
   const long long n = (long long)N * ldn;
   maxabs_diff_kernel<<<norm_blocks(n), RB, 0, st>>>(n, A, B, cs);
+}
+
+// cs->H_bits = max |T - 1| (Newton-Schulz residual of the overlap inverse)
+__global__ void __launch_bounds__(RB)
+maxabs_minus_identity_kernel(int N, int ldn, const double* __restrict__ T, ConvState* __restrict__ cs) {
+  double m = 0.0;
+  const long long n = (long long)N * ldn;
+  for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < n; r += (long long)gridDim.x * RB) {
+    const int i = (int)(r / ldn), j = (int)(r - (long long)i * ldn);
+    if (j < N) m = max_nf(m, fabs(T[r] - (i == j ? 1.0 : 0.0)));
+  }
+  m = block_max(m);
+  if (threadIdx.x == 0) atomicMax(&cs->H_bits, (unsigned long long)__double_as_longlong(m));
+}
+void launch_maxabs_minus_identity(int N, int ldn, const double* T, ConvState* cs, cudaStream_t st) {
+  maxabs_minus_identity_kernel<<<norm_blocks((long long)N * ldn), RB, 0, st>>>(N, ldn, T, cs);
+}
+
+// out[5] = sum_ij A_ij B_ij  (tr(H_KS Re P) for symmetric matrices); one block, fixed order
+__global__ void trace_product_kernel(int N, int ldn, const double* __restrict__ A, const double* __restrict__ B,
+                                     double* __restrict__ out) {
+  __shared__ double sh[32][5];
+  double v[5] = {0, 0, 0, 0, 0};
+  const long long n = (long long)N * ldn;
+  for (long long r = threadIdx.x; r < n; r += blockDim.x) v[0] += A[r] * B[r];
+  block_sum<5>(v, sh);
+  if (threadIdx.x == 0) out[5] = v[0];
+}
+void launch_trace_product(int N, int ldn, const double* A, const double* B, double* out, cudaStream_t st) {
+  trace_product_kernel<<<1, 1024, 0, st>>>(N, ldn, A, B, out);
 }
 
 __global__ void set_diag_kernel(int N, int ldn, double* __restrict__ M, const double* __restrict__ d) {

@@ -68,6 +68,13 @@ struct rt_ctx {
   // row-sharded propagator: rank `shard` of `nshard` owns the rows [row_beg, row_end) of every N x N product
   int nshard = 1, shard = 0, shard_rows = 0, row_beg = 0, row_end = 0;
   size_t nn_alloc = 0;            // doubles per N x N buffer (rows padded to nshard * shard_rows for the all-gathers)
+  // closer-to-paper propagation: general Omega = -i dt S^-1 Hbar (+ dt^2/12 [S^-1 H0, S^-1 H1])
+  int magnus = 1;                 // 2: second Magnus term (Eq. 13)
+  bool nonorth = false;           // RT_NONORTHOGONAL: S = dVol Phi Phi^T != 1 (Eq. 33-38)
+  bool general = false;           // magnus == 2 || nonorth: the series runs in the "one multiply + transpose" form
+  double *Hks = nullptr;          // ground-state Hamiltonian matrix when it is not diag(eps)   (rt_create_general)
+  double *Smat = nullptr, *Sinv = nullptr, *Bm = nullptr, *Wm = nullptr, *Rt = nullptr, *It = nullptr;
+  int newton_iters = 0;           // Newton-Schulz iterations that S^-1 took at create
   int slab_more = 0;              // decision of the last RT_SLAB_CHECK: another Hamiltonian update is needed
   std::map<int, cudaGraphExec_t> phase_exec;      // slab phases captured as CUDA graphs, key = 2 * phase + (it == 0)
   std::map<int, int64_t> phase_launches;
@@ -402,8 +409,66 @@ void enqueue_commutator(rt_ctx* c, const double* Ar, const double* Ai, double* O
   }
 }
 
+// The same series for a GENERAL Omega = -i B + W (Eq. 21-23; Eq. 37-38):
+//   B = dt (S^-1 Hbar - sigma 1)      real, symmetric only when S = 1        (Eq. 36; the shift commutes)
+//   W = dt^2/12 [S^-1 H0, S^-1 H1]    real, second Magnus term (Eq. 13); absent for magnus = 1
+//   dP^(k) = (1/k)(Omega dP + dP Omega^dagger) = (1/k)(M + M^dagger),  M = Omega dP^(k-1),  dP = S' + i A':
+//   Re M = B A' + W S',  Im M = -B S' + W A'  ->  S'' = (Re M + Re M^T)/k,  A'' = (Im M - Im M^T)/k.
+// This is the paper's "one matrix-matrix multiplication and a matrix transpose (DGEAM)" form (L434-L438): two full
+// (dual-term) GEMMs and one transpose-add kernel per order.  gemm_abt contracts against the second operand transposed:
+// B A' = -gemm(B, A'), W S' = gemm(W, S'), B S' = gemm(B, S'), W A' = -gemm(W, A').
+void enqueue_general_omega(rt_ctx* c) {
+  const double* X = c->X;                               // dt (Hbar - sigma S) from launch_hbar
+  if (c->nonorth) {
+    enqueue_gemm(c, 0, c->Sinv, X, 1.0, nullptr, nullptr, 0, c->Bm);                    // B = S^-1 X  (X symmetric)
+  }
+  if (c->magnus >= 2) {
+    const double w12 = c->dt * c->dt / 12.0;
+    if (!c->nonorth) {
+      enqueue_gemm(c, -1, c->H0, c->H1, w12, c->H1, c->H0, -w12, c->Wm);                // dt^2/12 (H0 H1 - H1 H0)
+    } else {
+      // G_a = S^-1 H_a and G_a^T = H_a S^-1 in the (still free) series buffers, then W = dt^2/12 (G0 G1 - G1 G0)
+      enqueue_gemm(c, 0, c->Sinv, c->H0, 1.0, nullptr, nullptr, 0, c->Yb);              // G0
+      enqueue_gemm(c, 0, c->Sinv, c->H1, 1.0, nullptr, nullptr, 0, c->Yc);              // G1
+      enqueue_gemm(c, 0, c->H0, c->Sinv, 1.0, nullptr, nullptr, 0, c->Cm);              // G0^T
+      enqueue_gemm(c, 0, c->H1, c->Sinv, 1.0, nullptr, nullptr, 0, c->Sm);              // G1^T
+      enqueue_gemm(c, 0, c->Yb, c->Sm, w12, c->Yc, c->Cm, -w12, c->Wm);
+    }
+  }
+}
+
+void enqueue_commutator_general(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
+  const size_t nn = (size_t)c->N * c->ldn * 8;
+  enqueue_general_omega(c);
+  cudaMemcpyAsync(Or, Ar, nn, cudaMemcpyDeviceToDevice, c->st);               // P1 <- P0
+  cudaMemcpyAsync(Oi, Ai, nn, cudaMemcpyDeviceToDevice, c->st);
+  const double* B = c->nonorth ? c->Bm : c->X;
+  const double* W = c->magnus >= 2 ? c->Wm : nullptr;
+  const double* pr = Ar;
+  const double* pi = Ai;
+  double* bufs[2][2] = {{c->Yb, c->Yc}, {c->Cm, c->Sm}};
+  const int* skip = &c->d_cs->done;
+  for (int k = 1; k <= c->kmax; ++k) {
+    double* nr = bufs[k & 1][0];
+    double* ni = bufs[k & 1][1];
+    if (W) {
+      enqueue_gemm(c, 0, B, pi, -1.0, W, pr, 1.0, c->Rt, nullptr, 0, nullptr, 0, skip);      // Re M
+      enqueue_gemm(c, 0, B, pr, -1.0, W, pi, -1.0, c->It, nullptr, 0, nullptr, 0, skip);     // Im M
+    } else {
+      enqueue_gemm(c, 0, B, pi, -1.0, nullptr, nullptr, 0, c->Rt, nullptr, 0, nullptr, 0, skip);
+      enqueue_gemm(c, 0, B, pr, -1.0, nullptr, nullptr, 0, c->It, nullptr, 0, nullptr, 0, skip);
+    }
+    launch_transpose_add(c->N, c->ldn, c->Rt, c->It, 1.0 / (double)k, nr, ni, Or, Oi, skip, c->st);
+    launch_commutator_check(c->N, c->ldn, nr, ni, k, c->dP_thrs, c->d_cs, c->st);             // line 22
+    c->launches += 2;
+    pr = nr;
+    pi = ni;
+  }
+}
+
 void enqueue_propagate(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
-  if (c->prop == RT_PROP_COMMUTATOR) enqueue_commutator(c, Ar, Ai, Or, Oi);
+  if (c->general) enqueue_commutator_general(c, Ar, Ai, Or, Oi);
+  else if (c->prop == RT_PROP_COMMUTATOR) enqueue_commutator(c, Ar, Ai, Or, Oi);
   else { enqueue_expm(c); enqueue_upu(c, Ar, Ai, Or, Oi); }
 }
 
@@ -424,10 +489,12 @@ void enqueue_poisson(rt_ctx* c, const std::vector<MgLevel>& lv, int n_vc, const 
   c->launches += launch_mg_solve(s, c->st);
 }
 
+// eps != nullptr: the ground-state Hamiltonian is added -- diag(eps), or the matrix Hks of rt_create_general
 void enqueue_project(rt_ctx* c, const double* w, const double* eps, double* H) {
   if (c->use_tma) launch_project_tma(c->pp, c->tmPhiK, w, c->d_tiles, c->W, c->st);
   else launch_project(c->pp, c->phi, w, c->d_tiles, c->W, c->st);
-  launch_project_reduce(c->pp, c->W, eps, c->dvol, H, c->st);
+  const bool mat = eps && c->Hks;
+  launch_project_reduce(c->pp, c->W, mat ? nullptr : eps, c->dvol, H, c->st, mat ? c->Hks : nullptr);
   c->launches += 2;
 }
 
@@ -452,7 +519,7 @@ void enqueue_density_stage(rt_ctx* c) {
 void enqueue_update_propagate(rt_ctx* c, int it) {
   stage_begin(c, RT_STAGE_ELDYN);
   if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);                          // lines 12, 16
-  launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st);     // lines 11, 14
+  launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st, c->Smat);   // lines 11, 14
   c->launches += 1;
   enqueue_propagate(c, c->P0r, c->P0i, c->P1r, c->P1i);                                        // Eq. 15 / Eq. 39
   stage_end(c);
@@ -563,10 +630,26 @@ int rt_destroy(rt_handle c) {
   return RT_OK;
 }
 
-int rt_create(const rt_config* cfg, const double* phi, const double* eps, const double* occ, rt_handle* out) {
+}  // extern "C"
+
+namespace {
+// Common body of rt_create (Hks = P0re = P0im = nullptr: KS basis, H_KS = diag(eps), P0 = diag(occ)) and
+// rt_create_general (ground state given as matrices; occ may be nullptr).
+int create_impl(const rt_config* cfg, const double* phi, const double* eps, const double* occ, const double* Hks_in,
+                const double* P0re_in, const double* P0im_in, rt_handle* out) {
   rt_ctx* c = nullptr;
-  if (!cfg || !phi || !eps || !occ || !out) return fail(c, RT_EINVAL, "rt_create: NULL argument");
+  if (!cfg || !phi || !eps || !out || (!occ && !P0re_in)) return fail(c, RT_EINVAL, "rt_create: NULL argument");
   *out = nullptr;
+  const bool want_nonorth = (cfg->flags & RT_NONORTHOGONAL) != 0;
+  const bool want_general = want_nonorth || cfg->magnus_order >= 2;
+  if (cfg->magnus_order < 0 || cfg->magnus_order > 2) return fail(c, RT_EINVAL, "rt_create: magnus_order must be 0, 1 or 2");
+  if (want_general && cfg->propagator != RT_PROP_COMMUTATOR)
+    return fail(c, RT_EINVAL, "rt_create: the second Magnus term and a non-orthogonal basis are propagated with the paper's "
+                              "series (Eq. 37-38): set propagator = RT_PROP_COMMUTATOR");
+  if (want_general && cfg->slab_nx > 0)
+    return fail(c, RT_EINVAL, "rt_create: magnus_order = 2 / RT_NONORTHOGONAL are not available on slab handles");
+  if (want_nonorth && !(Hks_in && P0re_in))
+    return fail(c, RT_EINVAL, "rt_create: RT_NONORTHOGONAL needs the ground state as matrices (rt_create_general)");
   if (cfg->nx < 2 || cfg->ny < 2 || cfg->nz < 2) return fail(c, RT_EINVAL, "rt_create: grid dims must be >= 2");
   if (!(cfg->h > 0) || !(cfg->dt > 0)) return fail(c, RT_EINVAL, "rt_create: h and dt must be > 0");
   if (cfg->norb < 1) return fail(c, RT_EINVAL, "rt_create: norb must be >= 1");
@@ -586,7 +669,7 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   if (cfg->max_order < 0 || cfg->max_order > MAX_ORDER || cfg->max_hupdates < 0 || !(cfg->dP_thrs >= 0.0) ||
       !(cfg->H_thrs >= 0.0))
     return fail(c, RT_EINVAL, "rt_create: bad max_order / max_hupdates / dP_thrs / H_thrs");
-  for (int i = 0; i < cfg->norb; ++i)
+  for (int i = 0; occ && i < cfg->norb; ++i)
     if (!(occ[i] >= 0.0 && occ[i] <= 2.0)) return fail(c, RT_EINVAL, "rt_create: occ must lie in [0, 2]");
 
   int ndev = 0;
@@ -630,6 +713,9 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
   c->use_h = !(cfg->flags & RT_NO_HARTREE);
   c->use_xc = !(cfg->flags & RT_NO_XC);
   c->use_graph = !(cfg->flags & RT_NO_GRAPH);
+  c->magnus = cfg->magnus_order >= 2 ? 2 : 1;
+  c->nonorth = want_nonorth;
+  c->general = want_general;
   c->st = reinterpret_cast<cudaStream_t>(cfg->stream);
   const int N = c->N, ldn = c->ldn;
   const long long Ng = c->Ngl;      // grid points of this handle's Phi: what the plans and Phi descriptors see
@@ -827,6 +913,13 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
                      &c->P0r, &c->P0i, &c->P1r, &c->P1i};
   for (double** mp : mats) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
   ALLOC(c->W, (size_t)c->pp.S * N * ldn);
+  if (Hks_in) { ALLOC(c->Hks, nn); CKC(cudaMemsetAsync(c->Hks, 0, nn * 8, c->st)); }
+  if (c->general) {
+    double** extra[] = {&c->Rt, &c->It, c->magnus >= 2 ? &c->Wm : nullptr, c->nonorth ? &c->Smat : nullptr,
+                        c->nonorth ? &c->Sinv : nullptr, c->nonorth ? &c->Bm : nullptr};
+    for (double** mp : extra)
+      if (mp) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
+  }
   // rho and the five sums share one allocation: it is the first exchange buffer of the slab mode
   ALLOC(c->rho, NgF + 8); ALLOC(c->rho0, NgF); ALLOC(c->vxc0, NgF);
   c->d_sums = c->rho + NgF;
@@ -879,14 +972,61 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
     }
   }
   CKC(cudaMemcpy(c->d_eps, eps, (size_t)N * 8, cudaMemcpyHostToDevice));
-  CKC(cudaMemcpy(c->d_occ, occ, (size_t)N * 8, cudaMemcpyHostToDevice));
+  if (occ) CKC(cudaMemcpy(c->d_occ, occ, (size_t)N * 8, cudaMemcpyHostToDevice));
+  else CKC(cudaMemset(c->d_occ, 0, (size_t)N * 8));
   {
     double e8[8] = {cfg->E0[0], cfg->E0[1], cfg->E0[2], 0, 0, 0, 0, 0};
     CKC(cudaMemcpy(c->d_E, e8, sizeof e8, cudaMemcpyHostToDevice));
   }
 
+  // non-orthogonal basis: overlap S = dVol Phi Phi^T (Eq. 30) by the projection kernel with unit weights, then S^-1
+  // by the Newton-Schulz iteration X <- X (2 - S X) on the N x N GEMM kernels (every iterate is a polynomial in S:
+  // symmetric outputs), started from X0 = S / (|S|_1 |S|_inf), stopped when max|S X - 1| <= 1e-14
+  if (c->nonorth) {
+    launch_set_field(c->d_E, 0.0, 0.0, 0.0, c->st);
+    std::vector<double> ones((size_t)NgF + 16, 1.0);
+    CKC(cudaMemcpyAsync(c->w, ones.data(), ((size_t)NgF + 16) * 8, cudaMemcpyHostToDevice, c->st));
+    enqueue_project(c, c->w, nullptr, c->Smat);
+    std::vector<double> Sh((size_t)N * ldn);
+    CKC(cudaMemcpyAsync(Sh.data(), c->Smat, Sh.size() * 8, cudaMemcpyDeviceToHost, c->st));
+    CKC(cudaStreamSynchronize(c->st));
+    double n1 = 0.0;
+    for (int i = 0; i < N; ++i) {
+      double r = 0.0;
+      for (int j = 0; j < N; ++j) r += std::fabs(Sh[(size_t)i * ldn + j]);
+      n1 = std::fmax(n1, r);
+    }
+    if (!(n1 > 0.0) || !std::isfinite(n1)) FAIL_CREATE(RT_EINVAL, "rt_create: the overlap matrix dVol Phi Phi^T is zero or non-finite");
+    launch_axpby(N, ldn, 1.0 / (n1 * n1), c->Smat, 0.0, c->Smat, c->Sinv, c->st);       // X0 (S symmetric: |S|_1 = |S|_inf)
+    double res = 1.0;
+    int itn = 0;
+    for (; itn < 100 && res > 1e-14; ++itn) {
+      enqueue_gemm(c, 1, c->Smat, c->Sinv, 1.0, nullptr, nullptr, 0, c->Rt);            // T = S X
+      CKC(cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st));
+      launch_maxabs_minus_identity(N, ldn, c->Rt, c->d_cs, c->st);
+      enqueue_gemm(c, 1, c->Sinv, c->Rt, 1.0, nullptr, nullptr, 0, c->It);              // X T
+      launch_axpby(N, ldn, 2.0, c->Sinv, -1.0, c->It, c->Sinv, c->st);                  // X <- 2 X - X T
+      ConvState hs;
+      CKC(cudaMemcpyAsync(&hs, c->d_cs, sizeof hs, cudaMemcpyDeviceToHost, c->st));
+      CKC(cudaStreamSynchronize(c->st));
+      memcpy(&res, &hs.H_bits, 8);
+      if (!std::isfinite(res)) break;
+    }
+    c->newton_iters = itn;
+    if (!(res <= 1e-12)) FAIL_CREATE(RT_EINVAL, "rt_create: the overlap matrix could not be inverted (Phi linearly dependent?)");
+    CKC(cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st));
+    double e8[8] = {cfg->E0[0], cfg->E0[1], cfg->E0[2], 0, 0, 0, 0, 0};
+    CKC(cudaMemcpy(c->d_E, e8, sizeof e8, cudaMemcpyHostToDevice));
+  }
+
   // initial state (Alg. 1 lines 7-8): P0 = diag(occ); rho0; vxc0; H0 = H-1 = diag(eps) + Proj(E0.r)
-  launch_set_diag(N, ldn, c->P0r, c->d_occ, c->st);
+  if (P0re_in) {
+    if (int rc = copy_matrix_in(c, P0re_in, c->P0r)) { std::string m_ = c->err; FAIL_CREATE(rc, m_); }
+    if (P0im_in) { if (int rc = copy_matrix_in(c, P0im_in, c->P0i)) { std::string m_ = c->err; FAIL_CREATE(rc, m_); } }
+  } else {
+    launch_set_diag(N, ldn, c->P0r, c->d_occ, c->st);
+  }
+  if (Hks_in) { if (int rc = copy_matrix_in(c, Hks_in, c->Hks)) { std::string m_ = c->err; FAIL_CREATE(rc, m_); } }
   launch_field(NgF, c->gd, c->h, c->d_E, c->w, c->st);
   if (!c->slab) {
     enqueue_density(c, c->P0r, c->rho0, nullptr);
@@ -953,6 +1093,20 @@ int rt_create(const rt_config* cfg, const double* phi, const double* eps, const 
 #undef FAIL_CREATE
   *out = c;
   return RT_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int rt_create(const rt_config* cfg, const double* phi, const double* eps, const double* occ, rt_handle* out) {
+  if (!occ) return fail(nullptr, RT_EINVAL, "rt_create: NULL argument");
+  return create_impl(cfg, phi, eps, occ, nullptr, nullptr, nullptr, out);
+}
+
+int rt_create_general(const rt_config* cfg, const double* phi, const double* eps, const double* Hks, const double* P0re,
+                      const double* P0im, rt_handle* out) {
+  if (!Hks || !P0re) return fail(nullptr, RT_EINVAL, "rt_create_general: NULL argument");
+  return create_impl(cfg, phi, eps, nullptr, Hks, P0re, P0im, out);
 }
 
 int rt_set_field(rt_handle c, const double E[3]) {
@@ -1188,6 +1342,10 @@ int rt_get_energy(rt_handle c, double* energy) {
   launch_energy(c->Ng, c->gd, c->h, c->rho, c->rho0, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->N, c->ldn,
                 c->d_eps, c->P0r, c->d_bsums, c->d_energy, c->st);
   c->launches += 3;
+  if (c->Hks) {                                      // tr(H_KS Re P) replaces sum_i eps_i Re P_ii
+    launch_trace_product(c->N, c->ldn, c->Hks, c->P0r, c->d_energy, c->st);
+    c->launches += 1;
+  }
   double out[8];
   CK(cudaMemcpyAsync(out, c->d_energy, sizeof out, cudaMemcpyDeviceToHost, c->st));
   if (int rc = sync_and_check(c)) return rc;
@@ -1215,6 +1373,15 @@ int rt_get_hmatrix(rt_handle c, double* H0) {
   CHECK_HANDLE(c);
   CK(cudaSetDevice(c->cfg.device));
   if (int rc = copy_matrix_out(c, c->H0, H0)) return rc;
+  return sync_and_check(c);
+}
+
+int rt_get_overlap(rt_handle c, double* S, double* Sinv) {
+  CHECK_HANDLE(c);
+  if (!c->nonorth) return fail(c, RT_EINVAL, "rt_get_overlap: handle was created without RT_NONORTHOGONAL");
+  CK(cudaSetDevice(c->cfg.device));
+  if (int rc = copy_matrix_out(c, c->Smat, S)) return rc;
+  if (int rc = copy_matrix_out(c, c->Sinv, Sinv)) return rc;
   return sync_and_check(c);
 }
 
@@ -1286,6 +1453,7 @@ int rt_op_propagate(rt_handle c, const double* Hbar, const double* P0re, const d
   CHECK_HANDLE(c);
   if (c->slab) return fail(c, RT_ESTATE, "rt_op_propagate: not available on a slab handle");
   if (!Hbar || !P0re || !P0im || !P1re || !P1im) return fail(c, RT_EINVAL, "rt_op_propagate: NULL");
+  if (c->general) return fail(c, RT_EINVAL, "rt_op_propagate: takes one Hbar; not defined for magnus_order = 2 / RT_NONORTHOGONAL");
   CK(cudaSetDevice(c->cfg.device));
   const size_t nn = (size_t)c->N * c->ldn;
   // The propagation state owns Hm1/H0/H1/P0/P1 and the series owns X..Sm: the call needs five more N x N matrices.

@@ -50,9 +50,10 @@ __device__ __forceinline__ ProjBlock project_decode(int b, const ProjectPlan& p)
 #endif
 void launch_project(const ProjectPlan& p, const double* phi, const double* w, const int2* tiles, double* W,
                     cudaStream_t st);
-// H[i][j] = scale * sum_s W[s][i][j] (+ eps_i if i == j and eps != nullptr), mirrored to the lower triangle.
+// H[i][j] = scale * sum_s W[s][i][j] (+ eps_i if i == j and eps != nullptr) (+ Hadd[i][j] if Hadd != nullptr), mirrored to
+// the lower triangle.
 void launch_project_reduce(const ProjectPlan& p, const double* W, const double* eps, double scale, double* H,
-                           cudaStream_t st);
+                           cudaStream_t st, const double* Hadd = nullptr);
 size_t project_smem_bytes();
 
 // ---- a5 density: rho_part[p][r] = sum over the j-tiles of pair p of sum_j phi_j(r) (Pfold Phi)_j(r) -------
@@ -116,8 +117,13 @@ size_t gemm_tma_sync_ints(int sms);
 
 // ---- elementwise N x N (a2 and series glue) -------------------------------------------------------------
 // first != 0: H1 = 2 H0 - Hm1 first.  X = dt * ((H0 + H1)/2 - sigma I)
+// S != nullptr (non-orthogonal basis): X = dt * ((H0 + H1)/2 - sigma S)
 void launch_hbar(int N, int ldn, const double* Hm1, const double* H0, double* H1, double* X, double dt,
-                 double sigma, int first, cudaStream_t st);
+                 double sigma, int first, cudaStream_t st, const double* S = nullptr);
+// dP' = (M + M^dagger)/k from R = Re M, I = Im M: Sn = (R + R^T)/k, An = (I - I^T)/k, P1r += Sn, P1i += An  (L434-L438)
+void launch_transpose_add(int N, int ldn, const double* R, const double* I, double inv_k, double* Sn, double* An,
+                          double* P1r, double* P1i, const int* skip, cudaStream_t st);
+void launch_axpby(int N, int ldn, double a, const double* X, double b, const double* Y, double* out, cudaStream_t st);
 // C = I + c1 Y ; S = I + s1 Y
 void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, double* S, double s1, cudaStream_t st);
 // dst = src for n matrices (state shift, line 28)
@@ -161,6 +167,8 @@ void launch_commutator_check(int N, int ldn, const double* dPr, const double* dP
                              cudaStream_t st);
 // cs->H_bits = max |A - B| over the N x N matrices (line 24)
 void launch_maxabs_diff(int N, int ldn, const double* A, const double* B, ConvState* cs, cudaStream_t st);
+void launch_maxabs_minus_identity(int N, int ldn, const double* T, ConvState* cs, cudaStream_t st);
+void launch_trace_product(int N, int ldn, const double* A, const double* B, double* out, cudaStream_t st);   // out[5]
 
 // energy diagnostic: out[0] = sum_r [1/2 drho VH + exc(rho) - exc(rho0) - vxc0 drho + E.r drho], out[5] = sum_i eps_i P_ii
 void launch_energy(long long Ng, GridDims gd, double h, const double* rho, const double* rho0, const double* vxc0,

@@ -31,7 +31,7 @@ def test_header_symbols_exported(built):
 def test_config_struct_layout(built):
     from paper_2410_09189_b200 import binding
     # values printed by a C program (sizeof / offsetof on include/rt_tddft.h, x86-64 SysV ABI)
-    assert ctypes.sizeof(binding.rt_config) == 160 and ctypes.sizeof(binding.rt_slab_buffers) == 48
+    assert ctypes.sizeof(binding.rt_config) == 176 and ctypes.sizeof(binding.rt_slab_buffers) == 48
     assert ctypes.sizeof(binding.rt_shard_buffers) == 64 and binding.rt_shard_buffers.block_count.offset == 40
     assert binding.rt_config.dt.offset == 32 and binding.rt_config.E0.offset == 72
     assert binding.rt_config.flags.offset == 96 and binding.rt_config.stream.offset == 104
@@ -41,6 +41,8 @@ def test_config_struct_layout(built):
     assert binding.rt_config.slab_x0.offset == 140 and binding.rt_config.slab_nx.offset == 144
     assert binding.rt_config.history.offset == 148
     assert binding.rt_config.prop_shards.offset == 152 and binding.rt_config.prop_shard.offset == 156
+    assert binding.rt_config.magnus_order.offset == 160 and binding.rt_config.xc_functional.offset == 164
+    assert binding.rt_config.poisson_order.offset == 168
 
 
 def test_no_cpu_fallback(built):

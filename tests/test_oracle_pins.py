@@ -600,3 +600,117 @@ def test_field_energy_term_and_work_done_by_a_laser(tiny_inputs):
     assert gained > 1e-5                                                # the pulse deposited energy (7.5e-5 Ha)
     assert abs(gained - work) < 1e-11                                   # discrete energy balance of the midpoint rule
     assert np.max(np.abs(es[41:] - es[41])) < 1e-11                     # field off: conserved
+
+
+# ------------------------------------------------------------------ NEXT(4): second Magnus term, non-orthogonal basis
+def _random_sym(rng, n, scale=1.0):
+    A = rng.standard_normal((n, n)) * scale
+    return 0.5 * (A + A.T)
+
+
+def test_magnus_second_term_raises_the_order_to_four():
+    """Eq. 12-13: for a Hamiltonian that IS linear in time, H(t) = A + t B, Omega_1 alone is a
+    second-order integrator and Omega_1 + Omega_2 = -i dt (H0+H1)/2 + dt^2/12 [H0, H1] a fourth-order one.  Reference:
+    scipy's DOP853 on dP/dt = -i [H(t), P] (Eq. 14) at rtol 1e-13 -- an independent library integrator.  A wrong sign
+    or coefficient of Omega_2 leaves the order at two."""
+    import scipy.integrate
+    rng = np.random.default_rng(21)
+    n, T = 6, 1.6
+    A, Bm = _random_sym(rng, n), _random_sym(rng, n, 0.7)
+    C = rng.standard_normal((n, 2)) + 1j * rng.standard_normal((n, 2))
+    Q, _ = np.linalg.qr(C)
+    P0 = 2.0 * Q @ Q.conj().T
+
+    def H(t):
+        return A + t * Bm
+
+    def rhs(t, y):
+        P = y.reshape(n, n)
+        return (-1j * (H(t) @ P - P @ H(t))).reshape(-1)
+
+    ref = scipy.integrate.solve_ivp(rhs, (0.0, T), P0.reshape(-1), method="DOP853", rtol=1e-13, atol=1e-14).y[:, -1].reshape(n, n)
+    errs = {1: [], 2: []}
+    for order in (1, 2):
+        for nst in (8, 16, 32):
+            dt, P = T / nst, P0.copy()
+            for k in range(nst):
+                P = O.propagate_exact_general(H(k * dt), H((k + 1) * dt), P, dt, order)
+            errs[order].append(np.max(np.abs(P - ref)))
+    r1 = [errs[1][i] / errs[1][i + 1] for i in range(2)]
+    r2 = [errs[2][i] / errs[2][i + 1] for i in range(2)]
+    assert all(3.5 < r < 4.5 for r in r1), r1              # second order
+    assert all(13.0 < r < 19.0 for r in r2), r2            # fourth order
+    assert errs[2][0] < 0.05 * errs[1][0] and errs[2][2] < 1e-6
+    # order 1 of the general routine is the plain midpoint propagator
+    assert np.allclose(O.propagate_exact_general(H(0.1), H(0.3), P0, 0.2, 1),
+                       O.propagate_eigh(0.5 * (H(0.1) + H(0.3)), P0, 0.2), rtol=0, atol=1e-14)
+
+
+def test_general_omega_series_equals_exact_exponential():
+    """Eq. 21-23 / 37-38 with a general Omega (second Magnus term, overlap matrix): the series {Omega, .} summed to
+    convergence equals exp(Omega) P exp(Omega)^+ computed by diagonalisation in the Cholesky-orthogonalised basis
+    ("Appendix A.2"); tr(P S) = N_e is invariant (L267); Eq. 33's right-hand side is the derivative."""
+    rng = np.random.default_rng(22)
+    n = 9
+    H0, H1 = _random_sym(rng, n), _random_sym(rng, n)
+    G = rng.standard_normal((n, n)) * 0.2 + np.eye(n)
+    S = G @ G.T                                           # overlap of a non-orthogonal basis
+    Sinv = np.linalg.inv(S)
+    C = rng.standard_normal((n, 3)) + 1j * rng.standard_normal((n, 3))
+    C = C @ np.linalg.inv(np.linalg.cholesky(C.conj().T @ S @ C)).conj().T       # C^+ S C = 1
+    P0 = 2.0 * C @ C.conj().T
+    assert abs(np.trace(P0 @ S).real - 6.0) < 1e-12
+    dt = 0.15
+    for order in (1, 2):
+        for Sm, Si in ((None, None), (S, Sinv)):
+            exact = O.propagate_exact_general(H0, H1, P0, dt, order, Sm)
+            ser, k = O.propagate_omega_series(O.magnus_omega(H0, H1, dt, order, Si), P0, 1e-16)
+            assert np.max(np.abs(ser - exact)) < 5e-14 and 5 < k < 60
+            assert np.max(np.abs(exact - exact.conj().T)) < 1e-13
+            SS = np.eye(n) if Sm is None else S
+            assert abs(np.trace(exact @ SS).real - np.trace(P0 @ SS).real) < 1e-12
+    # Eq. 33: dP/dt = -i (S^-1 H P - P H S^-1)
+    d = 1e-6
+    lhs = (O.propagate_exact_general(H0, H0, P0, d, 1, S) - O.propagate_exact_general(H0, H0, P0, -d, 1, S)) / (2 * d)
+    assert np.allclose(lhs, -1j * (Sinv @ H0 @ P0 - P0 @ H0 @ Sinv), atol=1e-8)
+    # S = 1, order 1: the general series is the commutator series of Eq. 39
+    a, ka = O.propagate_omega_series(O.magnus_omega(H0, H1, dt, 1), P0, 1e-15)
+    b, kb = O.propagate_commutator(0.5 * (H0 + H1), P0, dt, 1e-15)
+    assert ka == kb and np.allclose(a, b, rtol=0, atol=1e-15)
+
+
+def test_observables_do_not_depend_on_the_basis(tiny_inputs):
+    """The whole interacting step in a NON-orthogonal basis Phi_n = A Phi (S = A A^T != 1; H_KS,n = A diag(eps) A^T,
+    P_n = A^-T diag(occ) A^-1, Eq. 33-38) must give the same rho(r, t) and mu(t) as the orthonormal run: the density and
+    the matrix elements are basis-invariant (L267, L612-L618).  Exact-exponential and series modes, with and without
+    the second Magnus term."""
+    w, Phi, eps, occ = tiny_inputs
+    rng = np.random.default_rng(23)
+    A = np.eye(w.norb) + 0.15 * rng.standard_normal((w.norb, w.norb))
+    Ai = np.linalg.inv(A)
+    Phi_n = A @ Phi
+    Hks_n = A @ np.diag(eps) @ A.T
+    P0_n = Ai.T @ np.diag(occ) @ Ai
+    for magnus in (1, 2):
+        a = _make(tiny_inputs, E0=(0.05, 0.0, 0.02), magnus=magnus)
+        kw = dict(dt=w.dt, E0=(0.05, 0.0, 0.02), n_hupdates=2, n_vcycles=w.n_vcycles, magnus=magnus, Hks=Hks_n, P0=P0_n,
+                  nonorthogonal=True)
+        b = O.RTOracle(w.shape, w.h, Phi_n, eps, occ, **kw)
+        c = O.RTOracle(w.shape, w.h, Phi_n, eps, occ, propagator="commutator", dP_thrs=1e-15, **kw)
+        assert np.max(np.abs(b.S - A @ A.T)) < 1e-12 and np.max(np.abs(b.S - np.eye(w.norb))) > 0.1
+        assert np.allclose(a.dipole(), b.dipole(), rtol=0, atol=1e-12)
+        for _ in range(6):
+            a.step(1)
+            b.step(1)
+            c.step(1)
+            assert np.max(np.abs(a.dipole() - b.dipole())) < 1e-11
+            assert np.max(np.abs(a.dipole() - c.dipole())) < 1e-11
+            assert abs(np.trace(b.P0 @ b.S).real - occ.sum()) < 1e-11
+        assert np.max(np.abs(a.density() - b.density())) < 1e-12 * np.max(a.density()) * 10
+        assert np.max(np.abs(A.T @ b.P0 @ A - a.P0)) < 1e-11            # P_o = A^T P_n A
+    # and the second Magnus term changes the trajectory at O(dt^3) per step: visible, small
+    m1, m2 = _make(tiny_inputs, E0=(0.05, 0, 0.02), magnus=1), _make(tiny_inputs, E0=(0.05, 0, 0.02), magnus=2)
+    m1.step(6)
+    m2.step(6)
+    diff = np.max(np.abs(m1.P0 - m2.P0))
+    assert 1e-12 < diff < 1e-3
