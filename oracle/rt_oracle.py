@@ -106,6 +106,115 @@ def exc_density_lda(rho: np.ndarray) -> np.ndarray:
 
 
 # --------------------------------------------------------------------------------------------------
+# PBE generalised-gradient approximation (the functional the paper ran), unpolarised.
+# Perdew, Burke, Ernzerhof, PRL 77, 3865 (1996), restated:  e_xc(n, sigma) = e_x + e_c per unit volume, sigma = |grad n|^2,
+#   e_x = n eps_x^unif(n) F_x(s),  eps_x^unif = -(3/4)(3 n/pi)^(1/3),  s = |grad n| / (2 k_F n),  k_F = (3 pi^2 n)^(1/3),
+#         F_x = 1 + kappa - kappa / (1 + mu s^2 / kappa),  kappa = 0.804,  mu = beta pi^2 / 3
+#   e_c = n [eps_c^unif(r_s) + H(r_s, t)],  t = |grad n| / (2 k_s n),  k_s = sqrt(4 k_F / pi),
+#         H = gamma ln{1 + (beta/gamma) t^2 (1 + A t^2) / (1 + A t^2 + A^2 t^4)},  A = (beta/gamma) / (exp(-eps_c^unif/gamma) - 1),
+#         beta = 0.06672455060314922,  gamma = (1 - ln 2)/pi^2,  eps_c^unif = Perdew-Wang 1992 (PRB 45, 13244) at zeta = 0.
+# On the grid the gradient is a central finite difference D (grad_fd) and E_xc = dVol sum_r e_xc(n_r, |D n|_r^2), whose exact
+# derivative with respect to n_r is the potential used here (the grid analogue of v = d e/d n - div(d e/d grad n)):
+#   v_xc = d e/d n - sum_q D_q (2 d e/d sigma  D_q n)            (D is antisymmetric, so D^T = -D)
+# --------------------------------------------------------------------------------------------------
+PBE_KAPPA = 0.804
+PBE_BETA = 0.06672455060314922
+PBE_GAMMA = (1.0 - np.log(2.0)) / np.pi ** 2
+PBE_MU = PBE_BETA * np.pi ** 2 / 3.0
+PW92_A, PW92_ALPHA1 = 0.0310907, 0.21370
+PW92_B1, PW92_B2, PW92_B3, PW92_B4 = 7.5957, 3.5876, 1.6382, 0.49294
+# central-difference first-derivative weights c_1..c_n (f' ~ sum_i c_i (f_{+i} - f_{-i}) / h) of order 2n (Eq. 2's analogue)
+FD_GRAD = {2: (0.5,), 4: (2.0 / 3.0, -1.0 / 12.0)}
+# second-derivative weights a_0; a_1..a_n of Eq. 2 (L58-L60): f'' ~ (a_0 f_0 + sum_i a_i (f_{+i} + f_{-i})) / h^2, order 2n
+FD_LAPL = {2: (-2.0, (1.0,)), 4: (-5.0 / 2.0, (4.0 / 3.0, -1.0 / 12.0))}
+
+
+def pw92_eps_c(rs):
+    """Perdew-Wang 1992 correlation energy per electron of the unpolarised uniform gas, and d eps_c / d r_s."""
+    sq = np.sqrt(rs)
+    G = PW92_B1 * sq + PW92_B2 * rs + PW92_B3 * rs * sq + PW92_B4 * rs * rs
+    dG = 0.5 * PW92_B1 / sq + PW92_B2 + 1.5 * PW92_B3 * sq + 2.0 * PW92_B4 * rs
+    lg = np.log(1.0 + 1.0 / (2.0 * PW92_A * G))
+    eps = -2.0 * PW92_A * (1.0 + PW92_ALPHA1 * rs) * lg
+    deps = -2.0 * PW92_A * PW92_ALPHA1 * lg + (1.0 + PW92_ALPHA1 * rs) * dG / (G * G + G / (2.0 * PW92_A))
+    return eps, deps
+
+
+def pbe_exc(n, sigma):
+    """(e_xc, d e_xc / d n, d e_xc / d sigma) of PBE for density n > RHO_FLOOR and sigma = |grad n|^2 (arrays).
+    Points with n < RHO_FLOOR give zeros."""
+    n = np.asarray(n, dtype=np.float64)
+    sigma = np.asarray(sigma, dtype=np.float64)
+    e, dn, ds = np.zeros_like(n), np.zeros_like(n), np.zeros_like(n)
+    ok = n >= RHO_FLOOR
+    r, sg = n[ok], sigma[ok]
+    pi = np.pi
+    # ---- exchange
+    Cx = 0.75 * (3.0 / pi) ** (1.0 / 3.0)
+    n13 = np.cbrt(r)
+    q = 1.0 / (4.0 * (3.0 * pi * pi) ** (2.0 / 3.0) * n13 ** 8)          # d s^2 / d sigma
+    p = sg * q                                                            # s^2
+    den = 1.0 + PBE_MU * p / PBE_KAPPA
+    F = 1.0 + PBE_KAPPA - PBE_KAPPA / den
+    dF = PBE_MU / (den * den)
+    ex = -Cx * r * n13 * F
+    dex_dn = -Cx * n13 * ((4.0 / 3.0) * F - (8.0 / 3.0) * p * dF)
+    dex_ds = -Cx * r * n13 * dF * q
+    # ---- correlation
+    rs = np.cbrt(3.0 / (4.0 * pi * r))
+    eps, deps_drs = pw92_eps_c(rs)
+    deps_dn = deps_drs * (-rs / (3.0 * r))
+    du_ds = pi / (16.0 * (3.0 * pi * pi) ** (1.0 / 3.0) * n13 ** 7)      # u = t^2 = sigma * du_ds
+    u = sg * du_ds
+    ex1 = np.exp(-eps / PBE_GAMMA)
+    A = (PBE_BETA / PBE_GAMMA) / (ex1 - 1.0)
+    dA_deps = A * A * ex1 / PBE_BETA
+    Au = A * u
+    Dn = 1.0 + Au + Au * Au
+    Q = u * (1.0 + Au) / Dn
+    H = PBE_GAMMA * np.log(1.0 + (PBE_BETA / PBE_GAMMA) * Q)
+    HQ = PBE_BETA / (1.0 + (PBE_BETA / PBE_GAMMA) * Q)
+    Qu = (1.0 + 2.0 * Au) / (Dn * Dn)
+    QA = -A * u * u * u * (2.0 + Au) / (Dn * Dn)
+    du_dn = -(7.0 / 3.0) * u / r
+    ec = r * (eps + H)
+    dec_dn = eps + H + r * (deps_dn + HQ * (Qu * du_dn + QA * dA_deps * deps_dn))
+    dec_ds = r * HQ * Qu * du_ds
+    e[ok], dn[ok], ds[ok] = ex + ec, dex_dn + dec_dn, dex_ds + dec_ds
+    return e, dn, ds
+
+
+def grad_fd(u: np.ndarray, h: float, order: int = 2):
+    """Central finite-difference gradient (periodic), components along x, y, z; order 2 or 4 (FD_GRAD)."""
+    out = []
+    for ax in range(3):
+        g = np.zeros_like(u)
+        for i, c in enumerate(FD_GRAD[order], start=1):
+            g = g + c * (np.roll(u, -i, ax) - np.roll(u, i, ax))
+        out.append(g / h)
+    return out
+
+
+def vxc_pbe(rho: np.ndarray, shape, h: float, order: int = 2) -> np.ndarray:
+    """PBE potential on the grid: v = d e/d n - sum_q D_q (2 d e/d sigma D_q n)  (flat array in, flat array out)."""
+    n3 = np.asarray(rho, dtype=np.float64).reshape(shape)
+    g = grad_fd(n3, h, order)
+    sigma = g[0] * g[0] + g[1] * g[1] + g[2] * g[2]
+    _, dn, ds = pbe_exc(n3, sigma)
+    v = dn.copy()
+    for ax in range(3):
+        v = v - grad_fd(2.0 * ds * g[ax], h, order)[ax]
+    return v.reshape(-1)
+
+
+def exc_density_pbe(rho: np.ndarray, shape, h: float, order: int = 2) -> np.ndarray:
+    """e_xc(n, |D n|^2) per unit volume on the grid (energy diagnostic)."""
+    n3 = np.asarray(rho, dtype=np.float64).reshape(shape)
+    g = grad_fd(n3, h, order)
+    return pbe_exc(n3, g[0] * g[0] + g[1] * g[1] + g[2] * g[2])[0].reshape(-1)
+
+
+# --------------------------------------------------------------------------------------------------
 # Hartree: periodic 7-point Poisson, fixed count of V(nu1,nu2) cycles, weighted Jacobi (DESIGN R6)
 # --------------------------------------------------------------------------------------------------
 

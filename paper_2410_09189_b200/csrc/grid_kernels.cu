@@ -363,8 +363,7 @@ void launch_transpose_add(int N, int ldn, const double* R, const double* I, doub
 }
 
 // out = a X + b Y (whole N x ldn buffers; padding stays zero)
-__global__ void axpby_kernel(long long n, double a, const double* __restrict__ X, double b, const double* __restrict__ Y,
-                             double* __restrict__ out) {
+__global__ void axpby_kernel(long long n, double a, const double* X, double b, const double* Y, double* out) {   // out may alias X
   for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += (long long)gridDim.x * blockDim.x)
     out[r] = a * X[r] + b * Y[r];
 }
