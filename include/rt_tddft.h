@@ -104,9 +104,13 @@ typedef struct {
   /* -- closer-to-paper physics; all zero = the north_star step ------------------------------- */
   int32_t  magnus_order;    /* 0 or 1: Omega = Omega_1 (Eq. 12, "mid-point"); 2: + Omega_2 = dt^2/12 [H0, H1] (Eq. 13,
                                L125), fourth order in dt.  Needs RT_PROP_COMMUTATOR (the series takes any Omega)     */
-  int32_t  xc_functional;   /* RT_XC_LDA_PZ81 (0, north_star) or RT_XC_PBE (the functional the paper ran, L453)       */
-  int32_t  poisson_order;   /* 0 or 2: 7-point Laplacian in the Hartree solve; 4: fourth-order 13-point stencil
-                               (Eq. 2 with n = 2, L58-L60) as the operator whose solution V_H converges to            */
+  int32_t  xc_functional;   /* RT_XC_LDA_PZ81 (0, north_star) or RT_XC_PBE (the functional the paper ran, L453, L501):
+                               v_xc = de/dn - sum_q D_q (2 de/dsigma D_q rho) with central differences D of fd_order    */
+  int32_t  fd_order;        /* order of the finite-difference operators on the grid (Eq. 2): 0 or 2 = 7-point
+                               Laplacian in the Hartree solve and 2-point gradients; 4 = the 13-point fourth-order
+                               Laplacian as the operator V_H solves -- each of the n_vcycles cycles is then
+                               r = f - A4 u, d = one 7-point V-cycle on (0, r), u += d (multigrid as the preconditioner,
+                               L77; DESIGN R17) -- and 4-point gradients                                              */
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
@@ -204,9 +208,10 @@ int rt_op_density(rt_handle h, const double* reP, double* rho, double sums[5]);
  * (all [N][N], EITHER).  Eq. 12 (L123), Eq. 15 (L143). */
 int rt_op_propagate(rt_handle h, const double* Hbar, const double* P0re, const double* P0im,
                     double* P1re, double* P1im);
-/* a7 "Vh": n_vc V-cycles on -lap_h V = 4 pi (drho - mean drho), warm-started from vh (in/out) (EITHER). */
+/* a7 "Vh": n_vc V-cycles on -lap_h V = 4 pi (drho - mean drho), warm-started from vh (in/out) (EITHER); lap_h and the
+ * cycle follow rt_config.fd_order. */
 int rt_op_hartree(rt_handle h, double* vh, const double* drho, int32_t n_vc);
-/* a8 "exchange/correlation": vxc[Ng] = Slater + PZ81 potential of rho[Ng] (EITHER). */
+/* a8 "exchange/correlation": vxc[Ng] = potential of rho[Ng] (EITHER): Slater + PZ81, or PBE with rt_config.xc_functional. */
 int rt_op_vxc(rt_handle h, const double* rho, double* vxc);
 
 /* ---- grid-slab sharding: one handle per rank, phases separated by the two exchanges of the method --------

@@ -299,14 +299,52 @@ def vcycle(u: np.ndarray, f: np.ndarray, h: float, nu1: int, nu2: int, omega: fl
     return u
 
 
+def apply_A_order(u: np.ndarray, h: float, order: int) -> np.ndarray:
+    """A u = -lap_h u with the (2n+1)-point central second difference of Eq. 2 along every axis,
+    order = 2n (FD_LAPL): order 2 is the 7-point operator of apply_A, order 4 the 13-point one."""
+    a0, an = FD_LAPL[order]
+    out = 3.0 * a0 * u
+    for ax in range(3):
+        for i, a in enumerate(an, start=1):
+            out = out + a * (np.roll(u, i, ax) + np.roll(u, -i, ax))
+    return -out / (h * h)
+
+
+def lambda_1d_order(n: int, h: float, order: int) -> np.ndarray:
+    """Eigenvalues of the periodic 1-D operator -d2/dx2 discretised with FD_LAPL[order] (plane waves are eigenvectors)."""
+    a0, an = FD_LAPL[order]
+    th = 2.0 * np.pi * np.arange(n) / n
+    return -(a0 + sum(2.0 * a * np.cos(i * th) for i, a in enumerate(an, start=1))) / (h * h)
+
+
+def spectral_solve_order(f: np.ndarray, h: float, order: int) -> np.ndarray:
+    """Exact zero-mean solution of apply_A_order(u) = f (FFT); the potential the order-4 Hartree cycle converges to."""
+    nx, ny, nz = f.shape
+    lam = (lambda_1d_order(nx, h, order)[:, None, None] + lambda_1d_order(ny, h, order)[None, :, None]
+           + lambda_1d_order(nz, h, order)[None, None, :])
+    fh = np.fft.fftn(f)
+    lam[0, 0, 0] = 1.0
+    uh = fh / lam
+    uh[0, 0, 0] = 0.0
+    return np.real(np.fft.ifftn(uh))
+
+
 def hartree_mg(VH: np.ndarray, drho: np.ndarray, shape, h: float, n_vc: int,
-               nu1: int = 2, nu2: int = 2, omega: float = 6.0 / 7.0) -> np.ndarray:
-    """n_vc V-cycles on  -lap_h V_H = 4 pi (drho - mean drho), warm-started from VH (flat arrays)."""
+               nu1: int = 2, nu2: int = 2, omega: float = 6.0 / 7.0, order: int = 2) -> np.ndarray:
+    """n_vc V-cycles on  -lap_h V_H = 4 pi (drho - mean drho), warm-started from VH (flat arrays).
+    order = 2: the 7-point operator, u <- vcycle(u, f).  order = 4 (the paper's Laplacians are
+    high-order, Eq. 2-3): V_H solves the 13-point fourth-order operator A4, and the 7-point multigrid cycle
+    acts as its preconditioner -- the way RMG uses multigrid (L77: "multigrid ... as a preconditioner"), DESIGN R17:
+        r = f - A4 u ;  d = vcycle(0, r)  [one V(nu1, nu2) cycle of the 7-point hierarchy, zero initial guess] ;  u <- u + d."""
     f = 4.0 * np.pi * (drho - np.mean(drho))
     u = VH.reshape(shape)
     f = f.reshape(shape)
     for _ in range(n_vc):
-        u = vcycle(u, f, h, nu1, nu2, omega)
+        if order == 2:
+            u = vcycle(u, f, h, nu1, nu2, omega)
+        else:
+            r = f - apply_A_order(u, h, order)
+            u = u + vcycle(np.zeros_like(r), r, h, nu1, nu2, omega)
     return u.reshape(-1)
 
 
@@ -435,7 +473,7 @@ class RTOracle:
     def __init__(self, shape, h, Phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2,
                  nu_pre=2, nu_post=2, omega=6.0 / 7.0, hartree=True, xc=True,
                  propagator="eigh", dP_thrs=1e-10, max_order=200, H_thrs=0.0, max_hupdates=20,
-                 magnus=1, Hks=None, P0=None, nonorthogonal=False):
+                 magnus=1, Hks=None, P0=None, nonorthogonal=False, xc_functional="lda", fd_order=2):
         """propagator = "eigh": exact spectral exponential (north_star).  propagator = "commutator": the
         paper's own series applied to P (Eq. 39, Alg. 1 lines 15-23) until max|dP^(k)| <= dP_thrs
         (Alg. 1 line 5: 1e-10).  H_thrs > 0 turns the fixed count of Hamiltonian updates into the paper's
@@ -444,7 +482,11 @@ class RTOracle:
         magnus = 2 adds the second Magnus term Omega_2 = dt^2/12 [H0, H1] (Eq. 13).  nonorthogonal = True: Phi is
         any basis of real functions, S = dVol Phi Phi^T != 1 and P is propagated with Eq. 33-38 (L262-L304); the
         ground state then enters as a Hamiltonian matrix ``Hks`` [N][N] (instead of eps) and a density matrix ``P0``
-        [N][N] with tr(P0 S) = N_e (instead of occ).  Both options route the propagation through magnus_omega."""
+        [N][N] with tr(P0 S) = N_e (instead of occ).  Both options route the propagation through magnus_omega.
+        xc_functional = "pbe": the GGA the paper ran (L453) instead of north_star's LDA; fd_order = 2 or 4: order of the
+        finite-difference operators on the grid (gradient of the GGA, Laplacian the Hartree potential solves)."""
+        assert xc_functional in ("lda", "pbe") and fd_order in (2, 4)
+        self.xc_functional, self.fd_order = xc_functional, int(fd_order)
         assert propagator in ("eigh", "commutator")
         self.propagator, self.dP_thrs, self.max_order = propagator, float(dP_thrs), int(max_order)
         self.H_thrs, self.max_hupdates = float(H_thrs), int(max_hupdates)
@@ -469,11 +511,21 @@ class RTOracle:
         self.Sinv = np.linalg.inv(self.S) if self.nonorth else None
         self.rho0 = density(self.Phi, self.P0.real)
         self.rho = self.rho0.copy()
-        self.vxc0 = vxc_lda(self.rho0) if self.xc else np.zeros(self.Ng)
+        self.vxc0 = self._vxc(self.rho0) if self.xc else np.zeros(self.Ng)
         self.VH = np.zeros(self.Ng)
         self.E_next = np.zeros(3)
         self.H0 = self.Hks + project(self.Phi, field_potential(self.shape, self.h, np.asarray(E0, float)), self.dVol)
         self.Hm1 = self.H0.copy()
+
+    def _vxc(self, rho):
+        if self.xc_functional == "pbe":
+            return vxc_pbe(rho, self.shape, self.h, self.fd_order)
+        return vxc_lda(rho)
+
+    def _exc(self, rho):
+        if self.xc_functional == "pbe":
+            return exc_density_pbe(rho, self.shape, self.h, self.fd_order)
+        return exc_density_lda(rho)
 
     def set_field(self, E):
         self.E_next = np.asarray(E, dtype=np.float64).copy()
@@ -483,10 +535,10 @@ class RTOracle:
         dv = field_potential(self.shape, self.h, self.E_next)
         if self.hartree:
             self.VH = hartree_mg(self.VH, rho - self.rho0, self.shape, self.h, self.n_vc,
-                                 self.nu1, self.nu2, self.omega)
+                                 self.nu1, self.nu2, self.omega, self.fd_order)
             dv = dv + self.VH
         if self.xc:
-            dv = dv + vxc_lda(rho) - self.vxc0
+            dv = dv + self._vxc(rho) - self.vxc0
         return dv
 
     def _propagate(self, Hbar, H1=None):
@@ -538,7 +590,7 @@ class RTOracle:
         if self.hartree:
             e += 0.5 * self.dVol * float(np.sum(drho * self.VH))
         if self.xc:
-            e += self.dVol * float(np.sum(exc_density_lda(self.rho) - exc_density_lda(self.rho0) - self.vxc0 * drho))
+            e += self.dVol * float(np.sum(self._exc(self.rho) - self._exc(self.rho0) - self.vxc0 * drho))
         e += self.dVol * float(np.sum(field_potential(self.shape, self.h, self.E_next) * drho))
         return e
 

@@ -216,6 +216,170 @@ field_kernel(long long Ng, GridDims gd, double h, const double* __restrict__ E, 
   if (r < Ng) w[r] = field_at(r, gd, h, E);
 }
 
+__global__ void trace_eps_kernel(int N, int ldn, const double* __restrict__ eps, const double* __restrict__ P,
+                                 double* __restrict__ out);
+// ---------------------------------------------------------------------------------------------- a8, GGA
+// PBE (Perdew, Burke, Ernzerhof, PRL 77, 3865), unpolarised, with PW92 uniform-gas correlation -- the functional the
+// paper ran.  Same formulas, symbols and operation order as oracle.pbe_exc:
+//   e = e_x + e_c,  de/dn,  de/dsigma  at (n, sigma = |D n|^2).
+__device__ __forceinline__ void pbe_point(double n, double sigma, double& e, double& dn, double& ds) {
+  e = dn = ds = 0.0;
+  if (!(n >= 1e-30)) return;
+  const double PI = 3.14159265358979323846;
+  const double KAPPA = 0.804, BETA = 0.06672455060314922;
+  const double GAMMA = (1.0 - 0.6931471805599453) / (PI * PI);
+  const double MU = BETA * PI * PI / 3.0;
+  const double A0 = 0.0310907, AL1 = 0.21370, B1 = 7.5957, B2 = 3.5876, B3 = 1.6382, B4 = 0.49294;
+  // exchange
+  const double Cx = 0.75 * cbrt(3.0 / PI);
+  const double n13 = cbrt(n);
+  const double n23 = n13 * n13, n43 = n23 * n23, n83 = n43 * n43;
+  const double c32 = cbrt(3.0 * PI * PI);
+  const double q = 1.0 / (4.0 * c32 * c32 * n83);
+  const double p = sigma * q;
+  const double den = 1.0 + MU * p / KAPPA;
+  const double F = 1.0 + KAPPA - KAPPA / den;
+  const double dF = MU / (den * den);
+  const double ex = -Cx * n * n13 * F;
+  const double dex_dn = -Cx * n13 * ((4.0 / 3.0) * F - (8.0 / 3.0) * p * dF);
+  const double dex_ds = -Cx * n * n13 * dF * q;
+  // correlation (PW92 + H)
+  const double rs = cbrt(3.0 / (4.0 * PI * n));
+  const double sq = sqrt(rs);
+  const double G = B1 * sq + B2 * rs + B3 * rs * sq + B4 * rs * rs;
+  const double dG = 0.5 * B1 / sq + B2 + 1.5 * B3 * sq + 2.0 * B4 * rs;
+  const double lg = log(1.0 + 1.0 / (2.0 * A0 * G));
+  const double eps = -2.0 * A0 * (1.0 + AL1 * rs) * lg;
+  const double deps_drs = -2.0 * A0 * AL1 * lg + (1.0 + AL1 * rs) * dG / (G * G + G / (2.0 * A0));
+  const double deps_dn = deps_drs * (-rs / (3.0 * n));
+  const double du_ds = PI / (16.0 * c32 * n43 * n);            // n^(7/3)
+  const double u = sigma * du_ds;
+  const double ex1 = exp(-eps / GAMMA);
+  const double A = (BETA / GAMMA) / (ex1 - 1.0);
+  const double dA_deps = A * A * ex1 / BETA;
+  const double Au = A * u;
+  const double Dn = 1.0 + Au + Au * Au;
+  const double Q = u * (1.0 + Au) / Dn;
+  const double H = GAMMA * log(1.0 + (BETA / GAMMA) * Q);
+  const double HQ = BETA / (1.0 + (BETA / GAMMA) * Q);
+  const double Qu = (1.0 + 2.0 * Au) / (Dn * Dn);
+  const double QA = -A * u * u * u * (2.0 + Au) / (Dn * Dn);
+  const double du_dn = -(7.0 / 3.0) * u / n;
+  const double ec = n * (eps + H);
+  const double dec_dn = eps + H + n * (deps_dn + HQ * (Qu * du_dn + QA * dA_deps * deps_dn));
+  const double dec_ds = n * HQ * Qu * du_ds;
+  e = ex + ec; dn = dex_dn + dec_dn; ds = dex_ds + dec_ds;
+}
+
+__device__ __forceinline__ int wrap_idx(int i, int n) { i %= n; return i < 0 ? i + n : i; }
+
+// central-difference derivative along one axis at point (ix, iy, iz); ORDER = 2: (f+ - f-)/2h, 4: (2/3)(f+1 - f-1) - (1/12)(f+2 - f-2)
+template <int ORDER>
+__device__ __forceinline__ double ddx(const double* __restrict__ f, GridDims gd, int ix, int iy, int iz, int axis,
+                                      double inv_h) {
+  auto at = [&](int d) {
+    const int x = axis == 0 ? wrap_idx(ix + d, gd.nx) : ix;
+    const int y = axis == 1 ? wrap_idx(iy + d, gd.ny) : iy;
+    const int z = axis == 2 ? wrap_idx(iz + d, gd.nz) : iz;
+    return f[((long long)x * gd.ny + y) * gd.nz + z];
+  };
+  double g = (ORDER == 2 ? 0.5 : 2.0 / 3.0) * (at(1) - at(-1));
+  if (ORDER == 4) g += (-1.0 / 12.0) * (at(2) - at(-2));
+  return g * inv_h;
+}
+
+template <int ORDER>
+__global__ void __launch_bounds__(RB)
+pbe_pass1_kernel(GridDims gd, double inv_h, const double* __restrict__ rho, double* __restrict__ scr,
+                 double* __restrict__ exc) {
+  const long long n = (long long)gd.nx * gd.ny * gd.nz;
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= n) return;
+  const int nyz = gd.ny * gd.nz;
+  const int ix = (int)(r / nyz), rem = (int)(r - (long long)ix * nyz), iy = rem / gd.nz, iz = rem - iy * gd.nz;
+  const double gx = ddx<ORDER>(rho, gd, ix, iy, iz, 0, inv_h);
+  const double gy = ddx<ORDER>(rho, gd, ix, iy, iz, 1, inv_h);
+  const double gz = ddx<ORDER>(rho, gd, ix, iy, iz, 2, inv_h);
+  const double sigma = gx * gx + gy * gy + gz * gz;
+  double e, dn, ds;
+  pbe_point(rho[r], sigma, e, dn, ds);
+  scr[r] = dn;
+  scr[n + r] = 2.0 * ds * gx;
+  scr[2 * n + r] = 2.0 * ds * gy;
+  scr[3 * n + r] = 2.0 * ds * gz;
+  if (exc) exc[r] = e;
+}
+template <int ORDER>
+__global__ void __launch_bounds__(RB)
+pbe_pass2_kernel(GridDims gd, double inv_h, const double* __restrict__ scr, double* __restrict__ out) {
+  const long long n = (long long)gd.nx * gd.ny * gd.nz;
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= n) return;
+  const int nyz = gd.ny * gd.nz;
+  const int ix = (int)(r / nyz), rem = (int)(r - (long long)ix * nyz), iy = rem / gd.nz, iz = rem - iy * gd.nz;
+  double v = scr[r];
+  v -= ddx<ORDER>(scr + n, gd, ix, iy, iz, 0, inv_h);
+  v -= ddx<ORDER>(scr + 2 * n, gd, ix, iy, iz, 1, inv_h);
+  v -= ddx<ORDER>(scr + 3 * n, gd, ix, iy, iz, 2, inv_h);
+  out[r] = v;
+}
+void launch_vxc_pbe(GridDims gd, double h, int order, const double* rho, double* scr, double* out, double* exc,
+                    cudaStream_t st) {
+  const long long n = (long long)gd.nx * gd.ny * gd.nz;
+  const unsigned nb = (unsigned)((n + RB - 1) / RB);
+  if (order == 4) {
+    pbe_pass1_kernel<4><<<nb, RB, 0, st>>>(gd, 1.0 / h, rho, scr, exc);
+    if (out) pbe_pass2_kernel<4><<<nb, RB, 0, st>>>(gd, 1.0 / h, scr, out);
+  } else {
+    pbe_pass1_kernel<2><<<nb, RB, 0, st>>>(gd, 1.0 / h, rho, scr, exc);
+    if (out) pbe_pass2_kernel<2><<<nb, RB, 0, st>>>(gd, 1.0 / h, scr, out);
+  }
+}
+
+__global__ void __launch_bounds__(RB)
+delta_v_assemble_kernel(long long Ng, GridDims gd, double h, const double* __restrict__ vxc,
+                        const double* __restrict__ vxc0, const double* __restrict__ VH, const double* __restrict__ E,
+                        double* __restrict__ w) {
+  const long long r = (long long)blockIdx.x * RB + threadIdx.x;
+  if (r >= Ng) return;
+  double v = field_at(r, gd, h, E);
+  if (VH) v += VH[r];
+  if (vxc) v += vxc[r] - vxc0[r];
+  w[r] = v;
+}
+void launch_delta_v_assemble(long long Ng, GridDims gd, double h, const double* vxc, const double* vxc0, const double* VH,
+                             const double* E, double* w, cudaStream_t st) {
+  delta_v_assemble_kernel<<<(unsigned)((Ng + RB - 1) / RB), RB, 0, st>>>(Ng, gd, h, vxc, vxc0, VH, E, w);
+}
+
+// energy sum for a functional whose e_xc per point was computed separately: sum [1/2 drho VH + exc - exc0 - vxc0 drho + E.r drho]
+__global__ void __launch_bounds__(RB)
+energy_exc_kernel(long long Ng, GridDims gd, double h, const double* __restrict__ rho, const double* __restrict__ rho0,
+                  const double* __restrict__ vxc0, const double* __restrict__ VH, const double* __restrict__ E,
+                  const double* __restrict__ exc, const double* __restrict__ exc0, int use_h, double* __restrict__ bsums) {
+  __shared__ double sh[RB / 32][5];
+  double v[5] = {0, 0, 0, 0, 0};
+  for (long long r = (long long)blockIdx.x * RB + threadIdx.x; r < Ng; r += (long long)gridDim.x * RB) {
+    const double d = rho[r] - rho0[r];
+    double e = field_at(r, gd, h, E) * d;
+    if (use_h) e += 0.5 * d * VH[r];
+    if (exc) e += exc[r] - exc0[r] - vxc0[r] * d;
+    v[0] += e;
+  }
+  block_sum<5>(v, sh);
+  if (threadIdx.x == 0)
+#pragma unroll
+    for (int q = 0; q < 5; ++q) bsums[blockIdx.x * 5 + q] = v[q];
+}
+void launch_energy_exc(long long Ng, GridDims gd, double h, const double* rho, const double* rho0, const double* vxc0,
+                       const double* VH, const double* E, const double* exc, const double* exc0, int use_h, int N, int ldn,
+                       const double* eps, const double* P0r, double* bsums, double* out, cudaStream_t st) {
+  const int nb = reduce_rho_blocks(Ng);
+  energy_exc_kernel<<<nb, RB, 0, st>>>(Ng, gd, h, rho, rho0, vxc0, VH, E, exc, exc0, use_h, bsums);
+  final_sums_kernel<<<1, 32 * 5, 0, st>>>(bsums, nb, 5, out);
+  trace_eps_kernel<<<1, 1024, 0, st>>>(N, ldn, eps, P0r, out);
+}
+
 // Energy diagnostic (conserved after the kick; Figs. 3-4):
 //   E = sum_i eps_i Re P_ii + dVol sum_r [ 1/2 drho V_H + e_xc(rho) - e_xc(rho0) - vxc0 drho + E.r drho ]
 __global__ void __launch_bounds__(RB)

@@ -650,7 +650,7 @@ struct BigCycle {
   }
   void vcycle(int l) {
     const MgLevel& L = s.lv[l];
-    const bool zero = l > 0;
+    const bool zero = l > 0 || s.zero0;
     if (zero && s.nu1 == 0) { cudaMemsetAsync(L.u, 0, (size_t)L.n * 8, st); cur[l] = L.u; }
     else smooth(l, s.nu1, zero);
     launch_resid_restrict(L, s.lv[l + 1], cur[l], st);
@@ -690,16 +690,67 @@ int launch_mg_solve(const MgSolveArgs& s, cudaStream_t st) {
   int lc = 0;
   while (lc < s.nlev - 1 && !fits_smem(s, lc)) ++lc;
   if (lc == 0) {           // the whole hierarchy is small: rhs + every cycle in one launch
-    launch_coarse(s, 0, s.n_vc, 0, 1, st);
+    launch_coarse(s, 0, s.n_vc, s.zero0, s.rhs_given ? 0 : 1, st);
     return 1;
   }
-  launch_poisson_rhs(s.lv[0].n, s.rho, s.rho0, s.sums, s.lv[0].f, st);
+  if (!s.rhs_given) launch_poisson_rhs(s.lv[0].n, s.rho, s.rho0, s.sums, s.lv[0].f, st);
   BigCycle bc{s, lc, st};
   for (int l = 0; l < s.nlev; ++l) bc.cur[l] = s.lv[l].u;
   for (int v = 0; v < s.n_vc; ++v) bc.vcycle(0);
   if (bc.cur[0] != s.lv[0].u)
     cudaMemcpyAsync(s.lv[0].u, bc.cur[0], (size_t)s.lv[0].n * 8, cudaMemcpyDeviceToDevice, st);
-  return bc.launches + 1;
+  return bc.launches + (s.rhs_given ? 0 : 1);
+}
+
+// ---- fourth-order operator (Eq. 2 with n = 2): r = f - A4 u, A4 = -(13-point Laplacian) ---------
+// One thread per point, periodic wrap by index arithmetic; the arrays are L2-resident at every config.
+__global__ void __launch_bounds__(256)
+resid_order4_kernel(GridDims gd, double inv_h2, const double* __restrict__ u, const double* __restrict__ f,
+                    double* __restrict__ r) {
+  const long long n = (long long)gd.nx * gd.ny * gd.nz;
+  const long long p = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (p >= n) return;
+  const int nyz = gd.ny * gd.nz;
+  const int ix = (int)(p / nyz), rem = (int)(p - (long long)ix * nyz), iy = rem / gd.nz, iz = rem - iy * gd.nz;
+  auto at = [&](int x, int y, int z) { return u[((long long)x * gd.ny + y) * gd.nz + z]; };
+  auto wrap = [](int i, int n_) { i %= n_; return i < 0 ? i + n_ : i; };
+  const double c0 = -2.5, c1 = 4.0 / 3.0, c2 = -1.0 / 12.0;
+  double acc = 3.0 * c0 * u[p];
+  // same accumulation order as oracle.apply_A_order: axis by axis, distance 1 then 2, (minus side + plus side)
+  acc += c1 * (at(wrap(ix + 1, gd.nx), iy, iz) + at(wrap(ix - 1, gd.nx), iy, iz));
+  acc += c2 * (at(wrap(ix + 2, gd.nx), iy, iz) + at(wrap(ix - 2, gd.nx), iy, iz));
+  acc += c1 * (at(ix, wrap(iy + 1, gd.ny), iz) + at(ix, wrap(iy - 1, gd.ny), iz));
+  acc += c2 * (at(ix, wrap(iy + 2, gd.ny), iz) + at(ix, wrap(iy - 2, gd.ny), iz));
+  acc += c1 * (at(ix, iy, wrap(iz + 1, gd.nz)) + at(ix, iy, wrap(iz - 1, gd.nz)));
+  acc += c2 * (at(ix, iy, wrap(iz + 2, gd.nz)) + at(ix, iy, wrap(iz - 2, gd.nz)));
+  r[p] = f[p] - (-acc * inv_h2);
+}
+__global__ void __launch_bounds__(256) add_inplace_kernel(long long n, double* __restrict__ u, const double* __restrict__ d) {
+  const long long p = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (p < n) u[p] += d[p];
+}
+
+// Hartree solve with the fourth-order operator: the 7-point V-cycle is the preconditioner (oracle.hartree_mg, order = 4):
+//   f4 = 4 pi (rho - rho0 - mean);  n_vc times:  r = f4 - A4 u ;  d = Vcycle_7pt(0, r) ;  u += d.
+// `s.lv[0].u` is the warm-started potential; `dl0` supplies level-0 arrays of the correction hierarchy (u = d, f = r) and
+// f4 the right-hand side.  Returns the number of kernels enqueued.
+int launch_mg_solve_order4(const MgSolveArgs& s, const MgLevel& dl0, double* f4, cudaStream_t st) {
+  const MgLevel& L0 = s.lv[0];
+  const unsigned nb = (unsigned)((L0.n + 255) / 256);
+  launch_poisson_rhs(L0.n, s.rho, s.rho0, s.sums, f4, st);
+  int launches = 1;
+  MgLevel lv[MG_MAX_LEVELS];
+  for (int l = 0; l < s.nlev; ++l) lv[l] = s.lv[l];
+  lv[0] = dl0;
+  MgSolveArgs d = s;
+  d.lv = lv; d.n_vc = 1; d.zero0 = 1; d.rhs_given = 1;
+  for (int v = 0; v < s.n_vc; ++v) {
+    resid_order4_kernel<<<nb, 256, 0, st>>>(L0.gd, 1.0 / (L0.h * L0.h), L0.u, f4, dl0.f);
+    launches += 1 + launch_mg_solve(d, st);
+    add_inplace_kernel<<<nb, 256, 0, st>>>(L0.n, L0.u, dl0.u);
+    launches += 1;
+  }
+  return launches;
 }
 
 }  // namespace rt

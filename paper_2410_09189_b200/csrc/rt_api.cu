@@ -75,6 +75,11 @@ struct rt_ctx {
   double *Hks = nullptr;          // ground-state Hamiltonian matrix when it is not diag(eps)   (rt_create_general)
   double *Smat = nullptr, *Sinv = nullptr, *Bm = nullptr, *Wm = nullptr, *Rt = nullptr, *It = nullptr;
   int newton_iters = 0;           // Newton-Schulz iterations that S^-1 took at create
+  int xc_kind = RT_XC_LDA_PZ81;   // RT_XC_PBE: GGA with finite-difference gradients (grid_kernels.cu)
+  int fd_order = 2;               // order of the grid operators: gradient of the GGA, Laplacian of the Hartree solve
+  double *pbe_scr = nullptr, *vxc_cur = nullptr, *exc_a = nullptr, *exc_b = nullptr;     // [4 Ng], [Ng], [Ng], [Ng]
+  double *f4 = nullptr;           // right-hand side of the fourth-order Hartree solve
+  MgLevel dl0{};                  // level-0 arrays of its correction hierarchy
   int slab_more = 0;              // decision of the last RT_SLAB_CHECK: another Hamiltonian update is needed
   std::map<int, cudaGraphExec_t> phase_exec;      // slab phases captured as CUDA graphs, key = 2 * phase + (it == 0)
   std::map<int, int64_t> phase_launches;
@@ -486,7 +491,19 @@ void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double
 void enqueue_poisson(rt_ctx* c, const std::vector<MgLevel>& lv, int n_vc, const double* rho, const double* rho0) {
   MgSolveArgs s{lv.data(), (int)lv.size(), n_vc, c->nu1, c->nu2, c->omega, c->Qx, c->Qy, c->Qz, c->lx, c->ly, c->lz,
                 rho, rho0, c->d_sums};
-  c->launches += launch_mg_solve(s, c->st);
+  if (c->fd_order == 4) c->launches += launch_mg_solve_order4(s, c->dl0, c->f4, c->st);   // 13-point operator, MG-preconditioned
+  else c->launches += launch_mg_solve(s, c->st);
+}
+
+// v_xc(rho) into out (LDA: one elementwise kernel; PBE: gradient pass + divergence pass)
+void enqueue_vxc(rt_ctx* c, const double* rho, double* out) {
+  if (c->xc_kind == RT_XC_PBE) {
+    launch_vxc_pbe(c->gd, c->h, c->fd_order, rho, c->pbe_scr, out, nullptr, c->st);
+    c->launches += 2;
+  } else {
+    launch_vxc(c->Ng, rho, out, c->st);
+    c->launches += 1;
+  }
 }
 
 // eps != nullptr: the ground-state Hamiltonian is added -- diag(eps), or the matrix Hks of rt_create_general
@@ -536,7 +553,12 @@ void enqueue_update_potential(rt_ctx* c) {
   }
 
   stage_begin(c, RT_STAGE_XC);
-  launch_delta_v(c->Ng, c->gd, c->h, c->rho, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->w, c->st);
+  if (c->xc_kind == RT_XC_PBE && c->use_xc) {
+    enqueue_vxc(c, c->rho, c->vxc_cur);
+    launch_delta_v_assemble(c->Ng, c->gd, c->h, c->vxc_cur, c->vxc0, c->use_h ? c->lv[0].u : nullptr, c->d_E, c->w, c->st);
+  } else {
+    launch_delta_v(c->Ng, c->gd, c->h, c->rho, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->w, c->st);
+  }
   c->launches += 1;
   stage_end(c);
 
@@ -648,6 +670,10 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
                               "series (Eq. 37-38): set propagator = RT_PROP_COMMUTATOR");
   if (want_general && cfg->slab_nx > 0)
     return fail(c, RT_EINVAL, "rt_create: magnus_order = 2 / RT_NONORTHOGONAL are not available on slab handles");
+  if (cfg->xc_functional != RT_XC_LDA_PZ81 && cfg->xc_functional != RT_XC_PBE)
+    return fail(c, RT_EINVAL, "rt_create: unknown xc_functional");
+  if (cfg->fd_order != 0 && cfg->fd_order != 2 && cfg->fd_order != 4)
+    return fail(c, RT_EINVAL, "rt_create: fd_order must be 0, 2 or 4");
   if (want_nonorth && !(Hks_in && P0re_in))
     return fail(c, RT_EINVAL, "rt_create: RT_NONORTHOGONAL needs the ground state as matrices (rt_create_general)");
   if (cfg->nx < 2 || cfg->ny < 2 || cfg->nz < 2) return fail(c, RT_EINVAL, "rt_create: grid dims must be >= 2");
@@ -713,6 +739,8 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
   c->use_h = !(cfg->flags & RT_NO_HARTREE);
   c->use_xc = !(cfg->flags & RT_NO_XC);
   c->use_graph = !(cfg->flags & RT_NO_GRAPH);
+  c->xc_kind = cfg->xc_functional;
+  c->fd_order = cfg->fd_order == 4 ? 4 : 2;
   c->magnus = cfg->magnus_order >= 2 ? 2 : 1;
   c->nonorth = want_nonorth;
   c->general = want_general;
@@ -928,6 +956,15 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
   CKC(cudaMemsetAsync(c->w, 0, (size_t)(NgF + 16) * 8, c->st));
   CKC(cudaMemsetAsync(c->op_u, 0, (size_t)(NgF + 16) * 8, c->st));
   ALLOC(c->rho_part, (size_t)c->dp.ntypes * Ng);
+  if (c->xc_kind == RT_XC_PBE) {
+    ALLOC(c->pbe_scr, 4 * (size_t)NgF); ALLOC(c->vxc_cur, NgF); ALLOC(c->exc_a, NgF); ALLOC(c->exc_b, NgF);
+  }
+  if (c->fd_order == 4 && c->use_h) {
+    ALLOC(c->f4, NgF);
+    c->dl0 = c->lv[0];
+    ALLOC(c->dl0.u, NgF); ALLOC(c->dl0.tmp, NgF); ALLOC(c->dl0.f, NgF); ALLOC(c->dl0.r, NgF);
+    CKC(cudaMemsetAsync(c->dl0.u, 0, (size_t)NgF * 8, c->st));
+  }
   ALLOC(c->d_segs, c->segs.size());
   CKC(cudaMemcpyAsync(c->d_segs, c->segs.data(), c->segs.size() * sizeof(DensSeg), cudaMemcpyHostToDevice, c->st));
   for (size_t l = 0; l < c->lv.size(); ++l) {
@@ -1038,7 +1075,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
   if (!c->slab) {
     enqueue_density(c, c->P0r, c->rho0, nullptr);
     CKC(cudaMemcpyAsync(c->rho, c->rho0, (size_t)Ng * 8, cudaMemcpyDeviceToDevice, c->st));
-    launch_vxc(Ng, c->rho0, c->vxc0, c->st);
+    enqueue_vxc(c, c->rho0, c->vxc0);
     enqueue_project(c, c->w, c->d_eps, c->H0);
     CKC(cudaMemcpyAsync(c->Hm1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
     CKC(cudaMemcpyAsync(c->H1, c->H0, nn * 8, cudaMemcpyDeviceToDevice, c->st));
@@ -1346,8 +1383,16 @@ int rt_get_energy(rt_handle c, double* energy) {
   if (!energy) return fail(c, RT_EINVAL, "rt_get_energy: NULL");
   if (c->slab && c->slab_state != 1) return fail(c, RT_ESTATE, "rt_get_energy: RT_SLAB_INIT has not run");
   CK(cudaSetDevice(c->cfg.device));
-  launch_energy(c->Ng, c->gd, c->h, c->rho, c->rho0, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->N, c->ldn,
-                c->d_eps, c->P0r, c->d_bsums, c->d_energy, c->st);
+  if (c->xc_kind == RT_XC_PBE && c->use_xc) {
+    launch_vxc_pbe(c->gd, c->h, c->fd_order, c->rho, c->pbe_scr, nullptr, c->exc_a, c->st);     // e_xc(rho), e_xc(rho0)
+    launch_vxc_pbe(c->gd, c->h, c->fd_order, c->rho0, c->pbe_scr, nullptr, c->exc_b, c->st);
+    launch_energy_exc(c->Ng, c->gd, c->h, c->rho, c->rho0, c->vxc0, c->lv[0].u, c->d_E, c->exc_a, c->exc_b, c->use_h, c->N,
+                      c->ldn, c->d_eps, c->P0r, c->d_bsums, c->d_energy, c->st);
+    c->launches += 2;
+  } else {
+    launch_energy(c->Ng, c->gd, c->h, c->rho, c->rho0, c->vxc0, c->lv[0].u, c->d_E, c->use_h, c->use_xc, c->N, c->ldn,
+                  c->d_eps, c->P0r, c->d_bsums, c->d_energy, c->st);
+  }
   c->launches += 3;
   if (c->Hks) {                                      // tr(H_KS Re P) replaces sum_i eps_i Re P_ii
     launch_trace_product(c->N, c->ldn, c->Hks, c->P0r, c->d_energy, c->st);
@@ -1516,8 +1561,7 @@ int rt_op_vxc(rt_handle c, const double* rho, double* vxc) {
   CK(cudaSetDevice(c->cfg.device));
   CK(cudaMemcpyAsync(c->op_u, rho, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
   stage_begin(c, RT_STAGE_XC);
-  launch_vxc(c->Ng, c->op_u, c->w, c->st);
-  c->launches += 1;
+  enqueue_vxc(c, c->op_u, c->w);
   stage_end(c);
   CK(cudaMemcpyAsync(vxc, c->w, (size_t)c->Ng * 8, cudaMemcpyDefault, c->st));
   return sync_and_check(c);
@@ -1588,8 +1632,7 @@ int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
     case RT_SLAB_INIT:            // xchg_rho holds rho0 of the whole grid, xchg_H holds H(t = 0)  (Alg. 1 lines 7-8)
       if (c->slab_state != 0) return fail(c, RT_ESTATE, "rt_slab_phase: RT_SLAB_INIT already done");
       CK(cudaMemcpyAsync(c->rho0, c->rho, (size_t)c->Ng * 8, cudaMemcpyDeviceToDevice, c->st));
-      launch_vxc(c->Ng, c->rho0, c->vxc0, c->st);
-      c->launches += 1;
+      enqueue_vxc(c, c->rho0, c->vxc0);
       CK(cudaMemcpyAsync(c->H0, c->H1, nn, cudaMemcpyDeviceToDevice, c->st));
       CK(cudaMemcpyAsync(c->Hm1, c->H1, nn, cudaMemcpyDeviceToDevice, c->st));
       CK(cudaMemsetAsync(c->d_sums + 4, 0, 8, c->st));       // induced charge at t = 0

@@ -145,6 +145,16 @@ void launch_reduce_rho(const double* rho_part, int nparts, long long Ng, GridDim
 void launch_delta_v(long long Ng, GridDims gd, double h, const double* rho, const double* vxc0, const double* VH,
                     const double* E, int use_h, int use_xc, double* w, cudaStream_t st);
 void launch_vxc(long long Ng, const double* rho, double* vxc, cudaStream_t st);
+// PBE on the grid (oracle.vxc_pbe): pass 1 a = d e/d n, b_q = 2 d e/d sigma D_q rho (scr: 4 arrays of Ng, [a | bx | by | bz]);
+// pass 2 out = a - sum_q D_q b_q; order = 2 or 4 (central differences).  exc != nullptr: also e_xc per point (energy).
+void launch_vxc_pbe(GridDims gd, double h, int order, const double* rho, double* scr, double* out, double* exc,
+                    cudaStream_t st);
+// out[r] = fld(r) + (VH ? VH[r] : 0) + (vxc ? vxc[r] - vxc0[r] : 0)   (dV assembly when v_xc was computed separately)
+void launch_energy_exc(long long Ng, GridDims gd, double h, const double* rho, const double* rho0, const double* vxc0,
+                       const double* VH, const double* E, const double* exc, const double* exc0, int use_h, int N, int ldn,
+                       const double* eps, const double* P0r, double* bsums, double* out, cudaStream_t st);
+void launch_delta_v_assemble(long long Ng, GridDims gd, double h, const double* vxc, const double* vxc0, const double* VH,
+                             const double* E, double* w, cudaStream_t st);
 void launch_field(long long Ng, GridDims gd, double h, const double* E, double* w, cudaStream_t st);
 void launch_set_field(double* dE, double ex, double ey, double ez, cudaStream_t st);   // dE[0..2] = E, by value
 // f = 4 pi (rho - rho0 - sums[4]/Ng)      (rho0 may be nullptr: f = 4 pi (rho - sums[4]/Ng))
@@ -195,9 +205,13 @@ struct MgSolveArgs {
   const double *Qx, *Qy, *Qz, *lx, *ly, *lz;     // eigenbasis of the coarsest level (exact zero-mean solve)
   const double* rho; const double* rho0;         // rho0 may be nullptr
   const double* sums;                            // sums[4] = sum(rho - rho0)
+  int zero0 = 0;                                 // level 0 starts from a zero guess (the cycle is used as a preconditioner)
+  int rhs_given = 0;                             // lv[0].f already holds the right-hand side (rho, rho0, sums unused)
 };
 int init_mg_kernels();                           // dynamic shared-memory attributes; returns a cudaError_t value
 int launch_mg_solve(const MgSolveArgs& s, cudaStream_t st);
+// fourth-order operator, the 7-point cycle as preconditioner (mg_kernels.cu); dl0: level-0 arrays of the correction, f4: rhs
+int launch_mg_solve_order4(const MgSolveArgs& s, const MgLevel& dl0, double* f4, cudaStream_t st);
 // block sums of drho for rt_op_hartree (mean removal): sums[4] = sum(drho)
 void launch_sum_only(const double* v, long long n, double* bsums, double* sums, cudaStream_t st);
 

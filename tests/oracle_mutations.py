@@ -21,7 +21,7 @@ MUTATIONS = [
     ("step: line 14 midpoint", "Hbar = 0.5 * (self.H0 + H1)", "Hbar = H1"),
     ("step: line 28 shift order", "self.Hm1, self.H0, self.P0 = self.H0, H1, P1", "self.Hm1, self.H0, self.P0 = H1, H1, P1"),
     ("delta_v: E(t_{n+1}).x term", "dv = field_potential(self.shape, self.h, self.E_next)", "dv = 0.0 * field_potential(self.shape, self.h, self.E_next)"),
-    ("delta_v: - vxc0", "dv = dv + vxc_lda(rho) - self.vxc0", "dv = dv + vxc_lda(rho)"),
+    ("delta_v: - vxc0", "dv = dv + self._vxc(rho) - self.vxc0", "dv = dv + self._vxc(rho)"),
     ("delta_v: + V_H", "dv = dv + self.VH", "dv = dv - self.VH"),
     ("set_field: stored value", "self.E_next = np.asarray(E, dtype=np.float64).copy()", "self.E_next = 0.5 * np.asarray(E, dtype=np.float64).copy()"),
     ("__init__: H0 holds V(t_0)", "self.H0 = np.diag(self.eps) + project(", "self.H0 = np.diag(self.eps) + 0.0 * project("),
@@ -45,6 +45,21 @@ MUTATIONS = [
     ("hartree_mg: 4 pi", "f = 4.0 * np.pi * (drho - np.mean(drho))", "f = 2.0 * np.pi * (drho - np.mean(drho))"),
     ("spectral_solve: zero mode", "uh[0, 0, 0] = 0.0", "uh[0, 0, 0] = fh[0, 0, 0]"),
     ("energy: Hartree 1/2", "e += 0.5 * self.dVol * float(np.sum(drho * self.VH))", "e += self.dVol * float(np.sum(drho * self.VH))"),
+    ("magnus_omega: sign of Omega_2 (Eq. 13)", "Om = Om + (dt * dt / 12.0) * (H0 @ H1 - H1 @ H0)", "Om = Om - (dt * dt / 12.0) * (H0 @ H1 - H1 @ H0)"),
+    ("magnus_omega: 1/12", "Om = Om + (dt * dt / 12.0) * (H0 @ H1 - H1 @ H0)", "Om = Om + (dt * dt / 6.0) * (H0 @ H1 - H1 @ H0)"),
+    ("magnus_omega: S^-1 side (Eq. 36)", "H0, H1 = Sinv @ H0, Sinv @ H1", "H0, H1 = H0 @ Sinv, H1 @ Sinv"),
+    ("propagate_omega_series: Omega^dagger", "dP = (Om @ dP + dP @ Om.conj().T) / k", "dP = (Om @ dP + dP @ Om.T) / k"),
+    ("propagate_exact_general: back-transform", "P1 = Li.T @ P1 @ Li", "P1 = Li @ P1 @ Li.T"),
+    ("pbe_exc: kappa", "PBE_KAPPA = 0.804", "PBE_KAPPA = 0.84"),
+    ("pbe_exc: d s^2/d n", "dex_dn = -Cx * n13 * ((4.0 / 3.0) * F - (8.0 / 3.0) * p * dF)", "dex_dn = -Cx * n13 * ((4.0 / 3.0) * F - (4.0 / 3.0) * p * dF)"),
+    ("pbe_exc: t^2 prefactor", "du_ds = pi / (16.0 * (3.0 * pi * pi) ** (1.0 / 3.0) * n13 ** 7)", "du_ds = pi / (8.0 * (3.0 * pi * pi) ** (1.0 / 3.0) * n13 ** 7)"),
+    ("pbe_exc: dA/d eps", "dA_deps = A * A * ex1 / PBE_BETA", "dA_deps = A * ex1 / PBE_BETA"),
+    ("pw92: beta_3", "PW92_B1, PW92_B2, PW92_B3, PW92_B4 = 7.5957, 3.5876, 1.6382, 0.49294", "PW92_B1, PW92_B2, PW92_B3, PW92_B4 = 7.5957, 3.5876, 1.3682, 0.49294"),
+    ("vxc_pbe: divergence sign", "v = v - grad_fd(2.0 * ds * g[ax], h, order)[ax]", "v = v + grad_fd(2.0 * ds * g[ax], h, order)[ax]"),
+    ("vxc_pbe: factor 2", "v = v - grad_fd(2.0 * ds * g[ax], h, order)[ax]", "v = v - grad_fd(ds * g[ax], h, order)[ax]"),
+    ("FD_GRAD: fourth-order weights", "FD_GRAD = {2: (0.5,), 4: (2.0 / 3.0, -1.0 / 12.0)}", "FD_GRAD = {2: (0.5,), 4: (2.0 / 3.0, 1.0 / 12.0)}"),
+    ("FD_LAPL: fourth-order weights", "4: (-5.0 / 2.0, (4.0 / 3.0, -1.0 / 12.0))", "4: (-5.0 / 2.0, (4.0 / 3.0, -1.0 / 6.0))"),
+    ("hartree_mg order 4: residual operator", "r = f - apply_A_order(u, h, order)", "r = f - apply_A(u, h)"),
     ("dipole_strength: sign", "S[iw] = -(2.0 * w / (len(used) * np.pi)) * acc", "S[iw] = (2.0 * w / (len(used) * np.pi)) * acc"),
 ]
 

@@ -121,3 +121,85 @@ def test_general_mode_argument_checks(B):
     assert np.array_equal(a.dipole(), b.dipole())
     a.close()
     b.close()
+
+
+# ------------------------------------------------------------------ PBE and the fourth-order grid operators
+@pytest.mark.parametrize("name", ["tiny", "ragged", "small", "odd"])
+@pytest.mark.parametrize("order", [2, 4])
+def test_stage_vxc_pbe(B, name, order):
+    """rt_op_vxc with xc_functional = PBE against oracle.vxc_pbe (gradient pass + divergence pass), on the real rho0 of
+    the workload and on a rough positive field spanning five decades (large reduced gradients)."""
+    w = WORKLOADS[name]
+    Phi, eps, occ = make_inputs_numpy(w)
+    gpu = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, xc_functional="pbe", fd_order=order)
+    rng = np.random.default_rng(51)
+    rho0 = O.density(Phi, np.diag(occ))
+    rough = np.exp(rng.uniform(np.log(1e-5), np.log(1.0), w.ngrid))
+    for rho in (rho0, rough):
+        out = B.rt_op_vxc(gpu.handle, rho, np.empty(w.ngrid))
+        ref = O.vxc_pbe(rho, w.shape, w.h, order)
+        assert np.max(np.abs(out - ref)) < 1e-11 * np.max(np.abs(ref))
+    gpu.close()
+
+
+@pytest.mark.parametrize("name", ["tiny", "ragged", "small"])
+def test_stage_hartree_fourth_order(B, name):
+    """rt_op_hartree with fd_order = 4: r = f - A4 u, one 7-point V-cycle on (0, r), u += d, per cycle -- against
+    oracle.hartree_mg(order = 4); converged, it reaches the FFT solution of the 13-point operator."""
+    w = WORKLOADS[name]
+    Phi, eps, occ = make_inputs_numpy(w)
+    gpu = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, w.dt, n_vcycles=w.n_vcycles, fd_order=4)
+    rng = np.random.default_rng(52)
+    drho = rng.standard_normal(w.ngrid)
+    v0 = rng.standard_normal(w.ngrid) * 0.1
+    for ncyc in (0, 1, w.n_vcycles):
+        vh = B.rt_op_hartree(gpu.handle, v0.copy(), drho, ncyc)
+        ref = O.hartree_mg(v0.copy(), drho, w.shape, w.h, ncyc, order=4)
+        assert np.max(np.abs(vh - ref)) < 1e-12 * max(1.0, np.max(np.abs(ref)))
+    vh = B.rt_op_hartree(gpu.handle, np.zeros(w.ngrid), drho, 18)
+    exact = O.spectral_solve_order((4 * np.pi * (drho - drho.mean())).reshape(w.shape), w.h, 4).reshape(-1)
+    assert np.max(np.abs(vh - exact)) / np.max(np.abs(exact)) < 1e-8
+    gpu.close()
+
+
+@pytest.mark.parametrize("name,nsteps,xc,order", [("tiny", 20, "pbe", 2), ("tiny", 20, "pbe", 4), ("tiny", 10, "lda", 4),
+                                                  ("ragged", 8, "pbe", 4), ("small", 4, "pbe", 4), ("odd", 8, "pbe", 4)])
+def test_step_parity_pbe_and_fourth_order(B, name, nsteps, xc, order):
+    """The whole time step (Taylor propagator) with the paper's functional and high-order grid operators, 1e-9 gate."""
+    w = strong_kick(WORKLOADS[name], 0.1)
+    Phi, eps, occ = make_inputs_numpy(w)
+    kw = dict(dt=w.dt, E0=w.kick, n_hupdates=2, n_vcycles=w.n_vcycles, xc_functional=xc, fd_order=order)
+    gpu = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, **kw)
+    cpu = O.RTOracle(w.shape, w.h, Phi, eps, occ, **kw)
+    mg, mc = [gpu.dipole()], [cpu.dipole()]
+    assert abs(gpu.energy() - cpu.energy()) < 1e-11 * abs(cpu.energy())
+    for _ in range(nsteps):
+        gpu.step(1)
+        cpu.step(1)
+        mg.append(gpu.dipole())
+        mc.append(cpu.dipole())
+    mg, mc = np.array(mg), np.array(mc)
+    assert np.max(np.abs(mc - mc[0])) > 1e-5
+    assert np.max(np.abs(mg - mc)) / np.max(np.abs(mc)) < TOL
+    assert np.max(np.abs(gpu.density() - cpu.density())) / np.max(np.abs(cpu.density())) < TOL
+    assert np.max(np.abs(gpu.pmatrix() - cpu.P0)) < 1e-9
+    assert abs(gpu.energy() - cpu.energy()) < 1e-10 * abs(cpu.energy())
+    gpu.close()
+
+
+def test_everything_the_paper_ran_together(B):
+    """PBE + fourth-order operators + second Magnus term + the paper's series with its dynamic dP_thrs / H_thrs loops."""
+    w = strong_kick(WORKLOADS["ragged"], 0.05)
+    Phi, eps, occ = make_inputs_numpy(w)
+    kw = dict(dt=w.dt, E0=w.kick, n_vcycles=w.n_vcycles, xc_functional="pbe", fd_order=4, magnus=2, propagator="commutator",
+              dP_thrs=1e-12, H_thrs=1e-8, max_hupdates=12)
+    gpu = B.RTTDDFT(w.shape, w.h, Phi, eps, occ, **kw)
+    cpu = O.RTOracle(w.shape, w.h, Phi, eps, occ, **kw)
+    for _ in range(5):
+        gpu.step(1)
+        cpu.step(1)
+        conv = gpu.convergence()
+        assert conv["hupdates"] == cpu.last_hupdates or abs(cpu.last_H_err / 1e-8 - 1) < 1e-3
+        assert np.max(np.abs(gpu.dipole() - cpu.dipole())) / np.max(np.abs(cpu.dipole())) < TOL
+    assert np.max(np.abs(gpu.density() - cpu.density())) / np.max(np.abs(cpu.density())) < TOL
+    gpu.close()

@@ -714,3 +714,158 @@ def test_observables_do_not_depend_on_the_basis(tiny_inputs):
     m2.step(6)
     diff = np.max(np.abs(m1.P0 - m2.P0))
     assert 1e-12 < diff < 1e-3
+
+
+# ------------------------------------------------------------------ NEXT(4): PBE and the fourth-order grid operators
+def test_pbe_uniform_limit_and_bounds():
+    """PBE (PRL 77, 3865) restated in oracle.pbe_exc.  (i) sigma = 0: e_xc/n = Dirac exchange + PW92 correlation, which
+    reproduces the uniform-gas QMC energies (tests/golden) and agrees with the PZ81 fit of the same data; (ii) s -> inf:
+    F_x -> 1 + kappa = 1.804 (the local Lieb-Oxford bound PBE is built on) and H -> -eps_c, so e_xc -> 1.804 e_x^unif;
+    (iii) sigma -> 0: the gradient coefficients of exchange and correlation cancel EXACTLY because mu = beta pi^2/3 (PBE's
+    recovery of the LSD linear response) -- d e/d sigma vanishes relative to either part."""
+    g = _gold()
+    ex_rs, _ = g["dirac_ex_times_rs"]
+    for key, rs in (("ec_rs1", 1.0), ("ec_rs2", 2.0), ("ec_rs5", 5.0), ("ec_rs10", 10.0)):
+        n = np.array([rho_of_rs(rs)])
+        e = O.pbe_exc(n, np.zeros(1))[0][0] / n[0]
+        assert abs(e - ex_rs / rs - g[key][0]) < g[key][1]
+        assert abs(e - O.exc_density_lda(n * (1 - 1e-14))[0] / n[0]) < 1.5e-3            # PW92 vs PZ81: two fits, one data set
+    Cx = 0.75 * (3 / math.pi) ** (1 / 3)
+    for n in (1e-3, 0.05, 2.0):
+        e = O.pbe_exc(np.array([n]), np.array([1e12 * n ** (8 / 3)]))[0][0]
+        assert abs(e / (-Cx * n ** (4 / 3)) - 1.804) < 1e-6
+    assert abs(O.PBE_MU - 0.2195149727645171) < 1e-15 and abs(O.PBE_GAMMA - 0.031090690869654895) < 1e-16
+    for n in (0.01, 0.3, 4.0):
+        kF = (3 * math.pi ** 2 * n) ** (1 / 3)
+        part = 3 * O.PBE_MU / (16 * math.pi * kF * n)                                    # |d e_x / d sigma| at sigma = 0
+        ds = O.pbe_exc(np.array([n]), np.array([1e-14]))[2][0]
+        assert abs(ds) < 1e-9 * part
+
+
+def test_pbe_derivatives_by_numerical_differentiation():
+    """d e/d n and d e/d sigma of pbe_exc against central differences of e itself (5-point stencil), over six decades
+    of density and gradient.  Catches a slipped term anywhere in the chain rule (A(eps_c), t^2(n), s^2(n), PW92')."""
+    rng = np.random.default_rng(41)
+    n = np.exp(rng.uniform(np.log(1e-4), np.log(5.0), 400))
+    s2 = np.exp(rng.uniform(np.log(1e-3), np.log(50.0), 400))                            # reduced gradient squared
+    sigma = s2 * 4.0 * (3 * np.pi ** 2) ** (2 / 3) * n ** (8 / 3)
+    e, dn, ds = O.pbe_exc(n, sigma)
+
+    def d5(f, x, rel):
+        d = rel * x
+        return (f(x - 2 * d) - 8 * f(x - d) + 8 * f(x + d) - f(x + 2 * d)) / (12 * d)
+
+    fd_n = d5(lambda x: O.pbe_exc(x, sigma)[0], n, 1e-4)
+    fd_s = d5(lambda x: O.pbe_exc(n, x)[0], sigma, 1e-3)
+    assert np.max(np.abs(fd_n - dn) / np.abs(dn)) < 1e-8
+    # exchange and correlation nearly cancel in d e/d sigma (see the test above), so the difference quotient's rounding
+    # noise is measured against e/sigma, the size of the terms that cancel
+    assert np.max(np.abs(fd_s - ds) / (np.abs(ds) + 1e-4 * np.abs(e) / sigma)) < 1e-7
+    # PW92 derivative on its own
+    rs = np.exp(rng.uniform(np.log(0.05), np.log(50.0), 100))
+    eps, deps = O.pw92_eps_c(rs)
+    assert np.max(np.abs(d5(lambda x: O.pw92_eps_c(x)[0], rs, 1e-4) - deps) / np.abs(deps)) < 1e-9
+    assert np.all(eps < 0) and np.all(deps > 0)
+    assert np.all(O.pbe_exc(np.array([0.0, 1e-31]), np.array([1.0, 1.0]))[1] == 0.0)     # density floor
+
+
+def test_pbe_potential_is_the_derivative_of_the_grid_energy():
+    """v_xc = d E_xc / d n_r for E_xc = dVol sum_r e(n_r, |D n|_r^2) with the SAME finite-difference gradient D: brute
+    force, one grid point at a time, orders 2 and 4 (sign of the divergence term, the factor 2 d e/d sigma, D^T = -D)."""
+    rng = np.random.default_rng(42)
+    shape, h = (6, 5, 8), 0.45
+    n3 = 0.05 + 0.04 * rng.random(shape)
+    for order in (2, 4):
+        v = O.vxc_pbe(n3.reshape(-1), shape, h, order).reshape(shape)
+
+        def E(arr):
+            return float(np.sum(O.exc_density_pbe(arr.reshape(-1), shape, h, order)))
+
+        for idx in ((0, 0, 0), (3, 4, 7), (5, 2, 1), (2, 0, 6)):
+            d = 1e-6
+            up, dn_ = n3.copy(), n3.copy()
+            up[idx] += d
+            dn_[idx] -= d
+            assert abs((E(up) - E(dn_)) / (2 * d) - v[idx]) < 2e-9 * abs(v[idx]) + 1e-10
+    # gradient stencils: exact on plane waves up to the symbol, error O(h^2) / O(h^4)
+    L = 7.0
+    for order, rate in ((2, 4.0), (4, 16.0)):
+        errs = []
+        for nn in (16, 32):
+            x = np.arange(nn) * L / nn
+            f = np.sin(2 * np.pi * x / L)[:, None, None] * np.ones((nn, 4, 4))
+            gx = O.grad_fd(f, L / nn, order)[0][:, 0, 0]
+            errs.append(np.max(np.abs(gx - 2 * np.pi / L * np.cos(2 * np.pi * x / L))))
+        assert 0.85 * rate < errs[0] / errs[1] < 1.15 * rate
+        assert np.max(np.abs(O.grad_fd(f, L / nn, order)[1])) < 1e-13
+
+
+def test_fourth_order_hartree_operator():
+    """FD_LAPL[4] (Eq. 2 with n = 2: exact for polynomials up to degree 5, a_i = -5/2, 4/3, -1/12).  (i) brute-force stencil
+    and plane-wave symbol; (ii) the multigrid-preconditioned cycle converges to the FFT solution of the 13-point operator
+    at the rate of the plain V-cycle; (iii) against the continuum Gaussian-charge potential (Ewald closed form with the
+    Madelung constant from tests/golden) the error is O(h^4) where the 7-point operator gives O(h^2)."""
+    rng = np.random.default_rng(43)
+    u = rng.standard_normal((7, 5, 6))
+    h = 0.4
+    ref = np.zeros_like(u)
+    w = {0: -2.5, 1: 4 / 3, 2: -1 / 12}
+    for i, j, k in itertools.product(range(7), range(5), range(6)):
+        s = 0.0
+        for d in range(-2, 3):
+            s += w[abs(d)] * (u[(i + d) % 7, j, k] + u[i, (j + d) % 5, k] + u[i, j, (k + d) % 6])
+        ref[i, j, k] = -s / h ** 2
+    assert np.allclose(O.apply_A_order(u, h, 4), ref, rtol=0, atol=1e-12)
+    x = np.arange(10) * 1.0
+    for p in range(6):                                   # exact second derivative of x^p, p <= 5, away from the wrap
+        f = (x ** p)[:, None, None] * np.ones((10, 5, 5))
+        d2 = -O.apply_A_order(f, 1.0, 4)[4, 0, 0]
+        assert abs(d2 - (p * (p - 1) * 4.0 ** (p - 2) if p >= 2 else 0.0)) < 1e-9
+    f = rng.standard_normal((12, 8, 10))
+    f -= f.mean()
+    sol = O.spectral_solve_order(f, h, 4)
+    assert np.allclose(O.apply_A_order(sol, h, 4), f, rtol=0, atol=1e-11) and abs(sol.mean()) < 1e-14
+    assert np.allclose(O.spectral_solve_order(f, h, 2), O.spectral_solve(f, h), rtol=0, atol=1e-13)
+    # (ii)
+    shape = (24, 24, 24)
+    drho = rng.standard_normal(shape).reshape(-1)
+    exact = O.spectral_solve_order((4 * np.pi * (drho - drho.mean())).reshape(shape), 0.35, 4).reshape(-1)
+    V, errs = np.zeros_like(drho), []
+    for _ in range(14):
+        V = O.hartree_mg(V, drho, shape, 0.35, 1, order=4)
+        errs.append(np.max(np.abs(V - exact)) / np.max(np.abs(exact)))
+    assert errs[-1] < 1e-7 and max(errs[i + 1] / errs[i] for i in range(2, 9)) < 0.45
+    # (iii)
+    with open(GOLD) as fh_:
+        mad = [float(l.split()[1]) for l in fh_ if l.startswith("madelung_sc")][0]
+    L, s = 8.4, 0.8
+    errs = {2: [], 4: []}
+    for n in (12, 24, 48):
+        hh = L / n
+        xx = (np.arange(n) - n // 2) * hh
+        r2 = xx[:, None, None] ** 2 + xx[None, :, None] ** 2 + xx[None, None, :] ** 2
+        rho = np.exp(-r2 / (2 * s * s)) / ((2 * np.pi) ** 1.5 * s ** 3)
+        ref0 = math.sqrt(2 / math.pi) / s - mad / L + 2 * math.pi * s * s / L ** 3
+        for order in (2, 4):
+            V = O.hartree_mg(np.zeros(n ** 3), rho.reshape(-1), (n, n, n), hh, 30, order=order)
+            errs[order].append(abs(V.reshape(n, n, n)[n // 2, n // 2, n // 2] - ref0))
+    assert 3.0 < errs[2][1] / errs[2][2] < 5.5                     # O(h^2)
+    assert 11.0 < errs[4][1] / errs[4][2] < 22.0                   # O(h^4)
+    assert errs[4][2] < 0.03 * errs[2][2]
+
+
+def test_energy_conservation_with_pbe_and_fourth_order_operators(tiny_inputs):
+    """The whole step with the GGA and the fourth-order operators: the potential is the exact grid derivative of the
+    energy, so the diagnostic is conserved after the kick exactly as with the LDA."""
+    o = _make(tiny_inputs, E0=(0.1, 0, 0), n_vcycles=10, xc_functional="pbe", fd_order=4)
+    o.step(2)
+    e1 = o.energy()
+    assert e1 - float(np.sum(o.eps * o.occ)) > 1e-7
+    es = []
+    for _ in range(10):
+        o.step(1)
+        es.append(o.energy())
+    assert np.max(np.abs(np.array(es) - e1)) < 2e-11
+    lda = _make(tiny_inputs, E0=(0.1, 0, 0), n_vcycles=10)
+    lda.step(12)
+    assert 1e-6 < np.max(np.abs(lda.dipole() - o.dipole())) < 1e-2          # a different functional, a nearby trajectory
