@@ -602,6 +602,49 @@ void launch_resid_restrict(const MgLevel& F, const MgLevel& C, const double* u, 
   mg_resid_restrict_kernel<<<(unsigned)(t.tx * t.ty * t.tz), MG_THREADS, resrest_smem_bytes(t.bx, t.by, t.bz), st>>>(a);
 }
 
+// ---- exact coarsest-level solve on global memory, whole-GPU version ---------------------------------------------
+// The paper's grids (N_x x 132 x 132) halve only twice: 1176 x 132 x 132 -> 294 x 33 x 33 = 320 k points,
+// far beyond what one CTA (or the 8-CTA cluster, whose index decode is exact below 2^16 points per plane pair) can
+// hold.  The separable solve u = (Qx x Qy x Qz) L^+ (Qx x Qy x Qz)^T f is six batched small dense transforms; here each
+// is one launch with one thread per output point (plain 64-bit index arithmetic), contraction along one axis.
+// axis pass: out[.., o_axis, ..] = sum_i M(i, o_axis) in[.., i, ..]; TRANS = false: M(i, o) = Q[i * n + o] (Q^T f);
+// TRANS = true: M(i, o) = Q[o * n + i] (Q g).  DIV: divide by lx + ly + lz afterwards (zero for the constant mode).
+template <int AXIS, bool TRANS, bool DIV>
+__global__ void __launch_bounds__(256)
+coarse_axis_kernel(GridDims gd, const double* __restrict__ Q, const double* __restrict__ in, double* __restrict__ out,
+                   const double* __restrict__ lx, const double* __restrict__ ly, const double* __restrict__ lz) {
+  const long long n = (long long)gd.nx * gd.ny * gd.nz;
+  const long long o = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (o >= n) return;
+  const long long nyz = (long long)gd.ny * gd.nz;
+  const int ix = (int)(o / nyz);
+  const int rem = (int)(o - ix * nyz);
+  const int iy = rem / gd.nz, iz = rem - iy * gd.nz;
+  const int na = AXIS == 0 ? gd.nx : (AXIS == 1 ? gd.ny : gd.nz);
+  const int oa = AXIS == 0 ? ix : (AXIS == 1 ? iy : iz);
+  const long long stride = AXIS == 0 ? nyz : (AXIS == 1 ? gd.nz : 1);
+  const double* p = in + (o - (long long)oa * stride);
+  double s = 0.0;
+  for (int i = 0; i < na; ++i) s += (TRANS ? Q[(long long)oa * na + i] : Q[(long long)i * na + oa]) * p[(long long)i * stride];
+  if (DIV) {
+    const double lam = lx[ix] + ly[iy] + lz[iz];
+    s = (ix == 0 && iy == 0 && iz == 0) ? 0.0 : s / lam;
+  }
+  out[o] = s;
+}
+
+// same six passes, in the same order and through the same scratch arrays (L.r, L.tmp), as cl_coarse_solve
+void launch_coarse_exact_global(const MgLevel& L, const MgSolveArgs& s, cudaStream_t st) {
+  const unsigned nb = (unsigned)((L.n + 255) / 256);
+  coarse_axis_kernel<0, false, false><<<nb, 256, 0, st>>>(L.gd, s.Qx, L.f, L.r, nullptr, nullptr, nullptr);
+  coarse_axis_kernel<1, false, false><<<nb, 256, 0, st>>>(L.gd, s.Qy, L.r, L.tmp, nullptr, nullptr, nullptr);
+  coarse_axis_kernel<2, false, true><<<nb, 256, 0, st>>>(L.gd, s.Qz, L.tmp, L.r, s.lx, s.ly, s.lz);
+  coarse_axis_kernel<2, true, false><<<nb, 256, 0, st>>>(L.gd, s.Qz, L.r, L.tmp, nullptr, nullptr, nullptr);
+  coarse_axis_kernel<1, true, false><<<nb, 256, 0, st>>>(L.gd, s.Qy, L.tmp, L.r, nullptr, nullptr, nullptr);
+  coarse_axis_kernel<0, true, false><<<nb, 256, 0, st>>>(L.gd, s.Qx, L.r, L.u, nullptr, nullptr, nullptr);
+}
+constexpr long long CLUSTER_MAX_POINTS = 32768;    // largest coarsest level the 8-CTA cluster kernel handles
+
 constexpr size_t COARSE_SMEM_MAX = 200 * 1024;     // bytes of level arrays the single-CTA kernel may hold
 
 bool fits_smem(const MgSolveArgs& s, int l0) {
@@ -609,7 +652,16 @@ bool fits_smem(const MgSolveArgs& s, int l0) {
 }
 
 // levels l0.. : single CTA on shared memory when they fit, else the 8-CTA cluster on global memory
-void launch_coarse(const MgSolveArgs& s, int l0, int ncycles, int zero_guess, int do_rhs, cudaStream_t st) {
+int launch_coarse(const MgSolveArgs& s, int l0, int ncycles, int zero_guess, int do_rhs, cudaStream_t st) {
+  if (!fits_smem(s, l0) && l0 == s.nlev - 1 && s.lv[l0].n > CLUSTER_MAX_POINTS) {
+    // a large coarsest level: the exact solve as six whole-GPU launches (it ignores the initial guess; cycles beyond the
+    // first would reproduce the same exact solution)
+    int launches = 6;
+    if (do_rhs) { launch_poisson_rhs(s.lv[l0].n, s.rho, s.rho0, s.sums, s.lv[l0].f, st); ++launches; }
+    if (ncycles > 0) launch_coarse_exact_global(s.lv[l0], s, st);
+    else launches -= 6;
+    return launches;
+  }
   ClusterArgs a{};
   a.nlev = s.nlev - l0; a.ncycles = ncycles; a.zero_guess = zero_guess;
   a.nu1 = s.nu1; a.nu2 = s.nu2; a.omega = s.omega;
@@ -627,6 +679,7 @@ void launch_coarse(const MgSolveArgs& s, int l0, int ncycles, int zero_guess, in
     cfg.attrs = at; cfg.numAttrs = 1;
     cudaLaunchKernelEx(&cfg, mg_coarse_kernel<false>, a);
   }
+  return 1;
 }
 
 struct BigCycle {
@@ -656,8 +709,7 @@ struct BigCycle {
     launch_resid_restrict(L, s.lv[l + 1], cur[l], st);
     ++launches;
     if (l + 1 == lc) {
-      launch_coarse(s, lc, 1, 1, 0, st);
-      ++launches;
+      launches += launch_coarse(s, lc, 1, 1, 0, st);
       cur[l + 1] = s.lv[l + 1].u;
     } else {
       vcycle(l + 1);
@@ -690,8 +742,7 @@ int launch_mg_solve(const MgSolveArgs& s, cudaStream_t st) {
   int lc = 0;
   while (lc < s.nlev - 1 && !fits_smem(s, lc)) ++lc;
   if (lc == 0) {           // the whole hierarchy is small: rhs + every cycle in one launch
-    launch_coarse(s, 0, s.n_vc, s.zero0, s.rhs_given ? 0 : 1, st);
-    return 1;
+    return launch_coarse(s, 0, s.n_vc, s.zero0, s.rhs_given ? 0 : 1, st);
   }
   if (!s.rhs_given) launch_poisson_rhs(s.lv[0].n, s.rho, s.rho0, s.sums, s.lv[0].f, st);
   BigCycle bc{s, lc, st};

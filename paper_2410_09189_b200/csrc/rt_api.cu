@@ -800,8 +800,8 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
       g = GridDims{g.nx / 2, g.ny / 2, g.nz / 2};
       hh *= 2.0;
     }
-    if (c->use_h && c->lv.back().n > 32768)
-      FAIL_CREATE(RT_EINVAL, "rt_create: coarsest multigrid level has more than 32768 points (grid dims need more factors of 2)");
+    // a coarsest level of any size is accepted: beyond 32768 points its exact separable solve runs as six whole-GPU
+    // launches (mg_kernels.cu launch_coarse_exact_global); the eigenvector tables below are then up to ~10^5 doubles
   }
 
   // plans

@@ -43,6 +43,10 @@ GRIDS = [
     ((54, 40, 32), "tile level above a coarsest level that needs the cluster kernel"),
     ((9, 5, 7), "no coarsening: exact solve only"),
     ((6, 6, 66), "thin grid: tile halo wraps onto the tile itself"),
+    ((88, 66, 66), "the paper's 132-factor grids (PAPER.md:L523): coarsest level 44x33x33 = 47,916 points > 32,768 -> "
+                   "exact solve as six whole-GPU launches"),
+    ((35, 33, 37), "42,735 points that cannot be coarsened at all: rhs + whole-GPU exact solve only"),
+    ((84, 132, 66), "three tile levels?  no: 42x66x33 stops at the odd 33 -> coarsest 91,476 points"),
 ]
 
 
@@ -89,3 +93,22 @@ def test_converges_to_spectral_solution_on_tile_path(B):
     exact = O.spectral_solve((4 * np.pi * (drho - drho.mean())).reshape(shape), h).reshape(-1)
     assert np.max(np.abs(vh - exact)) < 1e-8 * np.max(np.abs(exact))
     gpu.close()
+
+
+def test_whole_step_on_a_paper_shaped_grid(B):
+    """A 132-factor grid like the paper's N_x x 132 x 132 (round 1 refused it: coarsest level too large):
+    the full time step against the oracle, with the fourth-order Hartree operator as well."""
+    from paper_2410_09189_b200.workloads import strong_kick  # noqa: F401  (same kick convention)
+    shape, h = (44, 66, 66), 0.4                      # -> 22 x 33 x 33 = 23,958 (cluster) ; and the larger one below
+    for shape, order in (((88, 66, 66), 2), ((88, 66, 66), 4), ((44, 66, 66), 2)):
+        Phi, eps, occ = tiny_system(shape, h, norb=6, seed=9)
+        kw = dict(dt=0.2, E0=(0.1, 0.0, 0.0), n_hupdates=2, n_vcycles=3, fd_order=order)
+        gpu = B.RTTDDFT(shape, h, Phi, eps, occ, **kw)
+        cpu = O.RTOracle(shape, h, Phi, eps, occ, **kw)
+        for _ in range(3):
+            gpu.step(1)
+            cpu.step(1)
+            assert np.max(np.abs(gpu.dipole() - cpu.dipole())) < 1e-9 * np.max(np.abs(cpu.dipole()))
+        assert np.max(np.abs(gpu.density() - cpu.density())) < 1e-9 * np.max(np.abs(cpu.density()))
+        assert np.max(np.abs(gpu.vhartree() - cpu.VH)) < 1e-9 * np.max(np.abs(cpu.VH))
+        gpu.close()
