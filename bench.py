@@ -362,7 +362,7 @@ def main():
             dist.barrier()
         # a step of the two largest configs takes seconds: a quarter of the K steps (at least 3) is enough for the wall
         # clock, and keeps the driver's --steps 20 run of the 24k config inside its time limit
-        e2e_steps = args.steps if ms_total / args.steps < 1000.0 else max(3, args.steps // 4)
+        e2e_steps = args.steps if ms_total / args.steps < 1000.0 else min(args.steps, max(3, args.steps // 4))
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             E = w.E_of_t((step_no[0] + 1) * w.dt)

@@ -24,7 +24,7 @@ MUTATIONS = [
     ("delta_v: - vxc0", "dv = dv + self._vxc(rho) - self.vxc0", "dv = dv + self._vxc(rho)"),
     ("delta_v: + V_H", "dv = dv + self.VH", "dv = dv - self.VH"),
     ("set_field: stored value", "self.E_next = np.asarray(E, dtype=np.float64).copy()", "self.E_next = 0.5 * np.asarray(E, dtype=np.float64).copy()"),
-    ("__init__: H0 holds V(t_0)", "self.H0 = np.diag(self.eps) + project(", "self.H0 = np.diag(self.eps) + 0.0 * project("),
+    ("__init__: H0 holds V(t_0)", "self.H0 = self.Hks + project(", "self.H0 = self.Hks + 0.0 * project("),
     ("field_potential: axis order", "v = E[0] * x[:, None, None] + E[1] * y[None, :, None] + E[2] * z[None, None, :]", "v = E[0] * x[:, None, None] + E[2] * y[None, :, None] + E[1] * z[None, None, :]"),
     ("axis_coords: centring", "- 0.5 * (n - 1)) * h", "- 0.5 * n) * h"),
     ("project: dVol", "return dVol * ((Phi * v[None, :]) @ Phi.T)", "return ((Phi * v[None, :]) @ Phi.T)"),
