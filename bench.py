@@ -288,6 +288,7 @@ def main():
         phi = torch.from_numpy(Phi).to(f"cuda:{local}")
         ortho_err = float(np.max(np.abs(w.dvol * Phi @ Phi.T - np.eye(w.norb))))
     torch.cuda.synchronize()
+    torch.cuda.empty_cache()          # hand the generator's scratch back to the driver: the library allocates with cudaMalloc
     t_gen = time.perf_counter() - t_gen
 
     stream = torch.cuda.Stream(device=local)

@@ -402,6 +402,36 @@ struct GemmTmaArgs {
 
 __device__ __forceinline__ long long range_begin(long long total, int G, int j) { return total * j / G; }
 
+// Work of CTA `range` of G.  Whole waves of tiles are taken data-parallel in list order (tile = wave * G + range, all
+// stages): the CTAs that run together then work on CONSECUTIVE tiles of the list, which share their operand row panels
+// in L2 -- at N = 13,000 the operands are 1.35 GB each and only this sharing keeps the kernel off the HBM roof.  Only the
+// tail (the last full wave together with the partial one, G .. 2G-1 tiles; everything when there are fewer than G) is
+// cut stream-K style into G contiguous ranges of (tile, stage) units.
+struct GemmWork { int t, kt0, kt1, tl; bool tail; };
+struct GemmIter {
+  int G, range, nk, nfw, w, tail0;
+  long long total, u, u1;
+  __device__ GemmIter(int ntiles, int nk_, int G_, int range_) : G(G_), range(range_), nk(nk_), w(0) {
+    const int nw = ntiles / G, R = ntiles - nw * G;
+    nfw = (R == 0) ? nw : (nw > 0 ? nw - 1 : 0);
+    tail0 = nfw * G;
+    total = (long long)(ntiles - tail0) * nk;
+    u = range_begin(total, G, range);
+    u1 = range_begin(total, G, range + 1);
+  }
+  __device__ bool next(GemmWork& it) {
+    if (w < nfw) { it.t = w * G + range; it.kt0 = 0; it.kt1 = nk; it.tl = 0; it.tail = false; ++w; return true; }
+    if (u >= u1) return false;
+    it.tl = (int)(u / nk);
+    it.kt0 = (int)(u - (long long)it.tl * nk);
+    it.kt1 = (int)((u1 - u < nk - it.kt0) ? (it.kt0 + (u1 - u)) : nk);
+    it.t = tail0 + it.tl;
+    it.tail = true;
+    u += it.kt1 - it.kt0;
+    return true;
+  }
+};
+
 __global__ void __launch_bounds__(NTHREADS, 1)
 gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmB0,
                     const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmB1,
@@ -420,8 +450,6 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
   const int N = ga.N, ldn = ga.ldn;
   const int nk1 = (N + BK - 1) / BK;
   const int nk = ga.nterms * nk1;
-  const long long total = (long long)ga.ntiles * nk;
-  const long long u0 = range_begin(total, G, range), u1 = range_begin(total, G, range + 1);
 
   if (warp >= NCONS) {
     regs_producer();
@@ -429,10 +457,11 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
       tma_prefetch_desc(&tmA0);
       tma_prefetch_desc(&tmB0);
       long long it = 0;
-      for (long long u = u0; u < u1;) {
-        const int t = (int)(u / nk), kt0 = (int)(u - (long long)t * nk);
-        const int kt1 = (int)((u1 - u < nk - kt0) ? (kt0 + (u1 - u)) : nk);
-        const int2 tt = ga.tiles[t];
+      GemmIter iter(ga.ntiles, nk, G, range);
+      GemmWork wk;
+      while (iter.next(wk)) {
+        const int kt0 = wk.kt0, kt1 = wk.kt1;
+        const int2 tt = ga.tiles[wk.t];
         const int i0 = tt.x * TILE, j0 = tt.y * TILE;
         for (int kt = kt0; kt < kt1; ++kt, ++it) {
           const int slot = (int)(it % ST);
@@ -445,7 +474,6 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
           tma_load_2d(sA, second ? &tmA1 : &tmA0, k0, i0, full);
           tma_load_2d(sA + TILE_D, second ? &tmB1 : &tmB0, k0, j0, full);
         }
-        u += kt1 - kt0;
       }
     }
   } else {
@@ -458,10 +486,11 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
     const double fin = (ga.nterms == 2 && ratio != 1.0) ? ga.alpha0 * ratio : ga.alpha0;
     const double msign = (double)ga.sym;
     long long it = 0;
-    for (long long u = u0; u < u1;) {
-      const int t = (int)(u / nk), kt0 = (int)(u - (long long)t * nk);
-      const int kt1 = (int)((u1 - u < nk - kt0) ? (kt0 + (u1 - u)) : nk);
-      const int2 tt = ga.tiles[t];
+    GemmIter iter(ga.ntiles, nk, G, range);
+    GemmWork wk;
+    while (iter.next(wk)) {
+      const int kt0 = wk.kt0, kt1 = wk.kt1;
+      const int2 tt = ga.tiles[wk.t];
       const int i0 = tt.x * TILE, j0 = tt.y * TILE;
       double acc[FA][FB][2];
 #pragma unroll
@@ -489,7 +518,6 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
 #pragma unroll
           for (int b = 0; b < FB; ++b) { acc[a][b][0] *= inv; acc[a][b][1] *= inv; }
       }
-      u += kt1 - kt0;
 
       if (kt0 > 0) {
         // ---- tail of a tile whose head lives in an earlier range: park the partial sums, raise the flag ----
@@ -510,8 +538,8 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
       }
       if (kt1 < nk) {
         // ---- head of a tile that continues in the following ranges: add their partial sums in range order ----
-        const long long tile_end = (long long)(t + 1) * nk;
-        for (int p = range + 1; p < G && range_begin(total, G, p) < tile_end; ++p) {
+        const long long tile_end = (long long)(wk.tl + 1) * nk;
+        for (int p = range + 1; p < G && range_begin(iter.total, G, p) < tile_end; ++p) {
           if (ctid == 0) {
             const long long t0 = clock64();
             while (atomicAdd(&ga.sync[2 + p], 0) == 0) {

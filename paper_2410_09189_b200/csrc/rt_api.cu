@@ -826,7 +826,21 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     long long smax = (Ng + kmin - 1) / kmin;
     if (smax > 4 * sms) smax = 4 * sms;
     const double slab_bytes = (double)N * ldn * 8;
-    while (smax > 1 && smax * slab_bytes > 2.0e9) --smax;          // workspace cap
+    // workspace cap: 2 GB, or up to 6 GB when the device has room after everything else (24k: S = 3 slabs of 1.35 GB
+    // turn the half-empty 36th wave of 5,253 one-shot tiles into balanced waves, ~1 % of a 5.5 s kernel)
+    double ws_cap = 2.0e9;
+    {
+      size_t freeb = 0, totalb = 0;
+      if (cudaMemGetInfo(&freeb, &totalb) == cudaSuccess) {
+        const double other = 16.0 * (double)c->nn_alloc * 8 + ((double)ntile + 1) / 2 * Ng * 8 + 14.0 * NgF * 8 +
+                             ((cfg->flags & RT_PHI_DEVICE) ? 0.0 : (double)N * Ng * 8);
+        const double room = 0.5 * ((double)freeb - other);
+        if (room > ws_cap) ws_cap = room < 6.0e9 ? room : 6.0e9;
+      } else {
+        cudaGetLastError();
+      }
+    }
+    while (smax > 1 && smax * slab_bytes > ws_cap) --smax;
     auto chunk_of = [&](long long S_) { long long kc = (Ng + S_ - 1) / S_; return (kc + 15) / 16 * 16; };
     auto makespan = [&](const long long (&n)[3], const double (&cst)[3]) {
       std::priority_queue<double, std::vector<double>, std::greater<double>> q;
