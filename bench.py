@@ -395,9 +395,14 @@ def main():
         Ng = slab[1] * w.shape[1] * w.shape[2]
     alg = {"Hupdate": ("tensor", N * (N + 1.0) * Ng, "a1 projection project_kernel: N(N+1)Ng flop per launch (symmetric output)"),
            "Rho": ("tensor", 1.0 * N * N * Ng, "a5 density density_kernel: N^2 Ng flop per launch (triangular fold)"),
-           "ELDYN": ("tensor", ((info["exp_order"] // 2 + 1) + 12.0) * N ** 3,
-                     "a3+a4 gemm_abt_tma_kernel: (q+1) symmetric-output series GEMMs (N^3 each) + U P U^dagger "
-                     "(2 full dual GEMMs 8N^3 + Hermitian output 4N^3)"),
+           "ELDYN": (("tensor", (2.0 * (info["exp_order"] // 2 + 1) + 16.0) * N ** 3 / world,
+                      "a3+a4 row-sharded: this rank's row block of (q+1) series GEMMs (2N^3 each, no symmetric saving) "
+                      "+ U P U^dagger (16N^3), divided by the number of ranks")
+                     if slabs and world > 1 and w.norb >= 2048 else
+                     ("tensor", ((info["exp_order"] // 2 + 1) + 12.0 - 2.0 * (w.n_hupdates - 1) / w.n_hupdates) * N ** 3,
+                      "a3+a4 gemm_abt_tma_kernel: (q+1) symmetric-output series GEMMs (N^3 each) + U P U^dagger "
+                      "(2 full dual GEMMs 8N^3 + Hermitian output: Re P1 2N^3 on every update, Im P1 2N^3 on the last "
+                      "update of a step only); mean over the m updates")),
            "Vh": ("hbm", 57.0 * w.ngrid * w.n_vcycles, "a7 V-cycles: 57 B/pt/cycle (SURVEY 8d fused-ideal, coarse levels "
                   "included); L2-resident and launch-latency-bound in practice"),
            "XC": ("hbm", 32.0 * w.ngrid, "a8 delta_v_kernel: 32 B/pt")}
@@ -437,7 +442,7 @@ def main():
 
     # CPU baseline: the oracle as it stands on the host cores, bounded sample
     cpu = None
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:          # the oracle is timed on rank 0 of a one-GPU run only
         cores = threads_used()
         if big:
             pts = slab_points(w)

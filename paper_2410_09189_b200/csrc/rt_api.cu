@@ -60,8 +60,9 @@ struct rt_ctx {
   double *Hm1 = nullptr, *H0 = nullptr, *H1 = nullptr, *X = nullptr, *Ya = nullptr, *Yb = nullptr, *Yc = nullptr,
          *Cm = nullptr, *Sc = nullptr, *Sm = nullptr, *P0r = nullptr, *P0i = nullptr, *P1r = nullptr, *P1i = nullptr,
          *W = nullptr;
-  int2* d_tiles = nullptr;        // upper tiles (ti <= tj), class-ordered for the projection; also the sym GEMMs' list
-  int2* d_tiles_full = nullptr;   // all ntile x ntile tiles, row-major (plain GEMMs; a row block is a contiguous piece)
+  int2* d_tiles = nullptr;        // upper tiles (ti <= tj), class-ordered and 2-D blocked for the projection
+  int2* d_tiles_full = nullptr;   // all ntile x ntile tiles, row-major (a row block of the sharded propagator is a contiguous piece)
+  int2* d_tiles_sym = nullptr;    // upper tiles (ti <= tj) row-major: the symmetric-output N x N GEMMs (stream-K walks them in order)
   int ntile = 0;
   double* gemm_ws = nullptr;      // stream-K fix-up workspace and flags of the TMA N x N GEMM (gemm_tma.cu)
   int* gemm_sync = nullptr;
@@ -81,7 +82,7 @@ struct rt_ctx {
   double *f4 = nullptr;           // right-hand side of the fourth-order Hartree solve
   MgLevel dl0{};                  // level-0 arrays of its correction hierarchy
   int slab_more = 0;              // decision of the last RT_SLAB_CHECK: another Hamiltonian update is needed
-  std::map<int, cudaGraphExec_t> phase_exec;      // slab phases captured as CUDA graphs, key = 2 * phase + (it == 0)
+  std::map<int, cudaGraphExec_t> phase_exec;      // slab phases captured as CUDA graphs, key = (phase, it == 0, last update)
   std::map<int, int64_t> phase_launches;
   std::vector<cudaGraph_t> phase_graphs;
   DensSeg* d_segs = nullptr;
@@ -303,7 +304,7 @@ void enqueue_gemm(rt_ctx* c, int sym, const double* A0, const double* B0, double
   if (c->use_tma && c->N > GEMM_SMALL_N) {
     const CUtensorMap& mA0 = nn_map(c, A0);
     const CUtensorMap& mB0 = nn_map(c, B0);
-    const int2* tiles = c->d_tiles;
+    const int2* tiles = c->d_tiles_sym;
     int ntiles = c->pp.T;
     if (shard) { sym = 0; tiles = c->d_tiles_full + (size_t)(c->row_beg / TILE) * c->ntile; ntiles = ((c->row_end - c->row_beg + TILE - 1) / TILE) * c->ntile; }
     else if (!sym) { tiles = c->d_tiles_full; ntiles = c->ntile * c->ntile; }
@@ -336,11 +337,13 @@ void enqueue_expm(rt_ctx* c) {
 // P1 = U P0 U^dagger (Eq. 15), U = C - iS, P0 = A + iB (A symmetric, B antisymmetric).
 //   Yr = C A + S B, Yi = C B - S A ; P1r = Yr C - Yi S, P1i = Yr S + Yi C.
 // gemm_abt contracts against B^T: a symmetric right factor is used as is, the antisymmetric one flips the sign.
-void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
+// need_im = false: Im P1 is not formed.  Only the LAST Hamiltonian update of a step hands its P1 on (line 28); the earlier
+// ones are read by the density alone, which takes Re P1 (Eq. 27: Im P is antisymmetric and drops out for real orbitals).
+void enqueue_upu(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi, bool need_im = true) {
   enqueue_gemm(c, 0, c->Cm, Ar, 1.0, c->Sm, Ai, -1.0, c->Yb);
   enqueue_gemm(c, 0, c->Cm, Ai, -1.0, c->Sm, Ar, -1.0, c->Yc);
   enqueue_gemm(c, 1, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, Or);      // P1 Hermitian: Re symmetric,
-  enqueue_gemm(c, -1, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, Oi);      // Im antisymmetric
+  if (need_im) enqueue_gemm(c, -1, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, Oi);      // Im antisymmetric
 }
 
 // ---- the same propagation with the N^3 work sharded over ranks by row blocks ("once N exceeds a few
@@ -381,6 +384,7 @@ void enqueue_shard_B(rt_ctx* c) {
 void enqueue_shard_C(rt_ctx* c) {
   stage_begin(c, RT_STAGE_ELDYN);
   enqueue_gemm(c, 0, c->Yb, c->Cm, 1.0, c->Yc, c->Sm, -1.0, c->P1r, nullptr, 0, nullptr, 0, nullptr, true);
+  // (Im P1 is formed and gathered on every update here: the caller's gather list is fixed per phase)
   enqueue_gemm(c, 0, c->Yb, c->Sm, 1.0, c->Yc, c->Cm, 1.0, c->P1i, nullptr, 0, nullptr, 0, nullptr, true);
   stage_end(c);
 }
@@ -471,10 +475,10 @@ void enqueue_commutator_general(rt_ctx* c, const double* Ar, const double* Ai, d
   }
 }
 
-void enqueue_propagate(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi) {
+void enqueue_propagate(rt_ctx* c, const double* Ar, const double* Ai, double* Or, double* Oi, bool need_im = true) {
   if (c->general) enqueue_commutator_general(c, Ar, Ai, Or, Oi);
   else if (c->prop == RT_PROP_COMMUTATOR) enqueue_commutator(c, Ar, Ai, Or, Oi);
-  else { enqueue_expm(c); enqueue_upu(c, Ar, Ai, Or, Oi); }
+  else { enqueue_expm(c); enqueue_upu(c, Ar, Ai, Or, Oi, need_im); }
 }
 
 void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double* rho0) {
@@ -538,7 +542,9 @@ void enqueue_update_propagate(rt_ctx* c, int it) {
   if (c->d_cs) cudaMemsetAsync(c->d_cs, 0, sizeof(ConvState), c->st);                          // lines 12, 16
   launch_hbar(c->N, c->ldn, c->Hm1, c->H0, c->H1, c->X, c->dt, c->sigma, it == 0, c->st, c->Smat);   // lines 11, 14
   c->launches += 1;
-  enqueue_propagate(c, c->P0r, c->P0i, c->P1r, c->P1i);                                        // Eq. 15 / Eq. 39
+  // fixed-count step: only the last update's Im P1 is ever read (by line 28); the dynamic loop cannot know which is last
+  const bool need_im = c->dynamic || it >= c->m - 1;
+  enqueue_propagate(c, c->P0r, c->P0i, c->P1r, c->P1i, need_im);                               // Eq. 15 / Eq. 39
   stage_end(c);
   enqueue_density_stage(c);
 }
@@ -891,9 +897,20 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     const int nsplit = 1;
     build_density_types(N, ntile, nsplit, c->segs);
     d.ntypes = (int)(c->segs.size() / 2);
-    int gr = (sms + d.ntypes - 1) / d.ntypes;
-    if (gr > d.nrt) gr = (int)d.nrt;
-    d.group_r = gr < 1 ? 1 : gr;
+    // supertile shape group_t x group_r (~ one item per SM): a supertile reads its group_t fold panels and its group_r Phi
+    // panels once from DRAM, so the launch moves about  |Phi| * ntypes/group_t + |P fold| * nrt/group_r  bytes
+    {
+      const double phi_b = (double)N * Ng * 8, pf_b = 0.5 * (double)N * ldn * 8;
+      double best_cost = 1e300;
+      d.group_t = 1; d.group_r = 1;
+      for (int gt = 1; gt <= d.ntypes && gt <= sms; ++gt) {
+        long long gr = sms / gt;
+        if (gr > d.nrt) gr = d.nrt;
+        if (gr < 1) gr = 1;
+        const double cost = phi_b * std::ceil((double)d.ntypes / gt) + pf_b * std::ceil((double)d.nrt / (double)gr);
+        if (cost < best_cost) { best_cost = cost; d.group_t = gt; d.group_r = (int)gr; }
+      }
+    }
   }
 
   // memory check, then allocations
@@ -989,9 +1006,16 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
   {
     std::vector<int2> tiles;
     // full off-diagonal tiles, then the narrow last column (if any), then the diagonal (ProjectPlan)
+    // The full tiles in 2-D blocks of bs x bs tiles (bs^2 ~ number of SMs): the CTAs of a wave then share bs row panels and
+    // bs column panels of Phi in L2 instead of streaming one private
+    // column panel each -- at N = 13,000 a row-major list made every one of the 5,151 tiles read its own 1.15 GB panel.
     const int tj_end = c->pp.Tn > 0 ? ntile - 1 : ntile;
-    for (int ti = 0; ti < ntile; ++ti)
-      for (int tj = ti + 1; tj < tj_end; ++tj) tiles.push_back(make_int2(ti, tj));
+    int bs = (int)std::floor(std::sqrt((double)c->sms));
+    if (bs < 1) bs = 1;
+    for (int bi = 0; bi < ntile; bi += bs)
+      for (int bj = bi; bj < tj_end; bj += bs)
+        for (int ti = bi; ti < std::min(bi + bs, ntile); ++ti)
+          for (int tj = std::max(bj, ti + 1); tj < std::min(bj + bs, tj_end); ++tj) tiles.push_back(make_int2(ti, tj));
     if (c->pp.Tn > 0)
       for (int ti = 0; ti < ntile - 1; ++ti) tiles.push_back(make_int2(ti, ntile - 1));
     for (int ti = 0; ti < ntile; ++ti) tiles.push_back(make_int2(ti, ti));
@@ -1002,6 +1026,11 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
       for (int tj = 0; tj < ntile; ++tj) full.push_back(make_int2(ti, tj));
     ALLOC(c->d_tiles_full, full.size());
     CKC(cudaMemcpyAsync(c->d_tiles_full, full.data(), full.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
+    std::vector<int2> symrm;
+    for (int ti = 0; ti < ntile; ++ti)
+      for (int tj = ti; tj < ntile; ++tj) symrm.push_back(make_int2(ti, tj));
+    ALLOC(c->d_tiles_sym, symrm.size());
+    CKC(cudaMemcpyAsync(c->d_tiles_sym, symrm.data(), symrm.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
     if (c->use_tma && N > GEMM_SMALL_N) {
       ALLOC(c->gemm_ws, gemm_tma_ws_doubles(c->sms));
       ALLOC(c->gemm_sync, gemm_tma_sync_ints(c->sms));
@@ -1664,7 +1693,8 @@ int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
     enqueue: {
       // The phases are fixed launch sequences: each (phase, first-update?) pair is captured once into a CUDA graph on a
       // private stream and replayed afterwards (one launch instead of ~50 at the small configs).
-      const int key = 2 * phase + (it == 0 ? 1 : 0);
+      const bool last = c->dynamic || it >= c->m - 1;          // the last update also forms Im P1 (enqueue_upu)
+      const int key = 4 * phase + 2 * (it == 0 ? 1 : 0) + (last ? 1 : 0);
       if (c->use_graph && !c->timing) {
         auto ex = c->phase_exec.find(key);
         if (ex == c->phase_exec.end()) {

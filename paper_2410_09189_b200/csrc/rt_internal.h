@@ -64,7 +64,8 @@ struct DensityPlan {
   int npairs;            // ceil(ntile / 2): CTA handles j-tiles (p, ntile-1-p)
   long long nrt;         // r tiles = ceil(Ng / TILE)
   int ldn;
-  int group_r;           // raster: r-tiles per supertile column
+  int group_r;           // raster: r-tiles per supertile
+  int group_t;           // TMA kernel: work types per supertile (group_t * group_r ~ number of SMs)
   int ntypes;            // TMA kernel: work types per r-tile (each owns one partial row); >= npairs
 };
 // TMA density kernel: one k-segment of j-tile jt: stages s0, s0 + dir, ... (ns of them), stage s covering the

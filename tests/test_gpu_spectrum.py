@@ -97,3 +97,26 @@ def test_three_kicks_together_match_three_oracle_runs(B):
     # the induced dipole is ~1e-3 of the total, so 1e-9 on mu is ~1e-6 on the transform of (mu - mu(0))
     assert np.max(np.abs(S - S_ref)) < 1e-5 * np.max(np.abs(S_ref))
     trio.close()
+
+
+def test_three_kicks_share_the_gpu_with_the_stream_k_gemm(B):
+    """N = 1,625 runs the stream-K N x N GEMM, whose CTAs wait on one another through flags.  Three handles on three
+    streams keep all of them in flight at once: the ticket-ordered ranges must make that safe (no deadlock) and the
+    results must be bit-identical to the same three runs done one after the other."""
+    import torch
+    from paper_2410_09189_b200.spectrum import KickTriple
+    w = WORKLOADS["24k_twin"]
+    Phi, eps, occ = make_inputs_numpy(w)
+    phi_d = torch.from_numpy(Phi).cuda()
+    kick, nsteps = 0.02, 3
+    trio = KickTriple(w.shape, w.h, phi_d, eps, occ, w.dt, kick=kick, n_vcycles=w.n_vcycles, max_steps=nsteps)
+    trio.step(nsteps, chunk=1)
+    mu = trio.dipoles()
+    trio.close()
+    for q in range(3):
+        one = B.RTTDDFT(w.shape, w.h, phi_d, eps, occ, w.dt, E0=tuple(kick * np.eye(3)[q]), n_vcycles=w.n_vcycles,
+                        history=nsteps + 1)
+        one.step(nsteps)
+        assert np.array_equal(one.dipole_series(0, nsteps + 1)[:, q], mu[q])
+        one.close()
+    assert np.max(np.abs(mu - mu[:, :1])) > 1e-9
