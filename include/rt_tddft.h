@@ -111,6 +111,11 @@ typedef struct {
                                Laplacian as the operator V_H solves -- each of the n_vcycles cycles is then
                                r = f - A4 u, d = one 7-point V-cycle on (0, r), u += d (multigrid as the preconditioner,
                                L77; DESIGN R17) -- and 4-point gradients                                              */
+  /* -- several handles side by side on one GPU (the three delta-kick polarisations of L453 on three streams) ------- */
+  int32_t  sm_limit;        /* > 0: size the split-K plans and the persistent grids of the DMMA kernels (a1, a5, a3/a4) for
+                               at most this many SMs, so that the kernels of handles on other streams fit beside them
+                               instead of queueing behind a launch that fills the GPU.  Results do not depend on it
+                               beyond the summation order of the split-K partial sums.  0 = all SMs                  */
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,
@@ -178,7 +183,8 @@ int rt_get_time(rt_handle h, double* t);
 /* Integrals of the current density, HOST double[2]: { dVol sum rho , dVol sum (rho - rho0) }.  Synchronises. */
 int rt_get_charge(rt_handle h, double q[2]);
 /* info[0] = exp_order K actually used, info[1] = number of multigrid levels, info[2..4] = coarsest nx,ny,nz,
- * info[5] = 1 if steps replay a CUDA graph (+2 if the TMA-fed DMMA kernels are in use), info[6] = kernels launched
+ * info[5] = 1 if steps (or slab phases) replay a CUDA graph, +2 if the TMA-fed DMMA kernels are in use, +4 if a slab
+ * phase capture was ever invalidated from outside (that phase was then enqueued directly), info[6] = kernels launched
  * per step, info[7] = split-K of the projection.  HOST int32[8]. */
 int rt_get_info(rt_handle h, int32_t info[8]);
 /* Total number of this library's kernel launches enqueued through the handle so far (graph replays count the

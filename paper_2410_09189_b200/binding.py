@@ -56,6 +56,7 @@ class rt_config(C.Structure):
         ("history", C.c_int32),
         ("prop_shards", C.c_int32), ("prop_shard", C.c_int32),
         ("magnus_order", C.c_int32), ("xc_functional", C.c_int32), ("fd_order", C.c_int32),
+        ("sm_limit", C.c_int32),
     ]
 
 
@@ -212,7 +213,8 @@ def rt_get_info(h) -> dict:
     a = np.zeros(8, dtype=np.int32)
     _check(h, _lib.rt_get_info(h, a.ctypes.data))
     return {"exp_order": int(a[0]), "mg_levels": int(a[1]), "coarsest": (int(a[2]), int(a[3]), int(a[4])),
-            "graph": bool(a[5] & 1), "tma": bool(a[5] & 2), "launches_per_step": int(a[6]),
+            "graph": bool(a[5] & 1), "tma": bool(a[5] & 2), "capture_retried": bool(a[5] & 4),
+            "launches_per_step": int(a[6]),
             "project_split_k": int(a[7])}
 
 
@@ -376,7 +378,7 @@ class RTTDDFT:
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
                  nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
                  device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0,
-                 slab=None, history=0, prop_shard=None, magnus=1, xc_functional="lda", fd_order=2, Hks=None,
+                 slab=None, history=0, prop_shard=None, magnus=1, xc_functional="lda", fd_order=2, sm_limit=0, Hks=None,
                  P0=None, nonorthogonal=False):
         """``slab = (x0, nx_local)``: the handle owns those x-planes and ``phi`` is [norb][nx_local*ny*nz]
         (rt_slab_* entry points; see slab.py).  ``prop_shard = (rank, nranks)``: row-sharded N x N propagator.
@@ -389,6 +391,7 @@ class RTTDDFT:
         cfg.magnus_order = int(magnus)
         cfg.xc_functional = {"lda": RT_XC_LDA_PZ81, "pbe": RT_XC_PBE}[xc_functional]
         cfg.fd_order = int(fd_order)
+        cfg.sm_limit = int(sm_limit)
         cfg.propagator = {"taylor": RT_PROP_TAYLOR, "commutator": RT_PROP_COMMUTATOR}[propagator]
         cfg.max_order, cfg.dP_thrs, cfg.H_thrs, cfg.max_hupdates = int(max_order), float(dP_thrs), float(H_thrs), int(max_hupdates)
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)

@@ -407,6 +407,7 @@ struct GemmTmaArgs {
   double alpha0, alpha1;
   double* D; double* Z1; double beta1; double* Z2; double beta2;
   const int* skip;         // non-zero -> no-op (orders past convergence of the commutator series)
+  int zmode;               // how Z1 / Z2 of a symmetric-output launch are maintained below the diagonal (see the epilogue)
   double* ws;              // [G][TILE*TILE] partial accumulators of the tail items, indexed by range
   int* sync;               // [0] = ticket counter, [1] = finished-CTA counter, [2 + p] = flag of range p (0 = empty)
 };
@@ -571,29 +572,66 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
       }
 
       // ---- epilogue of a complete tile ----
+      // The read-modify-writes of Z1 / Z2 are done in two phases per batch of 2 x 2 fragments -- all loads, then all
+      // stores: D, Z1 and Z2 are plain pointers that may alias as far as the compiler knows, so interleaved `Z[o] += ...`
+      // statements serialise into one L2 round trip each (measured at N = 2400: 0.68 ms against 0.48 ms for the same
+      // product without Z, DMMA pipe 70 % against 91 %).  zmode (symmetric outputs only): 0 = Z is accumulated on both
+      // sides of the diagonal; 1 = on the upper triangle only (the lower one is not maintained); 2 = upper triangle, and
+      // the finished value is stored to its mirror image too (the last accumulation of a chain started with zmode 1).
       const bool diag = ga.sym && i0 == j0;
+      const bool hasZ1 = ga.Z1 != nullptr, hasZ2 = ga.Z2 != nullptr;
+      const bool zrmw_mirror = ga.sym && ga.zmode == 0, zst_mirror = ga.sym && ga.zmode != 1;
 #pragma unroll
       for (int a = 0; a < FA; ++a) {
         const int row = i0 + wrow + 8 * a + pg;
         if (row < N) {
 #pragma unroll
-          for (int b = 0; b < FB; ++b) {
+          for (int bb = 0; bb < FB; bb += 2) {
+            double z1[2][2], z2[2][2], z1m[2][2], z2m[2][2];
+            if (hasZ1 || hasZ2) {
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-              const int col = j0 + wcol + 8 * b + c + 4 * e;
-              if (col < N && (!diag || col >= row)) {
-                const long long o = (long long)row * ldn + col;
-                double d = fin * acc[a][b][e];
-                if (ga.sym < 0 && row == col) d = 0.0;
-                if (ga.D) ga.D[o] = d;
-                if (ga.Z1) ga.Z1[o] += ga.beta1 * d;
-                if (ga.Z2) ga.Z2[o] += ga.beta2 * d;
-                if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
-                  const long long om = (long long)col * ldn + row;
-                  const double dm = msign * d;
-                  if (ga.D) ga.D[om] = dm;
-                  if (ga.Z1) ga.Z1[om] += ga.beta1 * dm;
-                  if (ga.Z2) ga.Z2[om] += ga.beta2 * dm;
+              for (int b = 0; b < 2; ++b)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                  const int col = j0 + wcol + 8 * (bb + b) + c + 4 * e;
+                  z1[b][e] = z2[b][e] = z1m[b][e] = z2m[b][e] = 0.0;
+                  if (col < N && (!diag || col >= row)) {
+                    const long long o = (long long)row * ldn + col;
+                    if (hasZ1) z1[b][e] = ga.Z1[o];
+                    if (hasZ2) z2[b][e] = ga.Z2[o];
+                    if (zrmw_mirror && row != col) {
+                      const long long om = (long long)col * ldn + row;
+                      if (hasZ1) z1m[b][e] = ga.Z1[om];
+                      if (hasZ2) z2m[b][e] = ga.Z2[om];
+                    }
+                  }
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+#pragma unroll
+              for (int e = 0; e < 2; ++e) {
+                const int col = j0 + wcol + 8 * (bb + b) + c + 4 * e;
+                if (col < N && (!diag || col >= row)) {
+                  const long long o = (long long)row * ldn + col;
+                  double d = fin * acc[a][bb + b][e];
+                  if (ga.sym < 0 && row == col) d = 0.0;
+                  const double v1 = z1[b][e] + ga.beta1 * d, v2 = z2[b][e] + ga.beta2 * d;
+                  if (ga.D) ga.D[o] = d;
+                  if (hasZ1) ga.Z1[o] = v1;
+                  if (hasZ2) ga.Z2[o] = v2;
+                  if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
+                    const long long om = (long long)col * ldn + row;
+                    const double dm = msign * d;
+                    if (ga.D) ga.D[om] = dm;
+                    if (zrmw_mirror) {
+                      if (hasZ1) ga.Z1[om] = z1m[b][e] + ga.beta1 * dm;
+                      if (hasZ2) ga.Z2[om] = z2m[b][e] + ga.beta2 * dm;
+                    } else if (zst_mirror) {             // zmode 2: Z is symmetric (sym = +1 chains only)
+                      if (hasZ1) ga.Z1[om] = v1;
+                      if (hasZ2) ga.Z2[om] = v2;
+                    }
+                  }
                 }
               }
             }
@@ -626,7 +664,7 @@ void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUten
                          cudaStream_t st) {
   if (ntiles <= 0) return;
   GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, sym, tiles, ntiles, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2,
-                g.skip, ws, sync};
+                g.skip, g.zmode, ws, sync};
   const int grid = gemm_tma_grid(ntiles, g.N, a.nterms, sms);
   gemm_abt_tma_kernel<<<grid, NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
 }

@@ -84,6 +84,8 @@ struct rt_ctx {
   int slab_more = 0;              // decision of the last RT_SLAB_CHECK: another Hamiltonian update is needed
   std::map<int, cudaGraphExec_t> phase_exec;      // slab phases captured as CUDA graphs, key = (phase, it == 0, last update)
   std::map<int, int64_t> phase_launches;
+  std::map<int, int> phase_capture_failures;      // captures of a phase that were invalidated (the phase then ran directly)
+  int capture_failures = 0;
   std::vector<cudaGraph_t> phase_graphs;
   DensSeg* d_segs = nullptr;
   std::vector<DensSeg> segs;
@@ -296,10 +298,10 @@ void stage_end(rt_ctx* c) {
 // plain product, because the mirror image of a row block belongs to other ranks.
 void enqueue_gemm(rt_ctx* c, int sym, const double* A0, const double* B0, double a0, const double* A1,
                   const double* B1, double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr,
-                  double b2 = 0, const int* skip = nullptr, bool rows = false) {
+                  double b2 = 0, const int* skip = nullptr, bool rows = false, int zmode = 0) {
   const bool shard = rows && c->nshard > 1;
   GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2, skip, shard ? c->row_beg : 0,
-             shard ? c->row_end : c->N};
+             shard ? c->row_end : c->N, zmode};
   if (g.row_end <= g.row_beg) return;                       // this rank owns no rows (more ranks than tile rows)
   if (c->use_tma && c->N > GEMM_SMALL_N) {
     const CUtensorMap& mA0 = nn_map(c, A0);
@@ -328,7 +330,8 @@ void enqueue_expm(rt_ctx* c) {
     ck = -ck / ((2.0 * k - 1.0) * (2.0 * k));
     sk = -sk / ((2.0 * k) * (2.0 * k + 1.0));
     double* cur = (k < c->q) ? ((k & 1) ? c->Yc : c->Yb) : nullptr;
-    enqueue_gemm(c, 1, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk);
+    // C and Sc are symmetric: the chain accumulates their upper triangles, the last product stores the mirror image
+    enqueue_gemm(c, 1, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk, nullptr, false, k < c->q ? 1 : 2);
     prev = cur;
   }
   enqueue_gemm(c, 1, c->X, c->Sc, 1.0, nullptr, nullptr, 0, c->Sm);
@@ -680,6 +683,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     return fail(c, RT_EINVAL, "rt_create: unknown xc_functional");
   if (cfg->fd_order != 0 && cfg->fd_order != 2 && cfg->fd_order != 4)
     return fail(c, RT_EINVAL, "rt_create: fd_order must be 0, 2 or 4");
+  if (cfg->sm_limit < 0) return fail(c, RT_EINVAL, "rt_create: sm_limit < 0");
   if (want_nonorth && !(Hks_in && P0re_in))
     return fail(c, RT_EINVAL, "rt_create: RT_NONORTHOGONAL needs the ground state as matrices (rt_create_general)");
   if (cfg->nx < 2 || cfg->ny < 2 || cfg->nz < 2) return fail(c, RT_EINVAL, "rt_create: grid dims must be >= 2");
@@ -820,7 +824,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     // full CTA costs kchunk/16, a narrow one 0.78 and a diagonal one 0.65 of that per stage (TMA kernel; measured), plus
     // a fixed prologue/epilogue per CTA and a term per split for the second-stage reduction.  (Wave quantisation was
     // 14 % of the first nano profile at S = 2.)
-    const int sms = prop.multiProcessorCount;
+    const int sms = (cfg->sm_limit > 0 && cfg->sm_limit < prop.multiProcessorCount) ? cfg->sm_limit : prop.multiProcessorCount;
     const bool tma_likely = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && get_encode_fn() != nullptr;
     const bool narrow = tma_likely && ntile > 1 && (N - (ntile - 1) * TILE) <= 96;
     p.Tn = narrow ? ntile - 1 : 0;
@@ -937,7 +941,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     CKC(cudaMemcpyAsync(c->phi_owned, phi, (size_t)N * Ng * 8, cudaMemcpyHostToDevice, c->st));
     c->phi = c->phi_owned;
   }
-  c->sms = prop.multiProcessorCount;
+  c->sms = (cfg->sm_limit > 0 && cfg->sm_limit < prop.multiProcessorCount) ? cfg->sm_limit : prop.multiProcessorCount;
   c->use_tma = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && ((reinterpret_cast<uintptr_t>(c->phi) & 15) == 0) &&
                get_encode_fn() != nullptr;
   if (c->use_tma) {
@@ -1494,7 +1498,7 @@ int rt_get_info(rt_handle c, int32_t info[8]) {
   info[0] = 2 * c->q + 1;
   info[1] = (int32_t)c->lv.size();
   info[2] = L.gd.nx; info[3] = L.gd.ny; info[4] = L.gd.nz;
-  info[5] = (c->gexec ? 1 : 0) | (c->use_tma ? 2 : 0);
+  info[5] = ((c->gexec || !c->phase_exec.empty()) ? 1 : 0) | (c->use_tma ? 2 : 0) | (c->capture_failures > 0 ? 4 : 0);
   info[6] = (int32_t)c->launches_per_step;
   info[7] = c->pp.S;
   return RT_OK;
@@ -1697,7 +1701,11 @@ int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
       const int key = 4 * phase + 2 * (it == 0 ? 1 : 0) + (last ? 1 : 0);
       if (c->use_graph && !c->timing) {
         auto ex = c->phase_exec.find(key);
-        if (ex == c->phase_exec.end()) {
+        // A capture can be invalidated from outside the library (another host thread of the process synchronising the
+        // device or using the legacy stream in a way the capture mode forbids).  The graph is only an optimisation: a
+        // failed capture is discarded, the phase is enqueued directly this time, and the capture is tried again on the
+        // next use (three times per phase at most).
+        if (ex == c->phase_exec.end() && c->phase_capture_failures[key] < 3) {
           cudaStream_t user = c->st, cap = nullptr;
           CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
           c->st = cap;
@@ -1714,12 +1722,22 @@ int rt_slab_phase(rt_handle c, int32_t phase, int32_t it) {
           cudaStreamDestroy(cap);
           cudaGraphExec_t gx = nullptr;
           if (e == cudaSuccess) e = cudaGraphInstantiate(&gx, g, 0);
-          if (e != cudaSuccess) { cudaGetLastError(); return fail(c, RT_ECUDA, std::string("slab phase capture: ") + cudaGetErrorString(e)); }
-          c->phase_graphs.push_back(g);
-          ex = c->phase_exec.emplace(key, gx).first;
+          if (e != cudaSuccess) {
+            cudaGetLastError();
+            if (g) cudaGraphDestroy(g);
+            c->phase_capture_failures[key] += 1;
+            c->capture_failures += 1;
+          } else {
+            c->phase_graphs.push_back(g);
+            ex = c->phase_exec.emplace(key, gx).first;
+          }
         }
-        CK(cudaGraphLaunch(ex->second, c->st));
-        c->launches += c->phase_launches[key];
+        if (ex != c->phase_exec.end()) {
+          CK(cudaGraphLaunch(ex->second, c->st));
+          c->launches += c->phase_launches[key];
+        } else {
+          enqueue_slab_phase(c, phase, it);
+        }
       } else {
         enqueue_slab_phase(c, phase, it);
       }

@@ -88,6 +88,8 @@ struct GemmArgs {
   int row_beg, row_end;                                 // rows of D computed by this launch (multiples of TILE; row_end
                                                         // clipped to N); 0, N = the whole matrix.  A row block is what
                                                         // one rank of the sharded propagator owns
+  int zmode = 0;                                        // TMA kernel, symmetric outputs: 0 = Z accumulated on both sides of
+                                                        // the diagonal, 1 = upper triangle only, 2 = upper + mirrored store
 };
 // N <= GEMM_SMALL_N32: 32 x 32 CTA tiles; N <= GEMM_SMALL_N: 64 x 64; above: 128 x 128 (rt_api.cu sends N > GEMM_SMALL_N
 // to the TMA-fed kernel when TMA is available)

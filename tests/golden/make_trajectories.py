@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Writes the full-length oracle trajectories that tests/test_gpu_trajectories.py compares the CUDA path with.
 
-    python tests/golden/make_trajectories.py small_weak|small_strong|mid_laser|tiny_weak [--threads T]
+    python tests/golden/make_trajectories.py small_weak|small_strong|mid_laser|tiny_weak [--snapshot-every K]
 
 Calls ONLY oracle/rt_oracle.py and the seeded input generator (paper_2410_09189_b200/workloads.py, which holds none of
 the method's arithmetic).  Nothing here touches the CUDA path.  A full-length oracle run of `small` (1000 steps) takes
@@ -11,6 +11,10 @@ why the oracle's output is stored ("tiny, small, mid: full-length ora
 File format (text): header lines starting with '#', then one line per time level n = 0..nsteps:
     n  mu_x  mu_y  mu_z            (%.17e: round-trip exact)
 then a block "rho <index> <value>" for NPTS seeded sample points of the final density, and "rhomax <value>".
+
+`--snapshot-every K`: every K steps the levels written so far plus the density block AT THAT LEVEL are published as a
+complete, self-consistent trajectory file (atomic replace), so that an hours-long run of `mid` leaves a usable, shorter
+golden file behind whenever it is interrupted; the last snapshot is the full-length file.
 """
 import os
 import sys
@@ -35,8 +39,22 @@ def sample_points(ngrid, seed=777):
     return np.sort(np.random.default_rng(seed).choice(ngrid, size=NPTS, replace=False))
 
 
+def publish(part, out, o, w):
+    """levels written so far + the density block of the oracle's CURRENT state -> `out` (atomic)."""
+    rho = o.density()
+    tmp = out + ".tmp"
+    with open(part) as src, open(tmp, "w") as f:
+        f.write(src.read())
+        for r in sample_points(w.ngrid):
+            f.write("rho %d %.17e\n" % (r, rho[r]))
+        f.write("rhomax %.17e\n" % np.max(np.abs(rho)))
+        f.write("trP %.17e\n" % np.trace(o.P0).real)
+    os.replace(tmp, out)
+
+
 def main():
     name = sys.argv[1]
+    every = int(sys.argv[sys.argv.index("--snapshot-every") + 1]) if "--snapshot-every" in sys.argv else 0
     from oracle import rt_oracle as O
     from paper_2410_09189_b200.workloads import WORKLOADS, make_inputs_numpy, strong_kick
     wname, amp, nsteps = CASES[name]
@@ -66,12 +84,10 @@ def main():
             f.flush()
             if (n + 1) % 10 == 0:
                 print(f"{name}: step {n + 1}/{nsteps}, {time.time() - t0:.0f} s", flush=True)
-        rho = o.density()
-        for r in sample_points(w.ngrid):
-            f.write("rho %d %.17e\n" % (r, rho[r]))
-        f.write("rhomax %.17e\n" % np.max(np.abs(rho)))
-        f.write("trP %.17e\n" % np.trace(o.P0).real)
-    os.replace(part, out)
+            if every and (n + 1) % every == 0 and n + 1 < nsteps:
+                publish(part, out, o, w)
+    publish(part, out, o, w)
+    os.remove(part)
 
 
 if __name__ == "__main__":
