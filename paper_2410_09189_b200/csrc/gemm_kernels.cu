@@ -360,26 +360,10 @@ gemm_abt_kernel(GemmArgs ga) {
   cp_async_wait<0>();
   const double fin = (ga.A1 && ratio != 1.0) ? ga.alpha0 * ratio : ga.alpha0;
 
-  // Z1 / Z2 are read for a whole row block first and written afterwards: D, Z1, Z2 may alias as far as the compiler
-  // knows, so interleaved read-modify-writes would serialise into one L2 round trip each.
-  const bool hasZ1 = ga.Z1 != nullptr, hasZ2 = ga.Z2 != nullptr;
 #pragma unroll
   for (int a = 0; a < FA; ++a) {
     const int row = i0 + wrow + 8 * a + g;
     if (row < N) {
-      double2 z1[FB], z2[FB];
-      if (hasZ1 || hasZ2) {
-#pragma unroll
-        for (int b = 0; b < FB; ++b) {
-          const int col = j0 + wcol + 8 * b + 2 * c;
-          z1[b] = z2[b] = make_double2(0.0, 0.0);
-          if (col < N) {
-            const long long o = (long long)row * ldn + col;
-            if (hasZ1) z1[b] = *reinterpret_cast<const double2*>(ga.Z1 + o);
-            if (hasZ2) z2[b] = *reinterpret_cast<const double2*>(ga.Z2 + o);
-          }
-        }
-      }
 #pragma unroll
       for (int b = 0; b < FB; ++b) {
         const int col = j0 + wcol + 8 * b + 2 * c;
@@ -387,13 +371,13 @@ gemm_abt_kernel(GemmArgs ga) {
           const long long o = (long long)row * ldn + col;
           const double2 d = make_double2(fin * acc[a][b][0], fin * acc[a][b][1]);
           if (ga.D) *reinterpret_cast<double2*>(ga.D + o) = d;
-          if (hasZ1) {
-            double2 z = z1[b];
+          if (ga.Z1) {
+            double2 z = *reinterpret_cast<double2*>(ga.Z1 + o);
             z.x += ga.beta1 * d.x; z.y += ga.beta1 * d.y;
             *reinterpret_cast<double2*>(ga.Z1 + o) = z;
           }
-          if (hasZ2) {
-            double2 z = z2[b];
+          if (ga.Z2) {
+            double2 z = *reinterpret_cast<double2*>(ga.Z2 + o);
             z.x += ga.beta2 * d.x; z.y += ga.beta2 * d.y;
             *reinterpret_cast<double2*>(ga.Z2 + o) = z;
           }

@@ -17,8 +17,8 @@ namespace {
 constexpr int FA = 8, FB = 4, WM = 2, WN = 4;
 constexpr int NCONS = WM * WN;                 // consumer warps
 constexpr int NTHREADS = 32 * (NCONS + 4);     // + one producer warpgroup (only its first lane works)
-// setmaxnreg budget: the CTA is launched with 384 x 168 = 64512 registers; 256*240 + 128*24 = 64512 exactly
-constexpr int REGS_CONSUMER = 240, REGS_PRODUCER = 24;
+// setmaxnreg budget: the CTA is launched with 384 x 168 = 64512 registers; 256*232 + 128*40 = 64512 exactly
+constexpr int REGS_CONSUMER = 232, REGS_PRODUCER = 40;
 constexpr int ST = 6;                          // pipeline stages
 constexpr int TILE_D = TILE * BK;              // doubles in one 128 x 16 operand tile (16 KB)
 constexpr int STAGE_D = 2 * TILE_D;            // A + B
@@ -59,9 +59,22 @@ __device__ __forceinline__ void init_bars(Bars* bars) {
 // ======================================================================================================
 // a1 projection
 // ======================================================================================================
+// Persistent: CTA c works through the items c, c + G, c + 2G, ... of the class-ordered (split, tile) list, so the G CTAs
+// that run together are always G consecutive items -- the same split of neighbouring tiles of one 2-D block, which share
+// Phi row panels.  That sharing only turns into L2 hits while the CTAs stay close together along k: all of them read the
+// same k-range of ~2 sqrt(G) row panels, 1 KB per panel and grid point, so a spread of a few thousand grid points
+// already overflows the L2.  A plain grid (one CTA per item, round 2 first capture) drifted apart over the 37 ms a CTA
+// lives at N = 13,000: 38 % L2 hits, 6.2 TB of DRAM reads per launch against 0.12 TB of Phi.  PACING keeps them together:
+// every PACE_CK stages the producer thread counts itself in at a checkpoint counter and does not run ahead of the
+// checkpoint PACE_W before until all G CTAs have reached it.  Only TMA issue is throttled, never the slowest CTA, and a
+// CTA whose peers are not there (tail of the launch, or SMs shared with another stream) gives up after two timeouts.
+constexpr int PACE_CK = 32;
+constexpr long long PACE_TIMEOUT_CLK = 100000;      // ~50 us
+
 __global__ void __launch_bounds__(NTHREADS, 1)
 project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __restrict__ w,
-                   const int2* __restrict__ tiles, double* __restrict__ W, const ProjectPlan pl) {
+                   const int2* __restrict__ tiles, double* __restrict__ W, const ProjectPlan pl, int nitems,
+                   int* __restrict__ pace_cnt, int pace_w) {
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -70,28 +83,44 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
   init_bars(bars);
 
   const int N = pl.N, ldn = pl.ldn;
-  const ProjBlock pb = project_decode(blockIdx.x, pl);
-  const int s = pb.s;
-  const int2 tt = tiles[pb.t];
-  const int i0 = tt.x * TILE, j0 = tt.y * TILE;
-  const long long kbeg = pb.kbeg, kend = pb.kend;
-  const int nk = (int)((kend - kbeg + BK - 1) / BK);
+  const int G = gridDim.x;
 
   if (warp >= NCONS) {
-    // ===== producer =====
+    // ===== producer: runs ahead across items =====
     regs_producer();
     if (warp == NCONS && lane == 0) {
       tma_prefetch_desc(&tmPhi);
-      for (int kt = 0; kt < nk; ++kt) {
-        const int slot = kt % ST;
-        if (kt >= ST) mbar_wait(smem_u32(&bars->empty[slot]), ((kt / ST) - 1) & 1);
-        const uint32_t full = smem_u32(&bars->full[slot]);
-        mbar_expect_tx(full, 2 * TILE_BYTES + BK * 8);
-        const long long k0 = kbeg + (long long)kt * BK;
-        double* sA = tilesm + (size_t)slot * STAGE_D;
-        tma_load_2d(sA, &tmPhi, (int)k0, i0, full);
-        tma_load_2d(sA + TILE_D, &tmPhi, (int)k0, j0, full);
-        bulk_load_1d(wsm + slot * BK, w + k0, BK * 8, full);     // w is padded to a multiple of 16 doubles
+      long long it = 0;
+      int misses = pace_cnt ? 0 : 2;
+      for (int item = blockIdx.x; item < nitems; item += G) {
+        const ProjBlock pb = project_decode(item, pl);
+        const int2 tt = tiles[pb.t];
+        const int i0 = tt.x * TILE, j0 = tt.y * TILE;
+        const int nk = (int)((pb.kend - pb.kbeg + BK - 1) / BK);
+        for (int kt = 0; kt < nk; ++kt, ++it) {
+          if (misses < 2 && (it % PACE_CK) == 0) {
+            const long long q = it / PACE_CK;
+            atomicAdd(pace_cnt + q, 1);
+            if (q >= pace_w) {
+              const volatile int* prev = pace_cnt + (q - pace_w);
+              if (*prev < G) {
+                const long long t0 = clock64();
+                while (*prev < G) {
+                  if (clock64() - t0 > PACE_TIMEOUT_CLK) { ++misses; break; }
+                }
+              }
+            }
+          }
+          const int slot = (int)(it % ST);
+          if (it >= ST) mbar_wait(smem_u32(&bars->empty[slot]), (uint32_t)((it / ST) - 1) & 1);
+          const uint32_t full = smem_u32(&bars->full[slot]);
+          mbar_expect_tx(full, 2 * TILE_BYTES + BK * 8);
+          const long long k0 = pb.kbeg + (long long)kt * BK;
+          double* sA = tilesm + (size_t)slot * STAGE_D;
+          tma_load_2d(sA, &tmPhi, (int)k0, i0, full);
+          tma_load_2d(sA + TILE_D, &tmPhi, (int)k0, j0, full);
+          bulk_load_1d(wsm + slot * BK, w + k0, BK * 8, full);     // w is padded to a multiple of 16 doubles
+        }
       }
     }
     return;
@@ -100,88 +129,95 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
   // ===== consumers =====
   regs_consumer();
   const int g = lane >> 2, c = lane & 3, pg = perm8(g);
-  // Diagonal tile of the symmetric output: only 8 x 8 blocks on or above the diagonal are needed (project_reduce reads
-  // j >= i), 136 of the CTA's 256.  The warp roles (wm, wn) are permuted so that every scheduler partition
-  // (warp % 4) gets 32-36 of them instead of 10-58: {(0,2),(1,0)}, {(0,3),(1,1)}, {(0,1),(1,2)}, {(0,0),(1,3)}.
-  const bool diag = i0 == j0;
-  double* Ws = W + (long long)s * N * ldn;
-  if (!diag && N - j0 <= 96) {
-    // Ragged last tile column with at most 96 valid columns (N = 2400: 96): the 8 warps cover 128 x 96 as 2 x 4 warp
-    // tiles of 64 x 24 instead of leaving the warps of the last 32 columns multiplying padding.
-    constexpr int FB3 = 3;
-    const int wrow3 = (warp / WN) * (8 * FA), wcol3 = (warp % WN) * (8 * FB3);
-    double acc3[FA][FB3][2];
+  long long it = 0;
+  for (int item = blockIdx.x; item < nitems; item += G) {
+    const ProjBlock pb = project_decode(item, pl);
+    const int2 tt = tiles[pb.t];
+    const int i0 = tt.x * TILE, j0 = tt.y * TILE;
+    const int nk = (int)((pb.kend - pb.kbeg + BK - 1) / BK);
+    // Diagonal tile of the symmetric output: only 8 x 8 blocks on or above the diagonal are needed (project_reduce reads
+    // j >= i), 136 of the CTA's 256.  The warp roles (wm, wn) are permuted so that every scheduler partition
+    // (warp % 4) gets 32-36 of them instead of 10-58: {(0,2),(1,0)}, {(0,3),(1,1)}, {(0,1),(1,2)}, {(0,0),(1,3)}.
+    const bool diag = i0 == j0;
+    double* Ws = W + (long long)pb.s * N * ldn;
+    if (!diag && N - j0 <= 96) {
+      // Ragged last tile column with at most 96 valid columns (N = 2400: 96): the 8 warps cover 128 x 96 as 2 x 4 warp
+      // tiles of 64 x 24 instead of leaving the warps of the last 32 columns multiplying padding.
+      constexpr int FB3 = 3;
+      const int wrow3 = (warp / WN) * (8 * FA), wcol3 = (warp % WN) * (8 * FB3);
+      double acc3[FA][FB3][2];
+#pragma unroll
+      for (int a = 0; a < FA; ++a)
+#pragma unroll
+        for (int b = 0; b < FB3; ++b) acc3[a][b][0] = acc3[a][b][1] = 0.0;
+      for (int kt = 0; kt < nk; ++kt, ++it) {
+        const int slot = (int)(it % ST);
+        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        const double* sA = tilesm + (size_t)slot * STAGE_D;
+        mma_stage_kc_tma<FA, FB3, true>(acc3, sA, sA + TILE_D, wsm + slot * BK, wrow3, wcol3, pg, c);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+      }
+#pragma unroll
+      for (int a = 0; a < FA; ++a) {
+        const int row = i0 + wrow3 + 8 * a + pg;
+        if (row < N) {
+#pragma unroll
+          for (int b = 0; b < FB3; ++b) {
+            const int col = j0 + wcol3 + 8 * b + c;
+            if (col < N) Ws[(long long)row * ldn + col] = acc3[a][b][0];
+            if (col + 4 < N) Ws[(long long)row * ldn + col + 4] = acc3[a][b][1];
+          }
+        }
+      }
+      continue;
+    }
+    const int role = diag ? ((warp < 4) ? ((0x0132 >> (4 * warp)) & 15) : warp) : warp;
+    const int wrow = (role / WN) * (8 * FA), wcol = (role % WN) * (8 * FB);
+    // blocks on or above the diagonal, as row counts for the two column halves of the warp tile (rounded up to a
+    // rectangle): (0,0), (1,2): rows < 2 | 4 ; (0,1), (1,3): rows < 6 | 8 ; (0,2), (0,3): all ; (1,0), (1,1): none
+    const int dlt = (wcol - wrow) / 8;
+    double acc[FA][FB][2];
 #pragma unroll
     for (int a = 0; a < FA; ++a)
 #pragma unroll
-      for (int b = 0; b < FB3; ++b) acc3[a][b][0] = acc3[a][b][1] = 0.0;
-    for (int kt = 0; kt < nk; ++kt) {
-      const int slot = kt % ST;
-      mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
-      const double* sA = tilesm + (size_t)slot * STAGE_D;
-      mma_stage_kc_tma<FA, FB3, true>(acc3, sA, sA + TILE_D, wsm + slot * BK, wrow3, wcol3, pg, c);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
-    }
-#pragma unroll
-    for (int a = 0; a < FA; ++a) {
-      const int row = i0 + wrow3 + 8 * a + pg;
-      if (row < N) {
-#pragma unroll
-        for (int b = 0; b < FB3; ++b) {
-          const int col = j0 + wcol3 + 8 * b + c;
-          if (col < N) Ws[(long long)row * ldn + col] = acc3[a][b][0];
-          if (col + 4 < N) Ws[(long long)row * ldn + col + 4] = acc3[a][b][1];
-        }
+      for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+
+    if (!diag) {
+      for (int kt = 0; kt < nk; ++kt, ++it) {
+        const int slot = (int)(it % ST);
+        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        const double* sA = tilesm + (size_t)slot * STAGE_D;
+        mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+      }
+    } else {
+      const bool live = i0 + wrow < N && j0 + wcol < N;
+      for (int kt = 0; kt < nk; ++kt, ++it) {
+        const int slot = (int)(it % ST);
+        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        const double* sA = tilesm + (size_t)slot * STAGE_D;
+        if (!live) {}                             // the whole warp tile is padding (N < 128: tiny systems)
+        else if (dlt >= 8) mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+        else if (dlt == 4) mma_stage_kc_tma<FA, FB, true, 6, 8>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+        else if (dlt == 0) mma_stage_kc_tma<FA, FB, true, 2, 4>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
       }
     }
-    return;
-  }
-  const int role = diag ? ((warp < 4) ? ((0x0132 >> (4 * warp)) & 15) : warp) : warp;
-  const int wrow = (role / WN) * (8 * FA), wcol = (role % WN) * (8 * FB);
-  // blocks on or above the diagonal, as row counts for the two column halves of the warp tile (rounded up to a
-  // rectangle): (0,0), (1,2): rows < 2 | 4 ; (0,1), (1,3): rows < 6 | 8 ; (0,2), (0,3): all ; (1,0), (1,1): none
-  const int dlt = (wcol - wrow) / 8;
-  double acc[FA][FB][2];
-#pragma unroll
-  for (int a = 0; a < FA; ++a)
-#pragma unroll
-    for (int b = 0; b < FB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
 
-  if (!diag) {
-    for (int kt = 0; kt < nk; ++kt) {
-      const int slot = kt % ST;
-      mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
-      const double* sA = tilesm + (size_t)slot * STAGE_D;
-      mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
-    }
-  } else {
-    const bool live = i0 + wrow < N && j0 + wcol < N;
-    for (int kt = 0; kt < nk; ++kt) {
-      const int slot = kt % ST;
-      mbar_wait(smem_u32(&bars->full[slot]), (kt / ST) & 1);
-      const double* sA = tilesm + (size_t)slot * STAGE_D;
-      if (!live) {}                             // the whole warp tile is padding (N < 128: tiny systems)
-      else if (dlt >= 8) mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
-      else if (dlt == 4) mma_stage_kc_tma<FA, FB, true, 6, 8>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
-      else if (dlt == 0) mma_stage_kc_tma<FA, FB, true, 2, 4>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
-    }
-  }
-
-  // epilogue: raw partial sums into slab s.  MMA row g <-> tile row perm8(g); tile col n' <-> perm8(n')
+    // epilogue: raw partial sums into slab s.  MMA row g <-> tile row perm8(g); tile col n' <-> perm8(n')
 #pragma unroll
-  for (int a = 0; a < FA; ++a) {
-    const int row = i0 + wrow + 8 * a + pg;
-    if (row < N) {
+    for (int a = 0; a < FA; ++a) {
+      const int row = i0 + wrow + 8 * a + pg;
+      if (row < N) {
 #pragma unroll
-      for (int b = 0; b < FB; ++b) {
-        const int col = j0 + wcol + 8 * b + c;        // perm8(2c) = c, perm8(2c+1) = c + 4
-        if (col < N) Ws[(long long)row * ldn + col] = acc[a][b][0];
-        if (col + 4 < N) Ws[(long long)row * ldn + col + 4] = acc[a][b][1];
+        for (int b = 0; b < FB; ++b) {
+          const int col = j0 + wcol + 8 * b + c;        // perm8(2c) = c, perm8(2c+1) = c + 4
+          if (col < N) Ws[(long long)row * ldn + col] = acc[a][b][0];
+          if (col + 4 < N) Ws[(long long)row * ldn + col + 4] = acc[a][b][1];
+        }
       }
     }
   }
@@ -189,9 +225,28 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
 
 size_t tma_smem_bytes() { return SMEM_TOTAL; }
 
+// Pacing pays where the 2-D blocking of the tile list does (ntile well above the 12 x 12 block: at N = 2,400 every wave
+// touches all 19 row panels anyway and pacing only cost 2 % of the kernel time) and on launches long enough to drift
+// (per-CTA stage count >= PACE_MIN_STAGES, ~35 ms).  Unpaced launches keep one CTA per item: the hardware then hands out
+// items as SMs free up, which measured less DRAM traffic than the static round-robin of persistent CTAs.
+constexpr long long PACE_MIN_STAGES = 16384;
+constexpr int PACE_MIN_NTILE = 32;
+size_t project_tma_pace_ints(const ProjectPlan& p, int sms) {
+  const long long nitems = p.grid();
+  const long long G = nitems < sms ? nitems : sms;
+  const long long per_item = (p.kchunk + BK - 1) / BK;               // the longest class
+  const long long stages = ((nitems + G - 1) / G) * per_item;
+  if (G < 2 || p.ntile < PACE_MIN_NTILE || stages < PACE_MIN_STAGES) return 0;
+  return (size_t)(stages / PACE_CK + 2);
+}
+
 void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const double* w, const int2* tiles, double* W,
-                        cudaStream_t st) {
-  project_tma_kernel<<<p.grid(), NTHREADS, SMEM_TOTAL, st>>>(tmPhi, w, tiles, W, p);
+                        int sms, int* pace_cnt, int pace_w, cudaStream_t st) {
+  const int nitems = p.grid();
+  const size_t npace = pace_cnt ? project_tma_pace_ints(p, sms) : 0;
+  const int G = npace ? (nitems < sms ? nitems : sms) : nitems;
+  if (npace) cudaMemsetAsync(pace_cnt, 0, npace * sizeof(int), st);
+  project_tma_kernel<<<G, NTHREADS, SMEM_TOTAL, st>>>(tmPhi, w, tiles, W, p, nitems, npace ? pace_cnt : nullptr, pace_w);
 }
 
 // ======================================================================================================
@@ -243,6 +298,10 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
     if (warp == NCONS && lane == 0) {
       tma_prefetch_desc(&tmP);
       tma_prefetch_desc(&tmPhiN);
+      // the Phi panels of the r-tiles in flight are what the launch keeps in L2 (every type re-reads them); the fold
+      // streams through (shared only by the group_r CTAs of the same type, which walk it together)
+      const uint64_t pol_phi = l2_policy_evict_last();
+      const uint64_t pol_fold = l2_policy_evict_first();
       long long it = 0;
       for (long long L = blockIdx.x; L < nwork; L += gridDim.x) {
         const DensWork wk = dens_decode(L, ntypes, nrt, group_r, group_t);
@@ -258,13 +317,13 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
             mbar_expect_tx(full, 2 * TILE_BYTES);
             const int k0 = j0 + (sg.s0 + sg.dir * i) * BK;
             double* sA = tilesm + (size_t)slot * STAGE_D;
-            tma_load_2d(sA, &tmP, k0, j0, full);                              // Pfold[j0.., k0..]
+            tma_load_2d_hint(sA, &tmP, k0, j0, full, pol_fold);               // Pfold[j0.., k0..]
             if (b3d) {                                                        // Phi[k0.., r0 .. r0+127] in one op
-              tma_load_3d(sA + TILE_D, &tmPhiN, 0, k0, (int)(r0 >> 4), full);
+              tma_load_3d_hint(sA + TILE_D, &tmPhiN, 0, k0, (int)(r0 >> 4), full, pol_phi);
             } else {
 #pragma unroll
               for (int bx = 0; bx < 8; ++bx)                                  // Phi[k0.., r0 + 16 bx ..]
-                tma_load_2d(sA + TILE_D + bx * 256, &tmPhiN, (int)(r0 + 16 * bx), k0, full);
+                tma_load_2d_hint(sA + TILE_D + bx * 256, &tmPhiN, (int)(r0 + 16 * bx), k0, full, pol_phi);
             }
           }
         }
@@ -407,7 +466,6 @@ struct GemmTmaArgs {
   double alpha0, alpha1;
   double* D; double* Z1; double beta1; double* Z2; double beta2;
   const int* skip;         // non-zero -> no-op (orders past convergence of the commutator series)
-  int zmode;               // how Z1 / Z2 of a symmetric-output launch are maintained below the diagonal (see the epilogue)
   double* ws;              // [G][TILE*TILE] partial accumulators of the tail items, indexed by range
   int* sync;               // [0] = ticket counter, [1] = finished-CTA counter, [2 + p] = flag of range p (0 = empty)
 };
@@ -572,66 +630,34 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
       }
 
       // ---- epilogue of a complete tile ----
-      // The read-modify-writes of Z1 / Z2 are done in two phases per batch of 2 x 2 fragments -- all loads, then all
-      // stores: D, Z1 and Z2 are plain pointers that may alias as far as the compiler knows, so interleaved `Z[o] += ...`
-      // statements serialise into one L2 round trip each (measured at N = 2400: 0.68 ms against 0.48 ms for the same
-      // product without Z, DMMA pipe 70 % against 91 %).  zmode (symmetric outputs only): 0 = Z is accumulated on both
-      // sides of the diagonal; 1 = on the upper triangle only (the lower one is not maintained); 2 = upper triangle, and
-      // the finished value is stored to its mirror image too (the last accumulation of a chain started with zmode 1).
+      // Every element is finished (D stored, Z1 / Z2 read, updated and stored) before the next one is touched.  A version
+      // that read Z1 / Z2 for a batch of fragments first and stored afterwards ran the accumulating products 30 % faster
+      // (the read-modify-writes are one dependent L2 round trip each) but gave results that changed from call to call at
+      // N >= 5,000 -- single rows of a power of Y off by 1e-17 ... 1e-10, gone with CUDA_LAUNCH_BLOCKING=1, cause not
+      // found -- so the order that is bit-reproducible in every test stays.
       const bool diag = ga.sym && i0 == j0;
-      const bool hasZ1 = ga.Z1 != nullptr, hasZ2 = ga.Z2 != nullptr;
-      const bool zrmw_mirror = ga.sym && ga.zmode == 0, zst_mirror = ga.sym && ga.zmode != 1;
 #pragma unroll
       for (int a = 0; a < FA; ++a) {
         const int row = i0 + wrow + 8 * a + pg;
         if (row < N) {
 #pragma unroll
-          for (int bb = 0; bb < FB; bb += 2) {
-            double z1[2][2], z2[2][2], z1m[2][2], z2m[2][2];
-            if (hasZ1 || hasZ2) {
+          for (int b = 0; b < FB; ++b) {
 #pragma unroll
-              for (int b = 0; b < 2; ++b)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                  const int col = j0 + wcol + 8 * (bb + b) + c + 4 * e;
-                  z1[b][e] = z2[b][e] = z1m[b][e] = z2m[b][e] = 0.0;
-                  if (col < N && (!diag || col >= row)) {
-                    const long long o = (long long)row * ldn + col;
-                    if (hasZ1) z1[b][e] = ga.Z1[o];
-                    if (hasZ2) z2[b][e] = ga.Z2[o];
-                    if (zrmw_mirror && row != col) {
-                      const long long om = (long long)col * ldn + row;
-                      if (hasZ1) z1m[b][e] = ga.Z1[om];
-                      if (hasZ2) z2m[b][e] = ga.Z2[om];
-                    }
-                  }
-                }
-            }
-#pragma unroll
-            for (int b = 0; b < 2; ++b) {
-#pragma unroll
-              for (int e = 0; e < 2; ++e) {
-                const int col = j0 + wcol + 8 * (bb + b) + c + 4 * e;
-                if (col < N && (!diag || col >= row)) {
-                  const long long o = (long long)row * ldn + col;
-                  double d = fin * acc[a][bb + b][e];
-                  if (ga.sym < 0 && row == col) d = 0.0;
-                  const double v1 = z1[b][e] + ga.beta1 * d, v2 = z2[b][e] + ga.beta2 * d;
-                  if (ga.D) ga.D[o] = d;
-                  if (hasZ1) ga.Z1[o] = v1;
-                  if (hasZ2) ga.Z2[o] = v2;
-                  if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
-                    const long long om = (long long)col * ldn + row;
-                    const double dm = msign * d;
-                    if (ga.D) ga.D[om] = dm;
-                    if (zrmw_mirror) {
-                      if (hasZ1) ga.Z1[om] = z1m[b][e] + ga.beta1 * dm;
-                      if (hasZ2) ga.Z2[om] = z2m[b][e] + ga.beta2 * dm;
-                    } else if (zst_mirror) {             // zmode 2: Z is symmetric (sym = +1 chains only)
-                      if (hasZ1) ga.Z1[om] = v1;
-                      if (hasZ2) ga.Z2[om] = v2;
-                    }
-                  }
+            for (int e = 0; e < 2; ++e) {
+              const int col = j0 + wcol + 8 * b + c + 4 * e;
+              if (col < N && (!diag || col >= row)) {
+                const long long o = (long long)row * ldn + col;
+                double d = fin * acc[a][b][e];
+                if (ga.sym < 0 && row == col) d = 0.0;
+                if (ga.D) ga.D[o] = d;
+                if (ga.Z1) ga.Z1[o] += ga.beta1 * d;
+                if (ga.Z2) ga.Z2[o] += ga.beta2 * d;
+                if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
+                  const long long om = (long long)col * ldn + row;
+                  const double dm = msign * d;
+                  if (ga.D) ga.D[om] = dm;
+                  if (ga.Z1) ga.Z1[om] += ga.beta1 * dm;
+                  if (ga.Z2) ga.Z2[om] += ga.beta2 * dm;
                 }
               }
             }
@@ -664,7 +690,7 @@ void launch_gemm_abt_tma(const GemmArgs& g, const CUtensorMap& tmA0, const CUten
                          cudaStream_t st) {
   if (ntiles <= 0) return;
   GemmTmaArgs a{g.N, g.ldn, g.A1 ? 2 : 1, sym, tiles, ntiles, g.alpha0, g.alpha1, g.D, g.Z1, g.beta1, g.Z2, g.beta2,
-                g.skip, g.zmode, ws, sync};
+                g.skip, ws, sync};
   const int grid = gemm_tma_grid(ntiles, g.N, a.nterms, sms);
   gemm_abt_tma_kernel<<<grid, NTHREADS, SMEM_TOTAL, st>>>(tmA0, tmB0, tmA1, tmB1, a);
 }

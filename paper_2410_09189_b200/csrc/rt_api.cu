@@ -4,7 +4,9 @@
 #include "../../include/rt_tddft.h"
 #include "rt_internal.h"
 
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstdio>
 #include <cstring>
 #include <map>
@@ -65,6 +67,8 @@ struct rt_ctx {
   int2* d_tiles_sym = nullptr;    // upper tiles (ti <= tj) row-major: the symmetric-output N x N GEMMs (stream-K walks them in order)
   int ntile = 0;
   double* gemm_ws = nullptr;      // stream-K fix-up workspace and flags of the TMA N x N GEMM (gemm_tma.cu)
+  int* pace_cnt = nullptr;        // checkpoint counters of the paced projection launch (gemm_tma.cu), nullptr: not paced
+  int pace_w = 1;                 // how many checkpoints a CTA may lead the slowest one by
   int* gemm_sync = nullptr;
   // row-sharded propagator: rank `shard` of `nshard` owns the rows [row_beg, row_end) of every N x N product
   int nshard = 1, shard = 0, shard_rows = 0, row_beg = 0, row_end = 0;
@@ -298,10 +302,10 @@ void stage_end(rt_ctx* c) {
 // plain product, because the mirror image of a row block belongs to other ranks.
 void enqueue_gemm(rt_ctx* c, int sym, const double* A0, const double* B0, double a0, const double* A1,
                   const double* B1, double a1, double* D, double* Z1 = nullptr, double b1 = 0, double* Z2 = nullptr,
-                  double b2 = 0, const int* skip = nullptr, bool rows = false, int zmode = 0) {
+                  double b2 = 0, const int* skip = nullptr, bool rows = false) {
   const bool shard = rows && c->nshard > 1;
   GemmArgs g{c->N, c->ldn, A0, B0, a0, A1, B1, a1, D, Z1, b1, Z2, b2, skip, shard ? c->row_beg : 0,
-             shard ? c->row_end : c->N, zmode};
+             shard ? c->row_end : c->N};
   if (g.row_end <= g.row_beg) return;                       // this rank owns no rows (more ranks than tile rows)
   if (c->use_tma && c->N > GEMM_SMALL_N) {
     const CUtensorMap& mA0 = nn_map(c, A0);
@@ -330,8 +334,7 @@ void enqueue_expm(rt_ctx* c) {
     ck = -ck / ((2.0 * k - 1.0) * (2.0 * k));
     sk = -sk / ((2.0 * k) * (2.0 * k + 1.0));
     double* cur = (k < c->q) ? ((k & 1) ? c->Yc : c->Yb) : nullptr;
-    // C and Sc are symmetric: the chain accumulates their upper triangles, the last product stores the mirror image
-    enqueue_gemm(c, 1, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk, nullptr, false, k < c->q ? 1 : 2);
+    enqueue_gemm(c, 1, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, c->Cm, ck, c->Sc, sk);
     prev = cur;
   }
   enqueue_gemm(c, 1, c->X, c->Sc, 1.0, nullptr, nullptr, 0, c->Sm);
@@ -515,7 +518,7 @@ void enqueue_vxc(rt_ctx* c, const double* rho, double* out) {
 
 // eps != nullptr: the ground-state Hamiltonian is added -- diag(eps), or the matrix Hks of rt_create_general
 void enqueue_project(rt_ctx* c, const double* w, const double* eps, double* H) {
-  if (c->use_tma) launch_project_tma(c->pp, c->tmPhiK, w, c->d_tiles, c->W, c->st);
+  if (c->use_tma) launch_project_tma(c->pp, c->tmPhiK, w, c->d_tiles, c->W, c->sms, c->pace_cnt, c->pace_w, c->st);
   else launch_project(c->pp, c->phi, w, c->d_tiles, c->W, c->st);
   const bool mat = eps && c->Hks;
   launch_project_reduce(c->pp, c->W, mat ? nullptr : eps, c->dvol, H, c->st, mat ? c->Hks : nullptr);
@@ -901,19 +904,23 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     const int nsplit = 1;
     build_density_types(N, ntile, nsplit, c->segs);
     d.ntypes = (int)(c->segs.size() / 2);
-    // supertile shape group_t x group_r (~ one item per SM): a supertile reads its group_t fold panels and its group_r Phi
-    // panels once from DRAM, so the launch moves about  |Phi| * ntypes/group_t + |P fold| * nrt/group_r  bytes
+    // Raster (gemm_tma.cu dens_decode): ALL types of a group of group_r r-tiles run before the next group starts, r-tile
+    // fastest.  What the launch keeps in L2 is the Phi column panel (N x 128 doubles) of every r-tile in flight -- each of
+    // the ntypes items of an r-tile re-reads its own k-range of that panel, at its own time, so only residency (TMA loads
+    // with the evict_last hint), not lock-step, makes the reuse happen -- while the fold streams through, shared by the
+    // group_r CTAs of one type that walk it together.  DRAM traffic ~ |Phi| + |P fold| * nrt / group_r, with group_r
+    // bounded by  group_r * panel <= ~40 MB  (the 126 MB L2 is two partitions that mirror remote lines).
+    // (Round-2 capture at N = 13,000 with 12 x 12 supertiles of types x r-tiles, which assumed that CTAs of different
+    // types share Phi tiles in lock-step -- they do not, their k-ranges differ: 7.2 TB of DRAM reads per launch.)
     {
-      const double phi_b = (double)N * Ng * 8, pf_b = 0.5 * (double)N * ldn * 8;
-      double best_cost = 1e300;
-      d.group_t = 1; d.group_r = 1;
-      for (int gt = 1; gt <= d.ntypes && gt <= sms; ++gt) {
-        long long gr = sms / gt;
-        if (gr > d.nrt) gr = d.nrt;
-        if (gr < 1) gr = 1;
-        const double cost = phi_b * std::ceil((double)d.ntypes / gt) + pf_b * std::ceil((double)d.nrt / (double)gr);
-        if (cost < best_cost) { best_cost = cost; d.group_t = gt; d.group_r = (int)gr; }
-      }
+      const double panel = (double)N * TILE * 8;
+      long long gr = (long long)(40.0e6 / panel);
+      if (gr > d.nrt) gr = d.nrt;
+      if (gr < 1) gr = 1;
+      d.group_t = d.ntypes;
+      d.group_r = (int)gr;
+      if (const char* e = getenv("RT_DBG_GROUP_R")) d.group_r = std::max(1, atoi(e));
+      if (const char* e = getenv("RT_DBG_GROUP_T")) d.group_t = std::max(1, std::min(d.ntypes, atoi(e)));
     }
   }
 
@@ -942,6 +949,11 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     c->phi = c->phi_owned;
   }
   c->sms = (cfg->sm_limit > 0 && cfg->sm_limit < prop.multiProcessorCount) ? cfg->sm_limit : prop.multiProcessorCount;
+  if (const char* e = getenv("RT_DBG_PACE_W")) c->pace_w = std::max(1, atoi(e));
+  if (getenv("RT_DBG_PERSIST_L2")) {
+    cudaError_t pe = cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)prop.persistingL2CacheMaxSize);
+    fprintf(stderr, "persisting L2 limit %d bytes -> %s\n", prop.persistingL2CacheMaxSize, cudaGetErrorString(pe));
+  }
   c->use_tma = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && ((reinterpret_cast<uintptr_t>(c->phi) & 15) == 0) &&
                get_encode_fn() != nullptr;
   if (c->use_tma) {
@@ -1035,6 +1047,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
       for (int tj = ti; tj < ntile; ++tj) symrm.push_back(make_int2(ti, tj));
     ALLOC(c->d_tiles_sym, symrm.size());
     CKC(cudaMemcpyAsync(c->d_tiles_sym, symrm.data(), symrm.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
+    if (c->use_tma && project_tma_pace_ints(c->pp, c->sms) > 0 && !getenv("RT_DBG_NOPACE")) ALLOC(c->pace_cnt, project_tma_pace_ints(c->pp, c->sms));
     if (c->use_tma && N > GEMM_SMALL_N) {
       ALLOC(c->gemm_ws, gemm_tma_ws_doubles(c->sms));
       ALLOC(c->gemm_sync, gemm_tma_sync_ints(c->sms));

@@ -88,8 +88,6 @@ struct GemmArgs {
   int row_beg, row_end;                                 // rows of D computed by this launch (multiples of TILE; row_end
                                                         // clipped to N); 0, N = the whole matrix.  A row block is what
                                                         // one rank of the sharded propagator owns
-  int zmode = 0;                                        // TMA kernel, symmetric outputs: 0 = Z accumulated on both sides of
-                                                        // the diagonal, 1 = upper triangle only, 2 = upper + mirrored store
 };
 // N <= GEMM_SMALL_N32: 32 x 32 CTA tiles; N <= GEMM_SMALL_N: 64 x 64; above: 128 x 128 (rt_api.cu sends N > GEMM_SMALL_N
 // to the TMA-fed kernel when TMA is available)
@@ -101,8 +99,9 @@ size_t gemm_smem_bytes();
 int    init_tma_kernels();                 // sets the dynamic shared-memory attribute; returns a cudaError_t value
 size_t tma_smem_bytes();
 // tmPhi: Phi [N][Ng] with box {16 k, 128 rows}; w must be readable up to roundup(Ng, 16) doubles
+size_t project_tma_pace_ints(const ProjectPlan& p, int sms);   // checkpoint counters of a paced launch (0: not paced)
 void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const double* w, const int2* tiles, double* W,
-                        cudaStream_t st);
+                        int sms, int* pace_cnt, int pace_w, cudaStream_t st);
 // tmP: Pfold [N][N] (ld = ldn) box {16, 128}; tmPhiN: Phi with box {16 r, 16 k-rows} (b3d = 0: 8 loads per stage)
 // or, when Ng % 16 == 0, the 3-D view {16 r-low, N k, Ng/16 r-high} with box {16, 16, 8} (b3d = 1: one load)
 void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, int b3d,
