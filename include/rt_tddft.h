@@ -111,11 +111,6 @@ typedef struct {
                                Laplacian as the operator V_H solves -- each of the n_vcycles cycles is then
                                r = f - A4 u, d = one 7-point V-cycle on (0, r), u += d (multigrid as the preconditioner,
                                L77; DESIGN R17) -- and 4-point gradients                                              */
-  /* -- several handles side by side on one GPU (the three delta-kick polarisations of L453 on three streams) ------- */
-  int32_t  sm_limit;        /* > 0: size the split-K plans and the persistent grids of the DMMA kernels (a1, a5, a3/a4) for
-                               at most this many SMs, so that the kernels of handles on other streams fit beside them
-                               instead of queueing behind a launch that fills the GPU.  Results do not depend on it
-                               beyond the summation order of the split-K partial sums.  0 = all SMs                  */
 } rt_config;
 
 /* Alg. 1 lines 4-8 (L348-L358): t = 0, P0 = diag(occ), rho0, vxc(rho0), V_H = 0,

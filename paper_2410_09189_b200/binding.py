@@ -56,7 +56,6 @@ class rt_config(C.Structure):
         ("history", C.c_int32),
         ("prop_shards", C.c_int32), ("prop_shard", C.c_int32),
         ("magnus_order", C.c_int32), ("xc_functional", C.c_int32), ("fd_order", C.c_int32),
-        ("sm_limit", C.c_int32),
     ]
 
 
@@ -378,7 +377,7 @@ class RTTDDFT:
     def __init__(self, shape, h, phi, eps, occ, dt, E0=(0.0, 0.0, 0.0), n_hupdates=2, n_vcycles=2, nu_pre=2,
                  nu_post=2, jacobi_omega=6.0 / 7.0, exp_order=0, hartree=True, xc=True, graph=True, tma=True,
                  device=0, stream=None, propagator="taylor", max_order=0, dP_thrs=0.0, H_thrs=0.0, max_hupdates=0,
-                 slab=None, history=0, prop_shard=None, magnus=1, xc_functional="lda", fd_order=2, sm_limit=0, Hks=None,
+                 slab=None, history=0, prop_shard=None, magnus=1, xc_functional="lda", fd_order=2, Hks=None,
                  P0=None, nonorthogonal=False):
         """``slab = (x0, nx_local)``: the handle owns those x-planes and ``phi`` is [norb][nx_local*ny*nz]
         (rt_slab_* entry points; see slab.py).  ``prop_shard = (rank, nranks)``: row-sharded N x N propagator.
@@ -391,7 +390,6 @@ class RTTDDFT:
         cfg.magnus_order = int(magnus)
         cfg.xc_functional = {"lda": RT_XC_LDA_PZ81, "pbe": RT_XC_PBE}[xc_functional]
         cfg.fd_order = int(fd_order)
-        cfg.sm_limit = int(sm_limit)
         cfg.propagator = {"taylor": RT_PROP_TAYLOR, "commutator": RT_PROP_COMMUTATOR}[propagator]
         cfg.max_order, cfg.dP_thrs, cfg.H_thrs, cfg.max_hupdates = int(max_order), float(dP_thrs), float(H_thrs), int(max_hupdates)
         cfg.nx, cfg.ny, cfg.nz = (int(s) for s in shape)

@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmPhiN,
                    const double* __restrict__ phi, const DensSeg* __restrict__ segs, double* __restrict__ rho_part,
                    int N, long long Ng, int ntypes, long long nrt, int group_r, int group_t, long long nwork,
-                   int b3d) {
+                   int b3d, int* __restrict__ pace_cnt, int pace_w, int hint) {
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -301,8 +301,9 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
       // the Phi panels of the r-tiles in flight are what the launch keeps in L2 (every type re-reads them); the fold
       // streams through (shared only by the group_r CTAs of the same type, which walk it together)
       const uint64_t pol_phi = l2_policy_evict_last();
-      const uint64_t pol_fold = l2_policy_evict_first();
       long long it = 0;
+      int misses = pace_cnt ? 0 : 2;
+      const int G = gridDim.x;
       for (long long L = blockIdx.x; L < nwork; L += gridDim.x) {
         const DensWork wk = dens_decode(L, ntypes, nrt, group_r, group_t);
         if (!wk.valid) continue;
@@ -311,19 +312,33 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
           const DensSeg sg = segs[2 * wk.type + which];
           const int j0 = sg.jt * TILE;
           for (int i = 0; i < sg.ns; ++i, ++it) {
+            if (misses < 2 && (it % PACE_CK) == 0) {                          // pacing: see project_tma_kernel
+              const long long q = it / PACE_CK;
+              atomicAdd(pace_cnt + q, 1);
+              if (q >= pace_w) {
+                const volatile int* prev = pace_cnt + (q - pace_w);
+                if (*prev < G) {
+                  const long long t0 = clock64();
+                  while (*prev < G) {
+                    if (clock64() - t0 > PACE_TIMEOUT_CLK) { ++misses; break; }
+                  }
+                }
+              }
+            }
             const int slot = (int)(it % ST);
             if (it >= ST) mbar_wait(smem_u32(&bars->empty[slot]), (uint32_t)((it / ST) - 1) & 1);
             const uint32_t full = smem_u32(&bars->full[slot]);
             mbar_expect_tx(full, 2 * TILE_BYTES);
             const int k0 = j0 + (sg.s0 + sg.dir * i) * BK;
             double* sA = tilesm + (size_t)slot * STAGE_D;
-            tma_load_2d_hint(sA, &tmP, k0, j0, full, pol_fold);               // Pfold[j0.., k0..]
+            tma_load_2d(sA, &tmP, k0, j0, full);                              // Pfold[j0.., k0..]
             if (b3d) {                                                        // Phi[k0.., r0 .. r0+127] in one op
-              tma_load_3d_hint(sA + TILE_D, &tmPhiN, 0, k0, (int)(r0 >> 4), full, pol_phi);
+              if (hint) tma_load_3d_hint(sA + TILE_D, &tmPhiN, 0, k0, (int)(r0 >> 4), full, pol_phi);
+              else tma_load_3d(sA + TILE_D, &tmPhiN, 0, k0, (int)(r0 >> 4), full);
             } else {
 #pragma unroll
               for (int bx = 0; bx < 8; ++bx)                                  // Phi[k0.., r0 + 16 bx ..]
-                tma_load_2d_hint(sA + TILE_D + bx * 256, &tmPhiN, (int)(r0 + 16 * bx), k0, full, pol_phi);
+                tma_load_2d(sA + TILE_D + bx * 256, &tmPhiN, (int)(r0 + 16 * bx), k0, full);
             }
           }
         }
@@ -435,13 +450,27 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
   }
 }
 
+size_t density_tma_pace_ints(const DensityPlan& p, int sms) {
+  const long long ngroups = (p.nrt + p.group_r - 1) / p.group_r;
+  const long long nwork = ngroups * p.group_r * p.ntypes;
+  const long long G = nwork < sms ? nwork : sms;
+  const long long per_item = (long long)(p.ntile + 1) * (TILE / BK) + 2;
+  const long long stages = ((nwork + G - 1) / G) * per_item;
+  if (G < 2 || p.ntile < PACE_MIN_NTILE || stages < PACE_MIN_STAGES) return 0;
+  return (size_t)(stages / PACE_CK + 2);
+}
+
 void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, int b3d,
-                        const double* phi, const DensSeg* segs, double* rho_part, int sms, cudaStream_t st) {
+                        const double* phi, const DensSeg* segs, double* rho_part, int sms, int* pace_cnt, int pace_w,
+                        int hint, cudaStream_t st) {
   const long long ngroups = (p.nrt + p.group_r - 1) / p.group_r;
   const long long nwork = ngroups * p.group_r * p.ntypes;
   const long long grid = nwork < sms ? nwork : sms;
+  const size_t npace = pace_cnt ? density_tma_pace_ints(p, sms) : 0;
+  if (npace) cudaMemsetAsync(pace_cnt, 0, npace * sizeof(int), st);
   density_tma_kernel<<<(unsigned)grid, NTHREADS, SMEM_TOTAL, st>>>(tmP, tmPhiN, phi, segs, rho_part, p.N, p.Ng,
-                                                                   p.ntypes, p.nrt, p.group_r, p.group_t, nwork, b3d);
+                                                                   p.ntypes, p.nrt, p.group_r, p.group_t, nwork, b3d,
+                                                                   npace ? pace_cnt : nullptr, pace_w, hint);
 }
 
 // ======================================================================================================

@@ -69,6 +69,8 @@ struct rt_ctx {
   double* gemm_ws = nullptr;      // stream-K fix-up workspace and flags of the TMA N x N GEMM (gemm_tma.cu)
   int* pace_cnt = nullptr;        // checkpoint counters of the paced projection launch (gemm_tma.cu), nullptr: not paced
   int pace_w = 1;                 // how many checkpoints a CTA may lead the slowest one by
+  bool dens_pace = false;         // pace the density launch too
+  int dens_hint = 0;              // evict_last hint on the density kernel's Phi loads
   int* gemm_sync = nullptr;
   // row-sharded propagator: rank `shard` of `nshard` owns the rows [row_beg, row_end) of every N x N product
   int nshard = 1, shard = 0, shard_rows = 0, row_beg = 0, row_end = 0;
@@ -201,29 +203,32 @@ bool can_coarsen(const GridDims& g) {
 
 // ---- a5 work types ---------------------------------------------------------------------------------
 // The triangular fold leaves j-tile jt with the contraction rows k >= jt*TILE, i.e. nk(jt) stages of 16.  Pair
-// (p, ntile-1-p) therefore always costs about (ntile + 1) tiles.  The time line of a pair is: short tile
-// ntile-1-p with k ascending to N, then long tile p with k descending from N (rows around the turn-around are
-// re-read while they are still in L2).  The time line is cut into `nsplit` pieces of equal length; each piece is a
-// work type (<= 2 segments) with its own partial-sum row.  nsplit > 1 puts more CTAs on the same r-tile, so fewer
-// r-tile panels of Phi are in flight: used when the folded P (4 N^2 bytes) is small enough to stay in L2 next to them.
+// (p, ntile-1-p) therefore always costs about (ntile + 1) tiles.  The time line of a pair is: LONG tile p with k
+// DESCENDING from N, then short tile ntile-1-p with k ASCENDING to N.  With that order the contraction row a CTA reads
+// at stage t of its item does not depend on the pair (first N - 16 (t + 1), then 16 t - (N - 128 (ntile - 1)) ... ): CTAs
+// that start their items together read the SAME Phi rows at the same time whatever their type, so the Phi tile of an
+// r-tile is fetched from DRAM once for all the types that run beside each other.  (Round 1 / first round-2 order --
+// short tile up, then long tile down -- made every type read its own rows: 7.2 TB of DRAM reads per launch at
+// N = 13,000, no reuse of Phi between types at all.)  The time line is cut into `nsplit` pieces of equal length; each
+// piece is a work type (<= 2 segments) with its own partial-sum row.
 void build_density_types(int N, int ntile, int nsplit, std::vector<DensSeg>& out) {
   out.clear();
   const int npairs = (ntile + 1) / 2;
   auto nk = [&](int jt) { return (N - jt * TILE + BK_HOST - 1) / BK_HOST; };
   for (int p = 0; p < npairs; ++p) {
     const int jb = ntile - 1 - p;
-    const int nkB = jb > p ? nk(jb) : 0, nkA = nk(p);
-    const int tot = nkB + nkA;
+    const int nkA = nk(p), nkB = jb > p ? nk(jb) : 0;
+    const int tot = nkA + nkB;
     for (int i = 0; i < nsplit; ++i) {
       const int t0 = (int)((long long)tot * i / nsplit), t1 = (int)((long long)tot * (i + 1) / nsplit);
-      DensSeg b{jb > p ? jb : p, 0, 0, 1}, a{p, 0, 0, -1};
-      if (t0 < nkB) { b.s0 = t0; b.ns = (t1 < nkB ? t1 : nkB) - t0; }
-      if (t1 > nkB) {
-        const int u0 = (t0 > nkB ? t0 : nkB) - nkB, u1 = t1 - nkB;
-        a.s0 = nkA - 1 - u0; a.ns = u1 - u0;
+      DensSeg a{p, 0, 0, -1}, b{jb > p ? jb : p, 0, 0, 1};
+      if (t0 < nkA) { a.s0 = nkA - 1 - t0; a.ns = (t1 < nkA ? t1 : nkA) - t0; }
+      if (t1 > nkA) {
+        const int u0 = (t0 > nkA ? t0 : nkA) - nkA, u1 = t1 - nkA;
+        b.s0 = u0; b.ns = u1 - u0;
       }
-      out.push_back(b);
       out.push_back(a);
+      out.push_back(b);
     }
   }
 }
@@ -490,7 +495,8 @@ void enqueue_propagate(rt_ctx* c, const double* Ar, const double* Ai, double* Or
 void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double* rho0) {
   launch_fold_upper(c->N, c->ldn, reP, c->X, c->st);
   if (c->use_tma)
-    launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phiN_3d, c->phi, c->d_segs, c->rho_part, c->sms, c->st);
+    launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phiN_3d, c->phi, c->d_segs, c->rho_part, c->sms,
+                       c->dens_pace ? c->pace_cnt : nullptr, c->pace_w, c->dens_hint, c->st);
   else launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
   launch_reduce_rho(c->rho_part, c->use_tma ? c->dp.ntypes : c->dp.npairs, c->Ngl, c->gd, c->h, c->x0, rho0, rho_out,
                     c->d_bsums, c->d_sums, c->st);
@@ -686,7 +692,6 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     return fail(c, RT_EINVAL, "rt_create: unknown xc_functional");
   if (cfg->fd_order != 0 && cfg->fd_order != 2 && cfg->fd_order != 4)
     return fail(c, RT_EINVAL, "rt_create: fd_order must be 0, 2 or 4");
-  if (cfg->sm_limit < 0) return fail(c, RT_EINVAL, "rt_create: sm_limit < 0");
   if (want_nonorth && !(Hks_in && P0re_in))
     return fail(c, RT_EINVAL, "rt_create: RT_NONORTHOGONAL needs the ground state as matrices (rt_create_general)");
   if (cfg->nx < 2 || cfg->ny < 2 || cfg->nz < 2) return fail(c, RT_EINVAL, "rt_create: grid dims must be >= 2");
@@ -827,7 +832,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     // full CTA costs kchunk/16, a narrow one 0.78 and a diagonal one 0.65 of that per stage (TMA kernel; measured), plus
     // a fixed prologue/epilogue per CTA and a term per split for the second-stage reduction.  (Wave quantisation was
     // 14 % of the first nano profile at S = 2.)
-    const int sms = (cfg->sm_limit > 0 && cfg->sm_limit < prop.multiProcessorCount) ? cfg->sm_limit : prop.multiProcessorCount;
+    const int sms = prop.multiProcessorCount;
     const bool tma_likely = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && get_encode_fn() != nullptr;
     const bool narrow = tma_likely && ntile > 1 && (N - (ntile - 1) * TILE) <= 96;
     p.Tn = narrow ? ntile - 1 : 0;
@@ -904,21 +909,24 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     const int nsplit = 1;
     build_density_types(N, ntile, nsplit, c->segs);
     d.ntypes = (int)(c->segs.size() / 2);
-    // Raster (gemm_tma.cu dens_decode): ALL types of a group of group_r r-tiles run before the next group starts, r-tile
-    // fastest.  What the launch keeps in L2 is the Phi column panel (N x 128 doubles) of every r-tile in flight -- each of
-    // the ntypes items of an r-tile re-reads its own k-range of that panel, at its own time, so only residency (TMA loads
-    // with the evict_last hint), not lock-step, makes the reuse happen -- while the fold streams through, shared by the
-    // group_r CTAs of one type that walk it together.  DRAM traffic ~ |Phi| + |P fold| * nrt / group_r, with group_r
-    // bounded by  group_r * panel <= ~40 MB  (the 126 MB L2 is two partitions that mirror remote lines).
-    // (Round-2 capture at N = 13,000 with 12 x 12 supertiles of types x r-tiles, which assumed that CTAs of different
-    // types share Phi tiles in lock-step -- they do not, their k-ranges differ: 7.2 TB of DRAM reads per launch.)
+    // Raster (gemm_tma.cu dens_decode): supertiles of group_t types x group_r r-tiles (~ one item per SM) run together and,
+    // all items having the same length, start their items together.  Inside a supertile a P-fold tile is fetched once for
+    // the group_r CTAs of its type and -- thanks to the type-independent k order above -- a Phi tile once for the group_t
+    // CTAs of its r-tile, in each of the two passes (down, up) over the contraction index:
+    //     DRAM bytes ~ 2 |Phi| ceil(ntypes / group_t) + |P fold| ceil(nrt / group_r)
+    // A fold that stays in L2 next to the tiles in flight (<= 24 MB) costs nothing to re-read: group_t = ntypes then.
     {
-      const double panel = (double)N * TILE * 8;
-      long long gr = (long long)(40.0e6 / panel);
-      if (gr > d.nrt) gr = d.nrt;
-      if (gr < 1) gr = 1;
-      d.group_t = d.ntypes;
-      d.group_r = (int)gr;
+      const double phi_b = (double)N * Ng * 8, pf_b = 0.5 * (double)N * ldn * 8;
+      double best_cost = 1e300;
+      d.group_t = 1; d.group_r = 1;
+      for (int gt = 1; gt <= d.ntypes && gt <= sms; ++gt) {
+        long long gr = sms / gt;
+        if (gr > d.nrt) gr = d.nrt;
+        if (gr < 1) gr = 1;
+        const double cost = 2.0 * phi_b * std::ceil((double)d.ntypes / gt) +
+                            (pf_b <= 24.0e6 ? 0.0 : pf_b * std::ceil((double)d.nrt / (double)gr));
+        if (cost < best_cost - 1.0) { best_cost = cost; d.group_t = gt; d.group_r = (int)gr; }
+      }
       if (const char* e = getenv("RT_DBG_GROUP_R")) d.group_r = std::max(1, atoi(e));
       if (const char* e = getenv("RT_DBG_GROUP_T")) d.group_t = std::max(1, std::min(d.ntypes, atoi(e)));
     }
@@ -948,7 +956,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     CKC(cudaMemcpyAsync(c->phi_owned, phi, (size_t)N * Ng * 8, cudaMemcpyHostToDevice, c->st));
     c->phi = c->phi_owned;
   }
-  c->sms = (cfg->sm_limit > 0 && cfg->sm_limit < prop.multiProcessorCount) ? cfg->sm_limit : prop.multiProcessorCount;
+  c->sms = prop.multiProcessorCount;
   if (const char* e = getenv("RT_DBG_PACE_W")) c->pace_w = std::max(1, atoi(e));
   if (getenv("RT_DBG_PERSIST_L2")) {
     cudaError_t pe = cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)prop.persistingL2CacheMaxSize);
@@ -1047,7 +1055,13 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
       for (int tj = ti; tj < ntile; ++tj) symrm.push_back(make_int2(ti, tj));
     ALLOC(c->d_tiles_sym, symrm.size());
     CKC(cudaMemcpyAsync(c->d_tiles_sym, symrm.data(), symrm.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
-    if (c->use_tma && project_tma_pace_ints(c->pp, c->sms) > 0 && !getenv("RT_DBG_NOPACE")) ALLOC(c->pace_cnt, project_tma_pace_ints(c->pp, c->sms));
+    c->dens_pace = getenv("RT_DBG_DENS_PACE") != nullptr;
+    c->dens_hint = getenv("RT_DBG_DENS_HINT") ? 1 : 0;
+    {
+      size_t np = c->use_tma && !getenv("RT_DBG_NOPACE") ? project_tma_pace_ints(c->pp, c->sms) : 0;
+      if (c->use_tma && c->dens_pace) np = std::max(np, density_tma_pace_ints(c->dp, c->sms));
+      if (np > 0) ALLOC(c->pace_cnt, np);
+    }
     if (c->use_tma && N > GEMM_SMALL_N) {
       ALLOC(c->gemm_ws, gemm_tma_ws_doubles(c->sms));
       ALLOC(c->gemm_sync, gemm_tma_sync_ints(c->sms));

@@ -104,8 +104,10 @@ void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const do
                         int sms, int* pace_cnt, int pace_w, cudaStream_t st);
 // tmP: Pfold [N][N] (ld = ldn) box {16, 128}; tmPhiN: Phi with box {16 r, 16 k-rows} (b3d = 0: 8 loads per stage)
 // or, when Ng % 16 == 0, the 3-D view {16 r-low, N k, Ng/16 r-high} with box {16, 16, 8} (b3d = 1: one load)
+size_t density_tma_pace_ints(const DensityPlan& p, int sms);
 void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUtensorMap& tmPhiN, int b3d,
-                        const double* phi, const DensSeg* segs, double* rho_part, int sms, cudaStream_t st);
+                        const double* phi, const DensSeg* segs, double* rho_part, int sms, int* pace_cnt, int pace_w,
+                        int hint, cudaStream_t st);
 // sym = +1 / -1: the product is known to be symmetric / antisymmetric (polynomials of the symmetric X commute; P1 is
 // Hermitian): only the upper tiles (list `tiles`, ti <= tj) are computed and the mirror image is written too
 // `tiles` / `ntiles`: the 128 x 128 output tiles of this launch (sym != 0: upper tiles only).  Stream-K: the (tile, stage)

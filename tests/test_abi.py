@@ -42,7 +42,7 @@ def test_config_struct_layout(built):
     assert binding.rt_config.history.offset == 148
     assert binding.rt_config.prop_shards.offset == 152 and binding.rt_config.prop_shard.offset == 156
     assert binding.rt_config.magnus_order.offset == 160 and binding.rt_config.xc_functional.offset == 164
-    assert binding.rt_config.fd_order.offset == 168 and binding.rt_config.sm_limit.offset == 172
+    assert binding.rt_config.fd_order.offset == 168
 
 
 def test_no_cpu_fallback(built):

@@ -51,7 +51,7 @@ def read_trajectory(name):
 
 # (golden case, workload, strong-kick amplitude, minimum number of steps the file must hold)
 CASES = [("tiny_weak", "tiny", None, 50), ("small_weak", "small", None, 1000), ("small_strong", "small", 0.1, 1000),
-         ("mid_laser", "mid", None, 100)]
+         ("mid_laser", "mid", None, 500)]
 
 
 @pytest.mark.parametrize("case,wname,amp,min_steps", CASES)
