@@ -74,7 +74,7 @@ constexpr long long PACE_TIMEOUT_CLK = 100000;      // ~50 us
 __global__ void __launch_bounds__(NTHREADS, 1)
 project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __restrict__ w,
                    const int2* __restrict__ tiles, double* __restrict__ W, const ProjectPlan pl, int nitems,
-                   int* __restrict__ pace_cnt, int pace_w) {
+                   int* __restrict__ pace_cnt, int pace_n, int pace_w) {
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -100,8 +100,9 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
         for (int kt = 0; kt < nk; ++kt, ++it) {
           if (misses < 2 && (it % PACE_CK) == 0) {
             const long long q = it / PACE_CK;
-            atomicAdd(pace_cnt + q, 1);
-            if (q >= pace_w) {
+            if (q >= pace_n) { misses = 2; }                 // past the counters (never with the host's bound): run free
+            else atomicAdd(pace_cnt + q, 1);
+            if (misses < 2 && q >= pace_w) {
               const volatile int* prev = pace_cnt + (q - pace_w);
               if (*prev < G) {
                 const long long t0 = clock64();
@@ -234,7 +235,10 @@ constexpr int PACE_MIN_NTILE = 32;
 size_t project_tma_pace_ints(const ProjectPlan& p, int sms) {
   const long long nitems = p.grid();
   const long long G = nitems < sms ? nitems : sms;
-  const long long per_item = (p.kchunk + BK - 1) / BK;               // the longest class
+  long long kc = p.kchunk;                                           // the class with the longest items
+  if (p.Tn > 0 && p.kchunk_n > kc) kc = p.kchunk_n;
+  if (p.kchunk_d > kc) kc = p.kchunk_d;
+  const long long per_item = (kc + BK - 1) / BK;
   const long long stages = ((nitems + G - 1) / G) * per_item;
   if (G < 2 || p.ntile < PACE_MIN_NTILE || stages < PACE_MIN_STAGES) return 0;
   return (size_t)(stages / PACE_CK + 2);
@@ -246,7 +250,8 @@ void launch_project_tma(const ProjectPlan& p, const CUtensorMap& tmPhi, const do
   const size_t npace = pace_cnt ? project_tma_pace_ints(p, sms) : 0;
   const int G = npace ? (nitems < sms ? nitems : sms) : nitems;
   if (npace) cudaMemsetAsync(pace_cnt, 0, npace * sizeof(int), st);
-  project_tma_kernel<<<G, NTHREADS, SMEM_TOTAL, st>>>(tmPhi, w, tiles, W, p, nitems, npace ? pace_cnt : nullptr, pace_w);
+  project_tma_kernel<<<G, NTHREADS, SMEM_TOTAL, st>>>(tmPhi, w, tiles, W, p, nitems, npace ? pace_cnt : nullptr, (int)npace,
+                                                      pace_w);
 }
 
 // ======================================================================================================
@@ -283,7 +288,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmPhiN,
                    const double* __restrict__ phi, const DensSeg* __restrict__ segs, double* __restrict__ rho_part,
                    int N, long long Ng, int ntypes, long long nrt, int group_r, int group_t, long long nwork,
-                   int b3d, int* __restrict__ pace_cnt, int pace_w, int hint) {
+                   int b3d, int* __restrict__ pace_cnt, int pace_n, int pace_w, int hint) {
   extern __shared__ uint8_t smem_raw[];
   double* tilesm = align1024(smem_raw);
   double* wsm = tilesm + (size_t)ST * STAGE_D;
@@ -314,8 +319,9 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
           for (int i = 0; i < sg.ns; ++i, ++it) {
             if (misses < 2 && (it % PACE_CK) == 0) {                          // pacing: see project_tma_kernel
               const long long q = it / PACE_CK;
-              atomicAdd(pace_cnt + q, 1);
-              if (q >= pace_w) {
+              if (q >= pace_n) { misses = 2; }
+              else atomicAdd(pace_cnt + q, 1);
+              if (misses < 2 && q >= pace_w) {
                 const volatile int* prev = pace_cnt + (q - pace_w);
                 if (*prev < G) {
                   const long long t0 = clock64();
@@ -456,7 +462,7 @@ size_t density_tma_pace_ints(const DensityPlan& p, int sms) {
   const long long G = nwork < sms ? nwork : sms;
   const long long per_item = (long long)(p.ntile + 1) * (TILE / BK) + 2;
   const long long stages = ((nwork + G - 1) / G) * per_item;
-  if (G < 2 || p.ntile < PACE_MIN_NTILE || stages < PACE_MIN_STAGES) return 0;
+  if (G < 2 || stages < PACE_MIN_STAGES) return 0;
   return (size_t)(stages / PACE_CK + 2);
 }
 
@@ -470,7 +476,7 @@ void launch_density_tma(const DensityPlan& p, const CUtensorMap& tmP, const CUte
   if (npace) cudaMemsetAsync(pace_cnt, 0, npace * sizeof(int), st);
   density_tma_kernel<<<(unsigned)grid, NTHREADS, SMEM_TOTAL, st>>>(tmP, tmPhiN, phi, segs, rho_part, p.N, p.Ng,
                                                                    p.ntypes, p.nrt, p.group_r, p.group_t, nwork, b3d,
-                                                                   npace ? pace_cnt : nullptr, pace_w, hint);
+                                                                   npace ? pace_cnt : nullptr, (int)npace, pace_w, hint);
 }
 
 // ======================================================================================================

@@ -6,7 +6,6 @@
 
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <cstdio>
 #include <cstring>
 #include <map>
@@ -69,8 +68,7 @@ struct rt_ctx {
   double* gemm_ws = nullptr;      // stream-K fix-up workspace and flags of the TMA N x N GEMM (gemm_tma.cu)
   int* pace_cnt = nullptr;        // checkpoint counters of the paced projection launch (gemm_tma.cu), nullptr: not paced
   int pace_w = 1;                 // how many checkpoints a CTA may lead the slowest one by
-  bool dens_pace = false;         // pace the density launch too
-  int dens_hint = 0;              // evict_last hint on the density kernel's Phi loads
+  bool dens_resident = false;     // density raster regime (a): fold resident in L2, Phi panels kept with evict_last
   int* gemm_sync = nullptr;
   // row-sharded propagator: rank `shard` of `nshard` owns the rows [row_beg, row_end) of every N x N product
   int nshard = 1, shard = 0, shard_rows = 0, row_beg = 0, row_end = 0;
@@ -211,7 +209,10 @@ bool can_coarsen(const GridDims& g) {
 // short tile up, then long tile down -- made every type read its own rows: 7.2 TB of DRAM reads per launch at
 // N = 13,000, no reuse of Phi between types at all.)  The time line is cut into `nsplit` pieces of equal length; each
 // piece is a work type (<= 2 segments) with its own partial-sum row.
-void build_density_types(int N, int ntile, int nsplit, std::vector<DensSeg>& out) {
+// aligned = false keeps the round-1 order (short tile up, then long tile down: the rows around the turn-around are re-read
+// while still in L2), which measured better when the Phi panels in flight are held in L2 anyway (regime (a) of the raster
+// below: nano 72 GB / 344.9 ms per launch against 280 GB / 351.9 ms with the aligned order).
+void build_density_types(int N, int ntile, int nsplit, bool aligned, std::vector<DensSeg>& out) {
   out.clear();
   const int npairs = (ntile + 1) / 2;
   auto nk = [&](int jt) { return (N - jt * TILE + BK_HOST - 1) / BK_HOST; };
@@ -222,13 +223,23 @@ void build_density_types(int N, int ntile, int nsplit, std::vector<DensSeg>& out
     for (int i = 0; i < nsplit; ++i) {
       const int t0 = (int)((long long)tot * i / nsplit), t1 = (int)((long long)tot * (i + 1) / nsplit);
       DensSeg a{p, 0, 0, -1}, b{jb > p ? jb : p, 0, 0, 1};
-      if (t0 < nkA) { a.s0 = nkA - 1 - t0; a.ns = (t1 < nkA ? t1 : nkA) - t0; }
-      if (t1 > nkA) {
-        const int u0 = (t0 > nkA ? t0 : nkA) - nkA, u1 = t1 - nkA;
-        b.s0 = u0; b.ns = u1 - u0;
+      if (aligned) {                       // long tile down, then short tile up
+        if (t0 < nkA) { a.s0 = nkA - 1 - t0; a.ns = (t1 < nkA ? t1 : nkA) - t0; }
+        if (t1 > nkA) {
+          const int u0 = (t0 > nkA ? t0 : nkA) - nkA, u1 = t1 - nkA;
+          b.s0 = u0; b.ns = u1 - u0;
+        }
+        out.push_back(a);
+        out.push_back(b);
+      } else {                             // short tile up, then long tile down
+        if (t0 < nkB) { b.s0 = t0; b.ns = (t1 < nkB ? t1 : nkB) - t0; }
+        if (t1 > nkB) {
+          const int u0 = (t0 > nkB ? t0 : nkB) - nkB, u1 = t1 - nkB;
+          a.s0 = nkA - 1 - u0; a.ns = u1 - u0;
+        }
+        out.push_back(b);
+        out.push_back(a);
       }
-      out.push_back(a);
-      out.push_back(b);
     }
   }
 }
@@ -496,7 +507,7 @@ void enqueue_density(rt_ctx* c, const double* reP, double* rho_out, const double
   launch_fold_upper(c->N, c->ldn, reP, c->X, c->st);
   if (c->use_tma)
     launch_density_tma(c->dp, nn_map(c, c->X), c->tmPhiN, c->phiN_3d, c->phi, c->d_segs, c->rho_part, c->sms,
-                       c->dens_pace ? c->pace_cnt : nullptr, c->pace_w, c->dens_hint, c->st);
+                       c->dens_resident ? nullptr : c->pace_cnt, c->pace_w, c->dens_resident ? 1 : 0, c->st);
   else launch_density(c->dp, c->phi, c->X, c->rho_part, c->st);
   launch_reduce_rho(c->rho_part, c->use_tma ? c->dp.ntypes : c->dp.npairs, c->Ngl, c->gd, c->h, c->x0, rho0, rho_out,
                     c->d_bsums, c->d_sums, c->st);
@@ -907,28 +918,38 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     // that fewer Phi panels are in flight, was measured on nano: 4 pieces -> 397 ms and 277 GB of DRAM reads against
     // 364 ms and 191 GB for whole pairs; the extra epilogues and pipeline refills cost more than the locality buys.)
     const int nsplit = 1;
-    build_density_types(N, ntile, nsplit, c->segs);
+    c->dens_resident = 0.5 * (double)N * ldn * 8 <= 24.0e6;          // the fold stays in L2: raster regime (a) below
+    build_density_types(N, ntile, nsplit, !c->dens_resident, c->segs);
     d.ntypes = (int)(c->segs.size() / 2);
-    // Raster (gemm_tma.cu dens_decode): supertiles of group_t types x group_r r-tiles (~ one item per SM) run together and,
-    // all items having the same length, start their items together.  Inside a supertile a P-fold tile is fetched once for
-    // the group_r CTAs of its type and -- thanks to the type-independent k order above -- a Phi tile once for the group_t
-    // CTAs of its r-tile, in each of the two passes (down, up) over the contraction index:
-    //     DRAM bytes ~ 2 |Phi| ceil(ntypes / group_t) + |P fold| ceil(nrt / group_r)
-    // A fold that stays in L2 next to the tiles in flight (<= 24 MB) costs nothing to re-read: group_t = ntypes then.
+    // Raster (gemm_tma.cu dens_decode), two regimes, both measured with ncu (profiles/r2_traffic.md):
+    // (a) the fold stays in L2 (<= 24 MB, N <= ~2,400): ALL types of a small group of r-tiles run side by side and the Phi
+    //     column panels of the r-tiles in flight are kept resident with the evict_last hint on their TMA loads -- every
+    //     type re-reads its own k-range of a panel at its own time, and re-reading the fold costs nothing.
+    //     nano: 72 GB of DRAM reads per launch (Phi = 40 GB) against 238 GB for the round-1 raster.
+    // (b) larger N: the fold streams, the L2 cannot hold panels of N rows for the ~2 ms an item lives (measured: hints or
+    //     not, 7.1-7.6 TB per launch at N = 13,000 = every item fetching its own panel).  Supertiles of group_t types x
+    //     group_r r-tiles (~ one item per SM) then run in LOCK-STEP (producer pacing, gemm_tma.cu): a fold tile is fetched
+    //     once for the group_r CTAs of its type and -- thanks to the type-independent k order of build_density_types -- a
+    //     Phi tile once for the group_t CTAs of its r-tile, in each of the two passes (down, up) over k:
+    //         DRAM bytes ~ 2 |Phi| ceil(ntypes / group_t) + |P fold| ceil(nrt / group_r)
+    //     24k: 1.25 TB per launch against 7.2 TB, L2 hit rate 78 % against 34 %, kernel time +0.5 %.
     {
-      const double phi_b = (double)N * Ng * 8, pf_b = 0.5 * (double)N * ldn * 8;
-      double best_cost = 1e300;
-      d.group_t = 1; d.group_r = 1;
-      for (int gt = 1; gt <= d.ntypes && gt <= sms; ++gt) {
-        long long gr = sms / gt;
-        if (gr > d.nrt) gr = d.nrt;
-        if (gr < 1) gr = 1;
-        const double cost = 2.0 * phi_b * std::ceil((double)d.ntypes / gt) +
-                            (pf_b <= 24.0e6 ? 0.0 : pf_b * std::ceil((double)d.nrt / (double)gr));
-        if (cost < best_cost - 1.0) { best_cost = cost; d.group_t = gt; d.group_r = (int)gr; }
+      const double phi_b = (double)N * Ng * 8, pf_b = 0.5 * (double)N * ldn * 8, panel = (double)N * TILE * 8;
+      if (c->dens_resident) {
+        long long gr = (long long)(10.0e6 / panel);
+        d.group_t = d.ntypes;
+        d.group_r = (int)std::max(1LL, std::min((long long)d.nrt, gr));
+      } else {
+        double best_cost = 1e300;
+        d.group_t = 1; d.group_r = 1;
+        for (int gt = 1; gt <= d.ntypes && gt <= sms; ++gt) {
+          long long gr = sms / gt;
+          if (gr > d.nrt) gr = d.nrt;
+          if (gr < 1) gr = 1;
+          const double cost = 2.0 * phi_b * std::ceil((double)d.ntypes / gt) + pf_b * std::ceil((double)d.nrt / (double)gr);
+          if (cost < best_cost - 1.0) { best_cost = cost; d.group_t = gt; d.group_r = (int)gr; }
+        }
       }
-      if (const char* e = getenv("RT_DBG_GROUP_R")) d.group_r = std::max(1, atoi(e));
-      if (const char* e = getenv("RT_DBG_GROUP_T")) d.group_t = std::max(1, std::min(d.ntypes, atoi(e)));
     }
   }
 
@@ -957,11 +978,6 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     c->phi = c->phi_owned;
   }
   c->sms = prop.multiProcessorCount;
-  if (const char* e = getenv("RT_DBG_PACE_W")) c->pace_w = std::max(1, atoi(e));
-  if (getenv("RT_DBG_PERSIST_L2")) {
-    cudaError_t pe = cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)prop.persistingL2CacheMaxSize);
-    fprintf(stderr, "persisting L2 limit %d bytes -> %s\n", prop.persistingL2CacheMaxSize, cudaGetErrorString(pe));
-  }
   c->use_tma = !(cfg->flags & RT_NO_TMA) && (Ng % 2 == 0) && ((reinterpret_cast<uintptr_t>(c->phi) & 15) == 0) &&
                get_encode_fn() != nullptr;
   if (c->use_tma) {
@@ -1055,11 +1071,10 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
       for (int tj = ti; tj < ntile; ++tj) symrm.push_back(make_int2(ti, tj));
     ALLOC(c->d_tiles_sym, symrm.size());
     CKC(cudaMemcpyAsync(c->d_tiles_sym, symrm.data(), symrm.size() * sizeof(int2), cudaMemcpyHostToDevice, c->st));
-    c->dens_pace = getenv("RT_DBG_DENS_PACE") != nullptr;
-    c->dens_hint = getenv("RT_DBG_DENS_HINT") ? 1 : 0;
-    {
-      size_t np = c->use_tma && !getenv("RT_DBG_NOPACE") ? project_tma_pace_ints(c->pp, c->sms) : 0;
-      if (c->use_tma && c->dens_pace) np = std::max(np, density_tma_pace_ints(c->dp, c->sms));
+    if (c->use_tma) {
+      // checkpoint counters of the paced launches (one array serves both kernels: they never run together on a handle)
+      const size_t np = std::max(project_tma_pace_ints(c->pp, c->sms),
+                                 c->dens_resident ? (size_t)0 : density_tma_pace_ints(c->dp, c->sms));
       if (np > 0) ALLOC(c->pace_cnt, np);
     }
     if (c->use_tma && N > GEMM_SMALL_N) {
