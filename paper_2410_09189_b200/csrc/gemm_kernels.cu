@@ -111,7 +111,17 @@ __global__ void project_reduce_kernel(const double* __restrict__ W, const double
   double sum = 0.0;
   // diagonal tiles and the tiles of a narrow last column have their own split counts (ProjectPlan)
   const int ns = (i / TILE == j / TILE) ? Sd : (j / TILE == narrow_tile ? Sn : S);
-  for (int s = 0; s < ns; ++s) sum += p[(long long)s * slab];
+  // 16 loads in flight per thread, added in split order (with one load per add the kernel is a chain of ns L2 round
+  // trips: 67 us for the 148 splits of `small`, 9 % of its step)
+  int s = 0;
+  for (; s + 16 <= ns; s += 16) {
+    double v[16];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) v[u] = p[(long long)(s + u) * slab];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) sum += v[u];
+  }
+  for (; s < ns; ++s) sum += p[(long long)s * slab];
   double v = scale * sum;
   if (i == j && eps) v += eps[i];
   if (Hadd) v += Hadd[(long long)i * ldn + j];

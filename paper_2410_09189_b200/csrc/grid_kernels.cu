@@ -551,6 +551,29 @@ void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, d
   series_init_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, Y, C, c1, S, s1);
 }
 
+// cos / sinc series from the stored powers of Y = X^2:  C = 1 + sum_k c_k Y^k,  Sc = 1 + sum_k s_k Y^k  (k = 1..q), summed
+// in the order k = 1, 2, ... -- the same order, and the same operations, as series_init_kernel followed by the
+// read-modify-write accumulation in the GEMM epilogues that this kernel replaces.
+__global__ void series_combine_kernel(int N, int ldn, SeriesArgs a, double* __restrict__ C, double* __restrict__ S) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j >= N) return;
+  const long long o = (long long)i * ldn + j;
+  const double d = (i == j) ? 1.0 : 0.0;
+  const double y1 = a.pw[0][o];
+  double cv = d + a.c[0] * y1, sv = d + a.s[0] * y1;
+#pragma unroll 1
+  for (int k = 1; k < a.q; ++k) {
+    const double y = a.pw[k][o];
+    cv += a.c[k] * y;
+    sv += a.s[k] * y;
+  }
+  C[o] = cv;
+  S[o] = sv;
+}
+void launch_series_combine(int N, int ldn, const SeriesArgs& a, double* C, double* S, cudaStream_t st) {
+  series_combine_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, a, C, S);
+}
+
 // Line 28 shifts H-1 <- H0 and H0 <- H1 in ONE launch, so H0 is both a source and a destination: no __restrict__
 // here, and every element is read into registers before any store.
 __global__ void copy4_kernel(long long n, double* d0, const double* s0, double* d1, const double* s1, double* d2,

@@ -149,3 +149,39 @@ def test_spectrum_kick_forms_the_impulse_inside_the_library(B):
     S = B.rt_spectrum_kick(mu, dt, E, 0.02, omega)
     ref = O.dipole_strength(mu, dt, 0.5 * dt, tuple(0.5 * e * dt for e in E), 0.02, omega)
     assert np.max(np.abs(S - ref)) < 1e-12 * np.max(np.abs(ref))
+
+
+@pytest.mark.parametrize("N", [2400, 5000])
+def test_propagator_is_bit_reproducible_and_accurate(B, N):
+    """The stream-K N x N GEMMs fix their summation order by (N, #SMs) alone: the same propagation, run four times through
+    rt_op_propagate, must give the same bits (a round-2 epilogue variant that batched the read-modify-writes of the series
+    accumulators failed exactly this at N >= 5,000 while staying within 1e-9 of the right answer), and the right answer:
+    U P0 U^dagger with U = exp(-i dt H) from torch.linalg.matrix_exp in complex128 -- a library routine, not oracle/
+    (its eigendecomposition of 5,000^2 would take minutes on the host), hence kept apart from the parity tests."""
+    import torch
+    Ng = 16 ** 3
+    gen = torch.Generator(device="cuda").manual_seed(1234 + N)
+    phi = torch.randn(N, Ng, dtype=torch.float64, device="cuda", generator=gen) * 0.1     # only sizes the handle
+    rng = np.random.default_rng(N)
+    eps = np.sort(rng.uniform(-0.5, 0.3, N))
+    occ = np.zeros(N)
+    occ[: (5 * N) // 6] = 2.0
+    sim = B.RTTDDFT((16, 16, 16), 0.4, phi, eps, occ, 0.2, E0=(0.05, 0.0, 0.0), n_hupdates=1, n_vcycles=1)
+    assert sim.info()["tma"]
+    A = torch.randn(N, N, dtype=torch.float64, device="cuda", generator=gen) * 2e-3
+    H = torch.diag(torch.from_numpy(eps).cuda()) + 0.5 * (A + A.T)
+    Hh = H.cpu().numpy()
+    P0r, P0i = np.diag(occ), np.zeros((N, N))
+    outs = []
+    for _ in range(4):
+        P1r, P1i = np.empty((N, N)), np.empty((N, N))
+        B.rt_op_propagate(sim.handle, Hh, P0r, P0i, P1r, P1i)
+        outs.append((P1r, P1i))
+    for P1r, P1i in outs[1:]:
+        assert np.array_equal(P1r, outs[0][0]) and np.array_equal(P1i, outs[0][1])
+    U = torch.linalg.matrix_exp((-0.2j) * H.to(torch.complex128))
+    Pref = (U * torch.from_numpy(occ).cuda().to(torch.complex128)[None, :]) @ U.conj().T
+    P1 = torch.from_numpy(outs[0][0]).cuda() + 1j * torch.from_numpy(outs[0][1]).cuda()
+    assert float((P1 - Pref).abs().max()) < 1e-11
+    assert float((P1 @ P1 - 2 * P1).abs().max()) < 1e-11
+    sim.close()
