@@ -179,7 +179,8 @@ int rt_get_time(rt_handle h, double* t);
 int rt_get_charge(rt_handle h, double q[2]);
 /* info[0] = exp_order K actually used, info[1] = number of multigrid levels, info[2..4] = coarsest nx,ny,nz,
  * info[5] = 1 if steps (or slab phases) replay a CUDA graph, +2 if the TMA-fed DMMA kernels are in use, +4 if a slab
- * phase capture was ever invalidated from outside (that phase was then enqueued directly), info[6] = kernels launched
+ * phase capture was ever invalidated from outside (that phase was then enqueued directly), +8 / +16 if the projection /
+ * density launches run persistent CTAs in lock-step (producer pacing, large systems only), info[6] = kernels launched
  * per step, info[7] = split-K of the projection.  HOST int32[8]. */
 int rt_get_info(rt_handle h, int32_t info[8]);
 /* Total number of this library's kernel launches enqueued through the handle so far (graph replays count the

@@ -213,6 +213,7 @@ def rt_get_info(h) -> dict:
     _check(h, _lib.rt_get_info(h, a.ctypes.data))
     return {"exp_order": int(a[0]), "mg_levels": int(a[1]), "coarsest": (int(a[2]), int(a[3]), int(a[4])),
             "graph": bool(a[5] & 1), "tma": bool(a[5] & 2), "capture_retried": bool(a[5] & 4),
+            "paced_projection": bool(a[5] & 8), "paced_density": bool(a[5] & 16),
             "launches_per_step": int(a[6]),
             "project_split_k": int(a[7])}
 

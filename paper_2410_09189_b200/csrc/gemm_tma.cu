@@ -153,11 +153,10 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
         for (int b = 0; b < FB3; ++b) acc3[a][b][0] = acc3[a][b][1] = 0.0;
       for (int kt = 0; kt < nk; ++kt, ++it) {
         const int slot = (int)(it % ST);
-        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        mbar_wait_warp(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
         const double* sA = tilesm + (size_t)slot * STAGE_D;
         mma_stage_kc_tma<FA, FB3, true>(acc3, sA, sA + TILE_D, wsm + slot * BK, wrow3, wcol3, pg, c);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+        release_stage(smem_u32(&bars->empty[slot]), lane);
       }
 #pragma unroll
       for (int a = 0; a < FA; ++a) {
@@ -187,24 +186,22 @@ project_tma_kernel(const __grid_constant__ CUtensorMap tmPhi, const double* __re
     if (!diag) {
       for (int kt = 0; kt < nk; ++kt, ++it) {
         const int slot = (int)(it % ST);
-        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        mbar_wait_warp(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
         const double* sA = tilesm + (size_t)slot * STAGE_D;
         mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+        release_stage(smem_u32(&bars->empty[slot]), lane);
       }
     } else {
       const bool live = i0 + wrow < N && j0 + wcol < N;
       for (int kt = 0; kt < nk; ++kt, ++it) {
         const int slot = (int)(it % ST);
-        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        mbar_wait_warp(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
         const double* sA = tilesm + (size_t)slot * STAGE_D;
         if (!live) {}                             // the whole warp tile is padding (N < 128: tiny systems)
         else if (dlt >= 8) mma_stage_kc_tma<FA, FB, true>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
         else if (dlt == 4) mma_stage_kc_tma<FA, FB, true, 6, 8>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
         else if (dlt == 0) mma_stage_kc_tma<FA, FB, true, 2, 4>(acc, sA, sA + TILE_D, wsm + slot * BK, wrow, wcol, pg, c);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+        release_stage(smem_u32(&bars->empty[slot]), lane);
       }
     }
 
@@ -383,7 +380,7 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
 
       for (int i = 0; i < sg.ns; ++i, ++it) {
         const int slot = (int)(it % ST);
-        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        mbar_wait_warp(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
         const double* sA = tilesm + (size_t)slot * STAGE_D;
         // stage sidx holds the contraction rows k = j0 + 16 sidx ...: inside the diagonal block (sidx < 8) the fold is
         // upper triangular, Pfold[j][k] = 0 for k < j, so row block a of this warp is all zeros in half `half` of the
@@ -394,8 +391,7 @@ density_tma_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constan
         else if (na == 6) mma_stage_nc_tma<FA, FB, 6>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
         else if (na == 4) mma_stage_nc_tma<FA, FB, 4>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
         else if (na == 2) mma_stage_nc_tma<FA, FB, 2>(acc, sA, sA + TILE_D, wrow, wcol, g, pg, c);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+        release_stage(smem_u32(&bars->empty[slot]), lane);
       }
 
       // fused row-dot: colsum(r) += sum_j phi_j(r) T_j(r); lane owns columns wcol + 16 t + 4 c + {0..3}
@@ -604,7 +600,7 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
 
       for (int kt = kt0; kt < kt1; ++kt, ++it) {
         const int slot = (int)(it % ST);
-        mbar_wait(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
+        mbar_wait_warp(smem_u32(&bars->full[slot]), (uint32_t)(it / ST) & 1);
         if (kt == nk1 && ratio != 1.0) {            // fold alpha1/alpha0 into the first term's sum
 #pragma unroll
           for (int a = 0; a < FA; ++a)
@@ -613,8 +609,7 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
         }
         const double* sA = tilesm + (size_t)slot * STAGE_D;
         mma_stage_kc_tma<FA, FB, false>(acc, sA, sA + TILE_D, nullptr, wrow, wcol, pg, c);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&bars->empty[slot]));
+        release_stage(smem_u32(&bars->empty[slot]), lane);
       }
       if (ga.nterms == 2 && ratio != 1.0 && kt1 <= nk1) {      // the item never reached the second term
 #pragma unroll
@@ -665,11 +660,10 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
       }
 
       // ---- epilogue of a complete tile ----
-      // Every element is finished (D stored, Z1 / Z2 read, updated and stored) before the next one is touched.  A version
-      // that read Z1 / Z2 for a batch of fragments first and stored afterwards ran the accumulating products 30 % faster
-      // (the read-modify-writes are one dependent L2 round trip each) but gave results that changed from call to call at
-      // N >= 5,000 -- single rows of a power of Y off by 1e-17 ... 1e-10, gone with CUDA_LAUNCH_BLOCKING=1, cause not
-      // found -- so the order that is bit-reproducible in every test stays.
+      // Every element is finished (D stored, Z1 / Z2 read, updated and stored) before the next one is touched: one
+      // dependent L2 round trip per read-modify-write, 70 % of the DMMA pipe against 91 % without Z.  The Taylor chain
+      // therefore no longer accumulates here (rt_api.cu enqueue_expm keeps the powers); the commutator series and the
+      // row-sharded propagator still do.
       const bool diag = ga.sym && i0 == j0;
 #pragma unroll
       for (int a = 0; a < FA; ++a) {

@@ -1228,34 +1228,48 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
     if (c->use_graph && !c->slab) {
       // capture on a private stream (the caller's may be the legacy default stream, which cannot capture);
       // the instantiated graph is replayed on the caller's stream
+      // A capture can be invalidated from outside the library (another host thread of the process; seen with several
+      // handles driven by host threads on one GPU): it is retried, and after three failures the handle simply launches
+      // its kernels directly -- the graph is an optimisation, not a requirement.
       cudaStream_t user = c->st, cap = nullptr;
       CKC(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
       c->st = cap;
       cudaError_t e = cudaSuccess;
-      if (!c->dynamic) {
-        e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
-        if (e == cudaSuccess) {
-          enqueue_step(c);
-          e = cudaStreamEndCapture(cap, &c->graph);
-        }
-        c->launches_per_step = c->launches - before;
-      } else {
-        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
-          const int64_t b0 = c->launches;
+      for (int attempt = 0; attempt < 3; ++attempt) {
+        e = cudaSuccess;
+        c->launches = before;
+        if (!c->dynamic) {
           e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
           if (e == cudaSuccess) {
-            enqueue_update(c, i);
-            e = cudaStreamEndCapture(cap, &c->graph_upd[i]);
+            enqueue_step(c);
+            e = cudaStreamEndCapture(cap, &c->graph);
           }
-          c->launches_per_upd[i] = c->launches - b0;
+          c->launches_per_step = c->launches - before;
+        } else {
+          for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+            const int64_t b0 = c->launches;
+            e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+            if (e == cudaSuccess) {
+              enqueue_update(c, i);
+              e = cudaStreamEndCapture(cap, &c->graph_upd[i]);
+            }
+            c->launches_per_upd[i] = c->launches - b0;
+          }
         }
+        if (e == cudaSuccess) break;
+        cudaGetLastError();
+        c->capture_failures += 1;
+        if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
+        for (int i = 0; i < 2; ++i)
+          if (c->graph_upd[i]) { cudaGraphDestroy(c->graph_upd[i]); c->graph_upd[i] = nullptr; }
       }
       c->st = user;
       cudaStreamDestroy(cap);
-      if (e != cudaSuccess) { cudaGetLastError(); FAIL_CREATE(RT_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
-      if (c->graph) CKC(cudaGraphInstantiate(&c->gexec, c->graph, 0));
-      for (int i = 0; i < 2; ++i)
-        if (c->graph_upd[i]) CKC(cudaGraphInstantiate(&c->gexec_upd[i], c->graph_upd[i], 0));
+      if (e == cudaSuccess) {
+        if (c->graph) CKC(cudaGraphInstantiate(&c->gexec, c->graph, 0));
+        for (int i = 0; i < 2; ++i)
+          if (c->graph_upd[i]) CKC(cudaGraphInstantiate(&c->gexec_upd[i], c->graph_upd[i], 0));
+      }
     }
     c->launches = before;
   }
@@ -1578,7 +1592,9 @@ int rt_get_info(rt_handle c, int32_t info[8]) {
   info[0] = 2 * c->q + 1;
   info[1] = (int32_t)c->lv.size();
   info[2] = L.gd.nx; info[3] = L.gd.ny; info[4] = L.gd.nz;
-  info[5] = ((c->gexec || !c->phase_exec.empty()) ? 1 : 0) | (c->use_tma ? 2 : 0) | (c->capture_failures > 0 ? 4 : 0);
+  info[5] = ((c->gexec || !c->phase_exec.empty()) ? 1 : 0) | (c->use_tma ? 2 : 0) | (c->capture_failures > 0 ? 4 : 0) |
+            ((c->use_tma && c->pace_cnt && project_tma_pace_ints(c->pp, c->sms) > 0) ? 8 : 0) |
+            ((c->use_tma && c->pace_cnt && !c->dens_resident && density_tma_pace_ints(c->dp, c->sms) > 0) ? 16 : 0);
   info[6] = (int32_t)c->launches_per_step;
   info[7] = c->pp.S;
   return RT_OK;

@@ -43,12 +43,22 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
   return ok != 0;
 }
-// Waits for the phase with the given parity.  A pipeline bug would otherwise hang the GPU until the driver's
+// Waits for the phase with the given parity (single-thread callers: the TMA producer).  A pipeline bug would otherwise hang the GPU until the driver's
 // watchdog fires, so after ~10 s of polling the kernel traps (the launch then fails loudly with a CUDA error).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   const long long t0 = clock64();
   while (!mbar_try_wait(bar, parity)) {
+    if (clock64() - t0 > 20000000000LL) __trap();
+  }
+}
+// The same for a whole (converged) consumer warp in front of warp-level MMAs: every lane polls, and the vote makes the
+// exit from the polling loop warp-uniform (the compiler emits no reconvergence point between the loop and the stage's
+// mma.sync, which must be executed by the whole warp together).
+__device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity) {
+  if (__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) return;
+  const long long t0 = clock64();
+  while (!__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) {
     if (clock64() - t0 > 20000000000LL) __trap();
   }
 }
@@ -105,6 +115,20 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
 // barrier among the consumer warps only (named barrier 1)
 __device__ __forceinline__ void consumer_sync(int nthreads) {
   asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+}
+
+// Consumer side of the ring: hand a stage back to the producer.  The fence is what makes this safe.  ptxas schedules the
+// arrive BEFORE the last DMMAs of the stage (SASS: SYNCS.ARRIVE followed by 24 DMMA.8x8x4), and the scoreboard wait for the
+// last fragment loads sits at their first use -- after the arrive.  The LDS of those fragments can therefore still be in
+// flight when the eighth arrival lets the producer's next TMA overwrite the slot, and they then return the NEW tile:
+// rows 48-63 of a warp tile (the last A fragments) built from the wrong grid points, once every few thousand stages when
+// the producer is already waiting for the slot.  __threadfence_block (MEMBAR.CTA) completes every earlier load of the
+// lane; __syncwarp extends that to the warp; then one lane arrives.  Latent since round 1; it surfaced in round 2 when
+// producer pacing (and, in the N x N GEMM, a faster epilogue) changed who waits for whom.
+__device__ __forceinline__ void release_stage(uint32_t empty_bar, int lane) {
+  __threadfence_block();
+  __syncwarp();
+  if (lane == 0) mbar_arrive(empty_bar);
 }
 
 __device__ __forceinline__ int perm8(int g) { return (g >> 1) | ((g & 1) << 2); }

@@ -185,3 +185,47 @@ def test_propagator_is_bit_reproducible_and_accurate(B, N):
     assert float((P1 - Pref).abs().max()) < 1e-11
     assert float((P1 @ P1 - 2 * P1).abs().max()) < 1e-11
     sim.close()
+
+
+def test_paced_kernels_give_the_same_bits_alone_and_beside_another_handle(B):
+    """Large systems run the projection and the density with persistent CTAs kept in lock-step by producer pacing
+    (gemm_tma.cu).  Pacing only delays TMA issue, so it must not change a bit of the result -- neither from run to run
+    (a held-back producer makes the consumer warps poll their barriers: this test is what exposed the divergent-warp race
+    fixed by mbar_wait_warp) nor when the peers a CTA waits for are not resident because a second
+    handle on another stream holds SMs (bounded waits, then the CTA runs free).  N = 4,096 on a 48 x 48 x 40 grid is the
+    smallest shape on which both kernels pace."""
+    import threading
+    import torch
+    N, shape, h, dt = 4096, (48, 48, 40), 0.4, 0.1
+    Ng = shape[0] * shape[1] * shape[2]
+    gen = torch.Generator(device="cuda").manual_seed(77)
+    phi = torch.randn(N, Ng, dtype=torch.float64, device="cuda", generator=gen)
+    phi *= 1.0 / (phi.norm(dim=1, keepdim=True) * (h ** 3) ** 0.5)           # normalised, not orthogonal: sizes only
+    torch.cuda.synchronize()                  # the handles below run on their own streams
+    rng = np.random.default_rng(5)
+    eps = np.sort(rng.uniform(-0.5, 0.3, N))
+    occ = np.zeros(N)
+    occ[: N // 2] = 2.0
+    kw = dict(E0=(1e-3, 0.0, 0.0), n_hupdates=2, n_vcycles=2)
+
+    def run(stream, out, key):
+        with torch.cuda.stream(stream):
+            sim = B.RTTDDFT(shape, h, phi, eps, occ, dt, stream=stream.cuda_stream, **kw)
+            info = sim.info()
+            sim.step(2)
+            out[key] = (sim.density().copy(), sim.hmatrix().copy(), info)
+            sim.close()
+
+    res = {}
+    run(torch.cuda.Stream(), res, "alone")
+    assert res["alone"][2]["paced_projection"] and res["alone"][2]["paced_density"]
+    run(torch.cuda.Stream(), res, "again")
+    assert np.array_equal(res["again"][0], res["alone"][0]) and np.array_equal(res["again"][1], res["alone"][1])
+    threads = [threading.Thread(target=run, args=(torch.cuda.Stream(), res, k)) for k in ("a", "b")]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=600)
+    for k in ("a", "b"):
+        assert np.array_equal(res[k][0], res["alone"][0]) and np.array_equal(res[k][1], res["alone"][1])
+    assert np.all(np.isfinite(res["alone"][0])) and np.array_equal(res["alone"][1], res["alone"][1].T)
