@@ -662,8 +662,8 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
       // ---- epilogue of a complete tile ----
       // Every element is finished (D stored, Z1 / Z2 read, updated and stored) before the next one is touched: one
       // dependent L2 round trip per read-modify-write, 70 % of the DMMA pipe against 91 % without Z.  The Taylor chain
-      // therefore no longer accumulates here (rt_api.cu enqueue_expm keeps the powers); the commutator series and the
-      // row-sharded propagator still do.
+      // therefore no longer accumulates here (rt_api.cu enqueue_expm / enqueue_shard_B keep the powers); the commutator
+      // series still does.
       const bool diag = ga.sym && i0 == j0;
 #pragma unroll
       for (int a = 0; a < FA; ++a) {

@@ -554,8 +554,9 @@ void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, d
 // cos / sinc series from the stored powers of Y = X^2:  C = 1 + sum_k c_k Y^k,  Sc = 1 + sum_k s_k Y^k  (k = 1..q), summed
 // in the order k = 1, 2, ... -- the same order, and the same operations, as series_init_kernel followed by the
 // read-modify-write accumulation in the GEMM epilogues that this kernel replaces.
-__global__ void series_combine_kernel(int N, int ldn, SeriesArgs a, double* __restrict__ C, double* __restrict__ S) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+__global__ void series_combine_kernel(int N, int ldn, SeriesArgs a, double* __restrict__ C, double* __restrict__ S,
+                                      int row_beg) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = row_beg + blockIdx.y;
   if (j >= N) return;
   const long long o = (long long)i * ldn + j;
   const double d = (i == j) ? 1.0 : 0.0;
@@ -570,8 +571,10 @@ __global__ void series_combine_kernel(int N, int ldn, SeriesArgs a, double* __re
   C[o] = cv;
   S[o] = sv;
 }
-void launch_series_combine(int N, int ldn, const SeriesArgs& a, double* C, double* S, cudaStream_t st) {
-  series_combine_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, ldn, a, C, S);
+void launch_series_combine(int N, int ldn, const SeriesArgs& a, double* C, double* S, int row_beg, int row_end,
+                           cudaStream_t st) {
+  if (row_end <= row_beg) return;
+  series_combine_kernel<<<dim3((N + 127) / 128, row_end - row_beg), 128, 0, st>>>(N, ldn, a, C, S, row_beg);
 }
 
 // Line 28 shifts H-1 <- H0 and H0 <- H1 in ONE launch, so H0 is both a source and a destination: no __restrict__

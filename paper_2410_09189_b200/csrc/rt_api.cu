@@ -360,7 +360,7 @@ void enqueue_expm(rt_ctx* c) {
       sa.pw[k - 1] = cur;
       prev = cur;
     }
-    launch_series_combine(c->N, c->ldn, sa, c->Cm, c->Sc, c->st);
+    launch_series_combine(c->N, c->ldn, sa, c->Cm, c->Sc, 0, c->N, c->st);
     c->launches += 1;
     enqueue_gemm(c, 1, c->X, c->Sc, 1.0, nullptr, nullptr, 0, c->Sm);
     return;
@@ -411,6 +411,29 @@ void enqueue_shard_A(rt_ctx* c, int it) {
 }
 void enqueue_shard_B(rt_ctx* c) {
   stage_begin(c, RT_STAGE_ELDYN);
+  if (c->q >= 2 && (int)c->pw_extra.size() >= c->q - 3 && c->q <= SERIES_MAX_Q) {
+    // stored powers (see enqueue_expm): the rank's row block of every power, then the series on those rows
+    SeriesArgs sa{};
+    sa.q = c->q;
+    sa.pw[0] = c->Ya;
+    sa.c[0] = -0.5; sa.s[0] = -1.0 / 6.0;
+    const double* prev = c->Ya;
+    for (int k = 2; k <= c->q; ++k) {
+      sa.c[k - 1] = -sa.c[k - 2] / ((2.0 * k - 1.0) * (2.0 * k));
+      sa.s[k - 1] = -sa.s[k - 2] / ((2.0 * k) * (2.0 * k + 1.0));
+      double* cur = k == 2 ? c->Yb : (k == 3 ? c->Yc : c->pw_extra[k - 4]);
+      enqueue_gemm(c, 0, prev, c->Ya, 1.0, nullptr, nullptr, 0, cur, nullptr, 0, nullptr, 0, nullptr, true);
+      sa.pw[k - 1] = cur;
+      prev = cur;
+    }
+    launch_series_combine(c->N, c->ldn, sa, c->Cm, c->Sc, c->row_beg, c->row_end, c->st);
+    c->launches += 1;
+    enqueue_gemm(c, 0, c->Sc, c->X, 1.0, nullptr, nullptr, 0, c->Sm, nullptr, 0, nullptr, 0, nullptr, true);   // S = Sc X (commute)
+    enqueue_gemm(c, 0, c->Cm, c->P0r, 1.0, c->Sm, c->P0i, -1.0, c->Yb, nullptr, 0, nullptr, 0, nullptr, true);
+    enqueue_gemm(c, 0, c->Cm, c->P0i, -1.0, c->Sm, c->P0r, -1.0, c->Yc, nullptr, 0, nullptr, 0, nullptr, true);
+    stage_end(c);
+    return;
+  }
   launch_series_init(c->N, c->ldn, c->Ya, c->Cm, -0.5, c->Sc, -1.0 / 6.0, c->st);    // elementwise on the whole matrix
   c->launches += 1;
   double ck = -0.5, sk = -1.0 / 6.0;
@@ -1036,7 +1059,7 @@ int create_impl(const rt_config* cfg, const double* phi, const double* eps, cons
                      &c->P0r, &c->P0i, &c->P1r, &c->P1i};
   for (double** mp : mats) { ALLOC(*mp, nn); CKC(cudaMemsetAsync(*mp, 0, nn * 8, c->st)); }
   ALLOC(c->W, (size_t)c->pp.S * N * ldn);
-  if (c->prop == RT_PROP_TAYLOR && !c->general && c->nshard <= 1 && c->q >= 4 && c->q <= SERIES_MAX_Q) {
+  if (c->prop == RT_PROP_TAYLOR && !c->general && c->q >= 4 && c->q <= SERIES_MAX_Q) {
     // the higher powers of Y, when they fit next to everything else with 2 GB to spare (else the products accumulate)
     size_t fb = 0, tb = 0;
     if (cudaMemGetInfo(&fb, &tb) == cudaSuccess && (double)fb > (double)(c->q - 3) * nn * 8 + 2.0e9) {

@@ -133,7 +133,8 @@ void launch_series_init(int N, int ldn, const double* Y, double* C, double c1, d
 // C = 1 + sum_k c[k-1] Y^k, S = 1 + sum_k s[k-1] Y^k, k = 1..q, from the stored powers pw[k-1] = Y^k
 constexpr int SERIES_MAX_Q = 12;
 struct SeriesArgs { const double* pw[SERIES_MAX_Q]; double c[SERIES_MAX_Q], s[SERIES_MAX_Q]; int q; };
-void launch_series_combine(int N, int ldn, const SeriesArgs& a, double* C, double* S, cudaStream_t st);
+void launch_series_combine(int N, int ldn, const SeriesArgs& a, double* C, double* S, int row_beg, int row_end,
+                           cudaStream_t st);    // rows [row_beg, row_end) only (a rank's block of the sharded propagator)
 // dst = src for n matrices (state shift, line 28)
 void launch_copy5(int N, int ldn, double* d0, const double* s0, double* d1, const double* s1, double* d2,
                   const double* s2, double* d3, const double* s3, cudaStream_t st);

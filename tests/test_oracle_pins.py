@@ -287,6 +287,29 @@ def test_zero_field_is_stationary(tiny_inputs):
     assert np.max(np.abs(o.P0 - np.diag(o.occ))) < 1e-13
 
 
+def test_hartree_warm_start_continues_the_iteration(tiny_inputs):
+    """DESIGN R6: every Poisson solve starts from the previous solve's potential.  Multigrid with a fixed cycle count is
+    a stationary linear iteration u <- M u + N f, so for a density held fixed the warm-started potential after k
+    `delta_v` calls of c cycles each must be (i) the potential of ONE solve with k c cycles from zero -- the iteration
+    simply goes on -- and therefore (ii) k c cycles close to the exact potential of the 7-point operator (FFT solve),
+    where a cold start would stay c cycles away for ever.  (Round 1 left this reading pinned by its definition only.)"""
+    w = tiny_inputs[0]
+    o = _make(tiny_inputs, E0=(0, 0, 0))
+    rng = np.random.default_rng(11)
+    rho = o.rho0 * (1.0 + 0.05 * rng.standard_normal(o.rho0.shape))           # a fixed perturbed density
+    drho = rho - o.rho0
+    exact = O.spectral_solve((4 * np.pi * (drho - drho.mean())).reshape(w.shape), w.h).reshape(-1)
+    c = o.n_vc
+    errs = []
+    for k in range(1, 5):
+        dv = o.delta_v(rho)
+        one_go = O.hartree_mg(np.zeros_like(drho), drho, w.shape, w.h, k * c)
+        assert np.array_equal(o.VH, one_go)                                    # (i), bit for bit: same operations
+        assert np.max(np.abs(dv - (o.VH + O.vxc_lda(rho) - o.vxc0))) < 1e-14
+        errs.append(np.max(np.abs(o.VH - exact)) / np.max(np.abs(exact)))
+    assert errs[3] < 0.45 ** (3 * c) * errs[0] and errs[3] < 0.02 * errs[0]    # (ii): keeps contracting call after call
+
+
 def test_invariants_after_kick(tiny_inputs):
     w = tiny_inputs[0]
     o = _make(tiny_inputs, E0=(0.1, 0, 0))
