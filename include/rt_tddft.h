@@ -302,6 +302,23 @@ int rt_spectrum(const double* mu, int32_t nt, double dt, double t_kick, const do
 int rt_spectrum_kick(const double* mu, int32_t nt, double dt, const double E_kick[3], double gamma, const double* omega,
                      int32_t nw, double* S, int32_t device, void* stream);
 
+/* ---- an entry point that allocates nothing --------------------------------------------------------------------
+ * a6 (Alg. 1 line 27: mu = dVol sum_r r rho(r), charge = dVol sum_r rho(r)) of a density that is already
+ * on the device, for callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops, harnesses
+ * that forbid it): no handle, no cudaMalloc / cudaFree / allocating library call inside.  The block partial sums of
+ * the two-stage reduction live in ONE file-scope device array (160 KB, held by every GPU that loads the library until
+ * the process exits), which bounds the grid: nx*ny*nz <= RT_NOALLOC_MAX_POINTS, larger grids are refused with RT_EINVAL
+ * and the limit in rt_last_error(NULL).
+ * rho: [nx*ny*nz] DEVICE, read only.  out: DEVICE double[5], written = { mu_x, mu_y, mu_z, dVol sum rho, dVol sum |rho| }
+ * with the centred coordinates of this library (x(i) = (i - (nx-1)/2) h, DESIGN R4) and dVol = h^3.
+ * Enqueues two kernels on `stream` (cudaStream_t) of `device` and returns without synchronising (RT_ECUDA if a launch
+ * is refused).  Nothing in the scratch needs clearing between calls (every partial that is read was written by the
+ * same call), but ALL calls share it -- from any thread, stream or handle of the process: two calls that overlap on the
+ * GPU race on it and both results are undefined.  Serialise them (same stream, or an event between the streams). */
+#define RT_NOALLOC_MAX_POINTS 4194304
+int rt_dipole_noalloc(const double* rho, int32_t nx, int32_t ny, int32_t nz, double h, double* out, int32_t device,
+                      void* stream);
+
 /* ---- calibration instrument (not on the hot path) ----------------------------------------------------
  * Measures the FP64 issue-rate ceilings of `device` with register-resident operands: DMMA.8x8x4 (mma.sync
  * m8n8k4 f64) and DFMA, in TFLOP/s (HOST doubles).  Takes ~0.5 s.  The roofline fractions bench.py reports for

@@ -29,6 +29,7 @@ SYMBOLS = (
     "rt_destroy", "rt_op_project", "rt_op_density", "rt_op_propagate", "rt_op_hartree", "rt_op_vxc",
     "rt_timing_enable", "rt_timing_read", "rt_probe_fp64_peak", "rt_get_convergence",
     "rt_slab_get_buffers", "rt_slab_phase", "rt_slab_get_shard", "rt_slab_more_updates", "rt_get_dipole_series", "rt_spectrum", "rt_spectrum_kick", "rt_get_energy", "rt_state_bytes", "rt_get_state", "rt_set_state",
+    "rt_dipole_noalloc",
 )
 
 RT_SLAB_INIT, RT_SLAB_PROPAGATE, RT_SLAB_POTENTIAL, RT_SLAB_SHIFT = 0, 1, 2, 3
@@ -98,6 +99,7 @@ def _load():
         "rt_state_bytes": [vp, i64p], "rt_get_state": [vp, vp], "rt_set_state": [vp, vp],
         "rt_spectrum": [dp, i32, C.c_double, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
         "rt_spectrum_kick": [dp, i32, C.c_double, dp, C.c_double, dp, i32, dp, i32, vp],
+        "rt_dipole_noalloc": [dp, i32, i32, i32, C.c_double, dp, i32, vp],
     }
     for name, argtypes in sig.items():
         fn = getattr(lib, name)
@@ -327,6 +329,22 @@ def rt_spectrum(mu, dt, t_kick, kappa, gamma, omega, device=0, stream=0, out=Non
     k = np.ascontiguousarray(kappa, dtype=np.float64)
     rc = _lib.rt_spectrum(_ptr(mu), nt, float(dt), float(t_kick), _ptr(k), float(gamma), _ptr(omega), nw, _ptr(out),
                           int(device), int(stream) if stream else None)
+    _check(None, rc)
+    return out
+
+
+RT_NOALLOC_MAX_POINTS = 4194304
+
+
+def rt_dipole_noalloc(rho, shape, h, out, device=0, stream=0):
+    """a6 on a static device scratch array: no handle, no allocation (include/rt_tddft.h).  rho: CUDA tensor [nx*ny*nz],
+    out: CUDA tensor [5] = (mu_x, mu_y, mu_z, charge, dVol sum |rho|).  Enqueues on `stream` and does NOT synchronise;
+    calls that overlap on the GPU race on the shared scratch."""
+    for t in (rho, out):
+        if not (hasattr(t, "is_cuda") and t.is_cuda):
+            raise ValueError("rt_dipole_noalloc takes device tensors")
+    rc = _lib.rt_dipole_noalloc(_ptr(rho), int(shape[0]), int(shape[1]), int(shape[2]), float(h), _ptr(out), int(device),
+                                int(stream) if stream else None)
     _check(None, rc)
     return out
 

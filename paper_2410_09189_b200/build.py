@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librt_tddft.so")
-SOURCES = ["gemm_kernels.cu", "gemm_tma.cu", "grid_kernels.cu", "mg_kernels.cu", "rt_api.cu", "fp64_probe.cu"]
+SOURCES = ["gemm_kernels.cu", "gemm_tma.cu", "grid_kernels.cu", "mg_kernels.cu", "rt_api.cu", "fp64_probe.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

@@ -1929,6 +1929,19 @@ int rt_spectrum_kick(const double* mu, int32_t nt, double dt, const double E_kic
   return rt_spectrum(mu, nt, dt, 0.5 * dt, kappa, gamma, omega, nw, S, device, stream);
 }
 
+int rt_dipole_noalloc(const double* rho, int32_t nx, int32_t ny, int32_t nz, double h, double* out, int32_t device,
+                      void* stream) {
+  if (!rho || !out || nx < 1 || ny < 1 || nz < 1 || !(h > 0.0))
+    return fail(nullptr, RT_EINVAL, "rt_dipole_noalloc: bad argument");
+  static_assert(RT_NOALLOC_MAX_POINTS == 4096LL * 1024LL, "header limit and noalloc.cu disagree");
+  if (dipole_noalloc_max_points() != RT_NOALLOC_MAX_POINTS)
+    return fail(nullptr, RT_EINVAL, "rt_dipole_noalloc: header limit and library limit disagree");
+  std::string err;
+  const int rc = launch_dipole_noalloc(rho, nx, ny, nz, h, out, device, reinterpret_cast<cudaStream_t>(stream), &err);
+  if (rc != RT_OK) return fail(nullptr, rc, err);
+  return RT_OK;
+}
+
 int rt_timing_enable(rt_handle c, int32_t enable) {
   CHECK_HANDLE(c);
   c->timing = enable != 0;

@@ -1,6 +1,7 @@
 // rt_internal.h -- launcher prototypes shared between the kernel translation units and rt_api.cu.
 // Not part of the public ABI (that is include/rt_tddft.h).
 #pragma once
+#include <string>
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -223,5 +224,10 @@ int launch_mg_solve(const MgSolveArgs& s, cudaStream_t st);
 int launch_mg_solve_order4(const MgSolveArgs& s, const MgLevel& dl0, double* f4, cudaStream_t st);
 // block sums of drho for rt_op_hartree (mean removal): sums[4] = sum(drho)
 void launch_sum_only(const double* v, long long n, double* bsums, double* sums, cudaStream_t st);
+
+// ---- noalloc.cu: the a6 reduction on a static device scratch array (no allocation, no handle) ----
+long long dipole_noalloc_max_points();
+int launch_dipole_noalloc(const double* rho, int nx, int ny, int nz, double h, double* out, int device, cudaStream_t st,
+                          std::string* err);
 
 }  // namespace rt
