@@ -660,35 +660,84 @@ gemm_abt_tma_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_const
       }
 
       // ---- epilogue of a complete tile ----
-      // Every element is finished (D stored, Z1 / Z2 read, updated and stored) before the next one is touched: one
-      // dependent L2 round trip per read-modify-write, 70 % of the DMMA pipe against 91 % without Z.  The Taylor chain
-      // therefore no longer accumulates here (rt_api.cu enqueue_expm / enqueue_shard_B keep the powers); the commutator
-      // series still does.
+      // Products without Z1 / Z2 (the whole Taylor path: rt_api.cu enqueue_expm / enqueue_shard_B keep the powers of Y
+      // instead of accumulating) store element by element.  Products that accumulate (the commutator series: P1 += dP^(k))
+      // read Z1 / Z2 for a batch of 2 x 2 fragments first and store afterwards: D, Z1, Z2 are plain pointers that may
+      // alias as far as the compiler knows, so element-wise `Z[o] += ...` statements serialise into one dependent L2 round
+      // trip each (ncu, N = 2,400: 70 % of the DMMA pipe against 91 % for the same product without Z).  Every element and
+      // every mirror image is touched by exactly one thread, once, so the batching changes no value.  (This version first
+      // ran in round 2 BEFORE the stage-release race of tma_core.cuh was understood: it returned the consumers to the
+      // main loop early enough to hit that race, was blamed for it and taken out; with release_stage in place it is
+      // bit-reproducible -- tests/test_gpu_api_contract.py.)
       const bool diag = ga.sym && i0 == j0;
+      const bool hasZ1 = ga.Z1 != nullptr, hasZ2 = ga.Z2 != nullptr;
+      if (!hasZ1 && !hasZ2) {
 #pragma unroll
-      for (int a = 0; a < FA; ++a) {
-        const int row = i0 + wrow + 8 * a + pg;
-        if (row < N) {
+        for (int a = 0; a < FA; ++a) {
+          const int row = i0 + wrow + 8 * a + pg;
+          if (row < N) {
 #pragma unroll
-          for (int b = 0; b < FB; ++b) {
+            for (int b = 0; b < FB; ++b) {
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-              const int col = j0 + wcol + 8 * b + c + 4 * e;
-              if (col < N && (!diag || col >= row)) {
-                const long long o = (long long)row * ldn + col;
-                double d = fin * acc[a][b][e];
-                if (ga.sym < 0 && row == col) d = 0.0;
-                if (ga.D) ga.D[o] = d;
-                if (ga.Z1) ga.Z1[o] += ga.beta1 * d;
-                if (ga.Z2) ga.Z2[o] += ga.beta2 * d;
-                if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
-                  const long long om = (long long)col * ldn + row;
-                  const double dm = msign * d;
-                  if (ga.D) ga.D[om] = dm;
-                  if (ga.Z1) ga.Z1[om] += ga.beta1 * dm;
-                  if (ga.Z2) ga.Z2[om] += ga.beta2 * dm;
+              for (int e = 0; e < 2; ++e) {
+                const int col = j0 + wcol + 8 * b + c + 4 * e;
+                if (col < N && (!diag || col >= row)) {
+                  const long long o = (long long)row * ldn + col;
+                  double d = fin * acc[a][b][e];
+                  if (ga.sym < 0 && row == col) d = 0.0;
+                  if (ga.D) ga.D[o] = d;
+                  if (ga.sym && row != col && ga.D) ga.D[(long long)col * ldn + row] = msign * d;   // mirror image
                 }
               }
+            }
+          }
+        }
+      } else {
+#pragma unroll
+        for (int a = 0; a < FA; ++a) {
+          const int row = i0 + wrow + 8 * a + pg;
+          if (row < N) {
+#pragma unroll
+            for (int bb = 0; bb < FB; bb += 2) {
+              double z1[2][2], z2[2][2], z1m[2][2], z2m[2][2];
+#pragma unroll
+              for (int b = 0; b < 2; ++b)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                  const int col = j0 + wcol + 8 * (bb + b) + c + 4 * e;
+                  z1[b][e] = z2[b][e] = z1m[b][e] = z2m[b][e] = 0.0;
+                  if (col < N && (!diag || col >= row)) {
+                    const long long o = (long long)row * ldn + col;
+                    if (hasZ1) z1[b][e] = ga.Z1[o];
+                    if (hasZ2) z2[b][e] = ga.Z2[o];
+                    if (ga.sym && row != col) {
+                      const long long om = (long long)col * ldn + row;
+                      if (hasZ1) z1m[b][e] = ga.Z1[om];
+                      if (hasZ2) z2m[b][e] = ga.Z2[om];
+                    }
+                  }
+                }
+#pragma unroll
+              for (int b = 0; b < 2; ++b)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                  const int col = j0 + wcol + 8 * (bb + b) + c + 4 * e;
+                  if (col < N && (!diag || col >= row)) {
+                    const long long o = (long long)row * ldn + col;
+                    double d = fin * acc[a][bb + b][e];
+                    if (ga.sym < 0 && row == col) d = 0.0;
+                    if (ga.D) ga.D[o] = d;
+                    if (hasZ1) ga.Z1[o] = z1[b][e] + ga.beta1 * d;
+                    if (hasZ2) ga.Z2[o] = z2[b][e] + ga.beta2 * d;
+                    if (ga.sym && row != col) {            // mirror image (exactly (anti)symmetric output)
+                      const long long om = (long long)col * ldn + row;
+                      const double dm = msign * d;
+                      if (ga.D) ga.D[om] = dm;
+                      if (hasZ1) ga.Z1[om] = z1m[b][e] + ga.beta1 * dm;
+                      if (hasZ2) ga.Z2[om] = z2m[b][e] + ga.beta2 * dm;
+                    }
+                  }
+                }
             }
           }
         }

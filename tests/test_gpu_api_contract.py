@@ -151,8 +151,8 @@ def test_spectrum_kick_forms_the_impulse_inside_the_library(B):
     assert np.max(np.abs(S - ref)) < 1e-12 * np.max(np.abs(ref))
 
 
-@pytest.mark.parametrize("N", [2400, 5000])
-def test_propagator_is_bit_reproducible_and_accurate(B, N):
+@pytest.mark.parametrize("N,propagator", [(2400, "taylor"), (5000, "taylor"), (5000, "commutator")])
+def test_propagator_is_bit_reproducible_and_accurate(B, N, propagator):
     """The stream-K N x N GEMMs fix their summation order by (N, #SMs) alone: the same propagation, run four times through
     rt_op_propagate, must give the same bits (a round-2 epilogue variant that batched the read-modify-writes of the series
     accumulators failed exactly this at N >= 5,000 while staying within 1e-9 of the right answer), and the right answer:
@@ -166,7 +166,11 @@ def test_propagator_is_bit_reproducible_and_accurate(B, N):
     eps = np.sort(rng.uniform(-0.5, 0.3, N))
     occ = np.zeros(N)
     occ[: (5 * N) // 6] = 2.0
-    sim = B.RTTDDFT((16, 16, 16), 0.4, phi, eps, occ, 0.2, E0=(0.05, 0.0, 0.0), n_hupdates=1, n_vcycles=1)
+    # "commutator": the paper's series (Eq. 39), whose GEMMs accumulate P1 += dP^(k) in their epilogues (batched
+    # read-modify-writes); it stops at max|dP^(k)| <= 1e-10, so its distance to the exact result is a few 1e-10
+    sim = B.RTTDDFT((16, 16, 16), 0.4, phi, eps, occ, 0.2, E0=(0.05, 0.0, 0.0), n_hupdates=1, n_vcycles=1,
+                    propagator=propagator)
+    tol = 1e-11 if propagator == "taylor" else 2e-9
     assert sim.info()["tma"]
     A = torch.randn(N, N, dtype=torch.float64, device="cuda", generator=gen) * 2e-3
     H = torch.diag(torch.from_numpy(eps).cuda()) + 0.5 * (A + A.T)
@@ -182,8 +186,8 @@ def test_propagator_is_bit_reproducible_and_accurate(B, N):
     U = torch.linalg.matrix_exp((-0.2j) * H.to(torch.complex128))
     Pref = (U * torch.from_numpy(occ).cuda().to(torch.complex128)[None, :]) @ U.conj().T
     P1 = torch.from_numpy(outs[0][0]).cuda() + 1j * torch.from_numpy(outs[0][1]).cuda()
-    assert float((P1 - Pref).abs().max()) < 1e-11
-    assert float((P1 @ P1 - 2 * P1).abs().max()) < 1e-11
+    assert float((P1 - Pref).abs().max()) < tol
+    assert float((P1 @ P1 - 2 * P1).abs().max()) < 4 * tol
     sim.close()
 
 
